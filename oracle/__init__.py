@@ -1,0 +1,140 @@
+"""CPU oracle (float64) for the matched-filter trajectory search -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product
+(``paper_2209_09848_b200``) never does, and this package never imports the product.
+
+The arithmetic lives in ``tno_oracle.c`` (plain C, float64, one exp per tap in ``point``); this
+file only marshals numpy arrays.  ``topk`` is the plain definition: threshold, then a library
+sort by (SNR descending, y ascending, x ascending) -- BASELINE.json:north_star "per-trajectory
+top-K candidate list above a threshold".
+
+Pins: tests/test_oracle_pins.py.  No function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+from typing import Optional, Tuple
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = ctypes.CDLL(_build())
+_f32p = ctypes.POINTER(ctypes.c_float)
+_f64p = ctypes.POINTER(ctypes.c_double)
+_i32p = ctypes.POINTER(ctypes.c_int)
+
+_lib.tno_oracle_threads.restype = ctypes.c_int
+_lib.tno_oracle_point.restype = ctypes.c_int
+_lib.tno_oracle_point.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, ctypes.c_float,
+                                  ctypes.c_float, ctypes.c_int, ctypes.c_int, _f64p, _f64p, _f64p]
+_lib.tno_oracle_map.restype = ctypes.c_int
+_lib.tno_oracle_map.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, ctypes.c_int,
+                                ctypes.c_float, ctypes.c_float] + [ctypes.c_int] * 4 + [_f64p] * 3
+_lib.tno_oracle_inject.restype = ctypes.c_int
+_lib.tno_oracle_inject.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f32p, _i32p,
+                                   _i32p, _f32p, ctypes.c_int, ctypes.c_float, ctypes.c_float]
+
+CAND_DTYPE = np.dtype([("snr", np.float64), ("x", np.int32), ("y", np.int32), ("k", np.int32)])
+
+
+def threads() -> int:
+    return int(_lib.tno_oracle_threads())
+
+
+def _f32(a, shape=None) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    if shape is not None:
+        assert a.shape == shape, (a.shape, shape)
+    return a
+
+
+def _geom(frames: np.ndarray, window, full_shape):
+    T, wh, ww = frames.shape
+    if window is None:
+        assert full_shape is None or tuple(full_shape) == (wh, ww)
+        return T, wh, ww, 0, 0, ww, wh
+    wx0, wy0 = window
+    H, W = full_shape
+    return T, H, W, int(wx0), int(wy0), ww, wh
+
+
+def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=None
+          ) -> Tuple[float, float, float]:
+    """(snr, N, D) at start pixel (x, y) for one trajectory (vx, vy, ax, ay)."""
+    frames = _f32(frames)
+    T, H, W, wx0, wy0, ww, wh = _geom(frames, window, full_shape)
+    sigma_t = _f32(sigma_t, (T,))
+    traj = _f32(traj, (4,))
+    N, D, S = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    rc = _lib.tno_oracle_point(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
+                               sigma_t.ctypes.data_as(_f32p), traj.ctypes.data_as(_f32p),
+                               float(prf_sigma), float(t0), int(x), int(y),
+                               ctypes.byref(N), ctypes.byref(D), ctypes.byref(S))
+    if rc != 0:
+        raise ValueError("oracle.point: tap outside the supplied window (rc=%d)" % rc)
+    return S.value, N.value, D.value
+
+
+def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, full_shape=None,
+            return_ND: bool = False):
+    """float64 [K, h, w] SNR for start pixels x in [x_lo, x_hi), y in [y_lo, y_hi)
+    (region = (x_lo, x_hi, y_lo, y_hi), default the whole frame)."""
+    frames = _f32(frames)
+    T, H, W, wx0, wy0, ww, wh = _geom(frames, window, full_shape)
+    sigma_t = _f32(sigma_t, (T,))
+    trajs = _f32(trajs)
+    assert trajs.ndim == 2 and trajs.shape[1] == 4
+    K = trajs.shape[0]
+    x_lo, x_hi, y_lo, y_hi = (0, W, 0, H) if region is None else region
+    out = np.empty((K, y_hi - y_lo, x_hi - x_lo), dtype=np.float64)
+    oN = np.empty_like(out) if return_ND else None
+    oD = np.empty_like(out) if return_ND else None
+    rc = _lib.tno_oracle_map(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
+                             sigma_t.ctypes.data_as(_f32p), trajs.ctypes.data_as(_f32p), K,
+                             float(prf_sigma), float(t0), int(x_lo), int(x_hi), int(y_lo),
+                             int(y_hi), out.ctypes.data_as(_f64p),
+                             oN.ctypes.data_as(_f64p) if return_ND else None,
+                             oD.ctypes.data_as(_f64p) if return_ND else None)
+    if rc != 0:
+        raise ValueError("oracle.snr_map failed (rc=%d): -1 = tap outside the window" % rc)
+    return (out, oN, oD) if return_ND else out
+
+
+def topk(snr: np.ndarray, ktop: int, threshold: float, k_index: int = 0,
+         origin: Tuple[int, int] = (0, 0)) -> np.ndarray:
+    """Candidates of ONE map [h, w]: all pixels with snr >= threshold, ordered by
+    (snr descending, y ascending, x ascending), first `ktop` of them, padded to `ktop` records
+    with (-inf, -1, -1, k)."""
+    snr = np.asarray(snr, dtype=np.float64)
+    ys, xs = np.nonzero(snr >= threshold)
+    vals = snr[ys, xs]
+    order = np.lexsort((xs, ys, -vals))[:ktop]     # last key is the primary one
+    out = np.empty(ktop, dtype=CAND_DTYPE)
+    out["snr"] = -np.inf
+    out["x"] = -1
+    out["y"] = -1
+    out["k"] = k_index
+    n = order.size
+    out["snr"][:n] = vals[order]
+    out["x"][:n] = xs[order] + origin[0]
+    out["y"][:n] = ys[order] + origin[1]
+    return out
+
+
+def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0) -> None:
+    """In place: add amp * g(p - c_t) for each source (full-frame float32 [T, H, W] buffer)."""
+    assert frames.dtype == np.float32 and frames.flags.c_contiguous and frames.ndim == 3
+    T, H, W = frames.shape
+    trajs = _f32(trajs)
+    n = trajs.shape[0]
+    xs = np.ascontiguousarray(xs, dtype=np.int32)
+    ys = np.ascontiguousarray(ys, dtype=np.int32)
+    amps = _f32(amps, (n,))
+    assert xs.shape == (n,) and ys.shape == (n,) and trajs.shape == (n, 4)
+    rc = _lib.tno_oracle_inject(frames.ctypes.data_as(_f32p), T, H, W,
+                                trajs.ctypes.data_as(_f32p), xs.ctypes.data_as(_i32p),
+                                ys.ctypes.data_as(_i32p), amps.ctypes.data_as(_f32p), n,
+                                float(prf_sigma), float(t0))
+    assert rc == 0

@@ -1,0 +1,222 @@
+/*
+ * tno_oracle.c -- TEST INFRASTRUCTURE, not product code.
+ *
+ * Plain, slow, float64 CPU oracle for the matched-filter trajectory search of
+ * Ganapathi, "Maximum Likelihood Systematic Effect Modeling and Matched Filtering to Detect
+ * Trans-Neptunian Objects with TESS" (arXiv 2209.09848).  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may call it.  It shares no code with the
+ * CUDA path under paper_2209_09848_b200/.
+ *
+ * What it computes (BASELINE.json:north_star; the paper's counterpart is Eq. 5, PAPER.md:L110,
+ * "S = D * F", the dot product of the filter with the data at every pixel location, L108, with
+ * the filter F = trajectory line convolved with the pixel response function, L106):
+ *
+ *   for trajectory k = (vx, vy, ax, ay), start pixel (x, y) at the reference epoch t0,
+ *   frames t = 0..T-1:
+ *       dt = t - t0
+ *       dx = vx*dt + ax*dt*dt            dy likewise             displacement in px
+ *       sx = floor(dx + 0.5), phx = dx - sx   (ties go up; phase in [-0.5, 0.5))  DESIGN.md c1
+ *       for j in -2..2, i in -2..2:                              5x5 window at round(c_t)
+ *           px = x + sx + i ; py = y + sy + j
+ *           skip the tap if (px, py) is outside the frame        dropped from N and D
+ *           g  = exp(-((i - phx)^2 + (j - phy)^2) / (2 prf_sigma^2))     peak-1 Gaussian PRF
+ *           N += g * R_t[py][px] / sigma_t^2
+ *           D += g * g / sigma_t^2
+ *   SNR_k(x, y) = N / sqrt(D) if D > 0 else 0
+ *
+ * tno_oracle_point is this literally (one exp per tap).  tno_oracle_map evaluates the same sums
+ * with (sx, sy, gx[i], gy[j]) computed once per (k, t) -- they do not depend on (x, y) -- and
+ * is pinned against tno_oracle_point on small inputs by tests/test_oracle_pins.py.
+ * tno_oracle_inject adds A * g(p - c_t) on the same 25 taps with the same rounding ("signal
+ * injection corresponds to adding a filter times a flux to the raw data").
+ *
+ * Parity pins (tests/test_oracle_pins.py): closed form N/D = A and SNR = A sqrt(D) for an
+ * injected noiseless source; zero in -> zero out; linearity; integer velocities reduce to
+ * scipy.ndimage.correlate + integer shifts; brute force with exact rational displacements;
+ * hand-listed tie cases; corner closed form; N(0,1) statistics on pure noise.
+ *
+ * Inputs are float32 where the C ABI of the product takes float32 (frames, sigma_t, trajectory
+ * parameters, prf_sigma, t0); every value is promoted to double before any arithmetic.
+ * Build: gcc -O2 -fopenmp -ffp-contract=off (no fast-math), see oracle/build.py.
+ *
+ * The frame buffer may be a WINDOW of the full frame: it holds rows [wy0, wy0+wh) and columns
+ * [wx0, wx0+ww) of an H x W frame for each t.  A tap that is inside the frame but outside the
+ * window is an error (return -1): the caller must pass a window with enough halo.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    int T, H, W;            /* full frame geometry */
+    int wx0, wy0, ww, wh;   /* window held by the buffer */
+} geom_t;
+
+static inline double disp(double v, double a, double dt) { return v * dt + a * dt * dt; }
+
+/* round-half-up of a displacement: integer shift s and phase d - s in [-0.5, 0.5) */
+static inline void split(double d, int *s, double *ph) {
+    double f = floor(d + 0.5);
+    *s = (int)f;
+    *ph = d - f;
+}
+
+int tno_oracle_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* literal definition, one exp per tap */
+int tno_oracle_point(const float *frames, int T, int H, int W,
+                     int wx0, int wy0, int ww, int wh,
+                     const float *sigma_t, const float *traj4, float prf_sigma_f, float t0_f,
+                     int x, int y, double *N_out, double *D_out, double *snr_out)
+{
+    const double vx = traj4[0], vy = traj4[1], ax = traj4[2], ay = traj4[3];
+    const double s = prf_sigma_f, t0 = t0_f;
+    double N = 0.0, D = 0.0;
+    for (int t = 0; t < T; ++t) {
+        const double dt = (double)t - t0;
+        int sx, sy; double phx, phy;
+        split(disp(vx, ax, dt), &sx, &phx);
+        split(disp(vy, ay, dt), &sy, &phy);
+        const double sig = sigma_t[t];
+        const double q = 1.0 / (sig * sig);
+        for (int j = -2; j <= 2; ++j) {
+            for (int i = -2; i <= 2; ++i) {
+                const int px = x + sx + i, py = y + sy + j;
+                if (px < 0 || px >= W || py < 0 || py >= H) continue;
+                if (px < wx0 || px >= wx0 + ww || py < wy0 || py >= wy0 + wh) return -1;
+                const double ux = (double)i - phx, uy = (double)j - phy;
+                const double g = exp(-(ux * ux + uy * uy) / (2.0 * s * s));
+                const double R = frames[((size_t)t * wh + (size_t)(py - wy0)) * ww + (size_t)(px - wx0)];
+                N += g * R * q;
+                D += g * g * q;
+            }
+        }
+    }
+    if (N_out) *N_out = N;
+    if (D_out) *D_out = D;
+    if (snr_out) *snr_out = (D > 0.0) ? N / sqrt(D) : 0.0;
+    return 0;
+}
+
+/* same sums, per-(k,t) quantities hoisted out of the pixel loop.
+ * Region of start pixels: x in [x_lo, x_hi), y in [y_lo, y_hi).
+ * out_snr / out_N / out_D: double [K][y_hi-y_lo][x_hi-x_lo]; out_N, out_D may be NULL. */
+int tno_oracle_map(const float *frames, int T, int H, int W,
+                   int wx0, int wy0, int ww, int wh,
+                   const float *sigma_t, const float *traj, int K,
+                   float prf_sigma_f, float t0_f,
+                   int x_lo, int x_hi, int y_lo, int y_hi,
+                   double *out_snr, double *out_N, double *out_D)
+{
+    const double s = prf_sigma_f, t0 = t0_f;
+    const int rw = x_hi - x_lo, rh = y_hi - y_lo;
+    if (rw <= 0 || rh <= 0 || K <= 0 || T <= 0) return -2;
+    int *SX = (int *)malloc(sizeof(int) * (size_t)T * 2);
+    double *G = (double *)malloc(sizeof(double) * (size_t)T * 11);
+    if (!SX || !G) { free(SX); free(G); return -3; }
+    int err = 0;
+    for (int k = 0; k < K; ++k) {
+        const double vx = traj[4 * k + 0], vy = traj[4 * k + 1];
+        const double ax = traj[4 * k + 2], ay = traj[4 * k + 3];
+        for (int t = 0; t < T; ++t) {
+            const double dt = (double)t - t0;
+            int sx, sy; double phx, phy;
+            split(disp(vx, ax, dt), &sx, &phx);
+            split(disp(vy, ay, dt), &sy, &phy);
+            SX[2 * t] = sx; SX[2 * t + 1] = sy;
+            for (int i = -2; i <= 2; ++i) {
+                const double ux = (double)i - phx, uy = (double)i - phy;
+                G[11 * t + (i + 2)] = exp(-(ux * ux) / (2.0 * s * s));
+                G[11 * t + 5 + (i + 2)] = exp(-(uy * uy) / (2.0 * s * s));
+            }
+            const double sig = sigma_t[t];
+            G[11 * t + 10] = 1.0 / (sig * sig);
+        }
+        double *Nk = (double *)calloc((size_t)rw * rh, sizeof(double));
+        double *Dk = (double *)calloc((size_t)rw * rh, sizeof(double));
+        if (!Nk || !Dk) { free(Nk); free(Dk); err = -3; break; }
+#pragma omp parallel for schedule(static) reduction(min : err)
+        for (int y = y_lo; y < y_hi; ++y) {
+            double *Nr = Nk + (size_t)(y - y_lo) * rw;
+            double *Dr = Dk + (size_t)(y - y_lo) * rw;
+            for (int t = 0; t < T; ++t) {
+                const int sx = SX[2 * t], sy = SX[2 * t + 1];
+                const double *gx = G + 11 * t, *gy = G + 11 * t + 5;
+                const double q = G[11 * t + 10];
+                for (int j = -2; j <= 2; ++j) {
+                    const int py = y + sy + j;
+                    if (py < 0 || py >= H) continue;
+                    if (py < wy0 || py >= wy0 + wh) { err = -1; continue; }
+                    const float *row = frames + ((size_t)t * wh + (size_t)(py - wy0)) * ww;
+                    for (int i = -2; i <= 2; ++i) {
+                        const double g = gx[i + 2] * gy[j + 2];
+                        const double wN = g * q, wD = g * g * q;
+                        int xa = x_lo, xb = x_hi;           /* start pixels with px inside the frame */
+                        if (xa + sx + i < 0) xa = -(sx + i);
+                        if (xb + sx + i > W) xb = W - (sx + i);
+                        if (xa >= xb) continue;
+                        if (xa + sx + i < wx0 || xb + sx + i > wx0 + ww) { err = -1; continue; }
+                        const float *src = row + (sx + i - wx0);
+                        for (int x = xa; x < xb; ++x) {
+                            Nr[x - x_lo] += wN * (double)src[x];
+                            Dr[x - x_lo] += wD;
+                        }
+                    }
+                }
+            }
+        }
+        for (size_t p = 0; p < (size_t)rw * rh; ++p) {
+            const double D = Dk[p];
+            out_snr[(size_t)k * rw * rh + p] = (D > 0.0) ? Nk[p] / sqrt(D) : 0.0;
+            if (out_N) out_N[(size_t)k * rw * rh + p] = Nk[p];
+            if (out_D) out_D[(size_t)k * rw * rh + p] = D;
+        }
+        free(Nk); free(Dk);
+        if (err) break;
+    }
+    free(SX); free(G);
+    return err;
+}
+
+/* Injection: for each source, in order, add amp * g(p - c_t) on the 25 taps of
+ * every frame, computed in double and rounded once to float32:
+ *     R <- (float)((double)R + amp * g).
+ * Works on a full-frame buffer [T][H][W].  traj: [n][4] per source. */
+int tno_oracle_inject(float *frames, int T, int H, int W,
+                      const float *traj, const int *xs, const int *ys, const float *amp, int n,
+                      float prf_sigma_f, float t0_f)
+{
+    const double s = prf_sigma_f, t0 = t0_f;
+    for (int m = 0; m < n; ++m) {
+        const double vx = traj[4 * m + 0], vy = traj[4 * m + 1];
+        const double ax = traj[4 * m + 2], ay = traj[4 * m + 3];
+        const double A = amp[m];
+        for (int t = 0; t < T; ++t) {
+            const double dt = (double)t - t0;
+            int sx, sy; double phx, phy;
+            split(disp(vx, ax, dt), &sx, &phx);
+            split(disp(vy, ay, dt), &sy, &phy);
+            for (int j = -2; j <= 2; ++j) {
+                for (int i = -2; i <= 2; ++i) {
+                    const int px = xs[m] + sx + i, py = ys[m] + sy + j;
+                    if (px < 0 || px >= W || py < 0 || py >= H) continue;
+                    const double ux = (double)i - phx, uy = (double)j - phy;
+                    const double g = exp(-(ux * ux + uy * uy) / (2.0 * s * s));
+                    float *p = frames + ((size_t)t * H + (size_t)py) * W + (size_t)px;
+                    *p = (float)((double)*p + A * g);
+                }
+            }
+        }
+    }
+    return 0;
+}
