@@ -1,0 +1,137 @@
+/*
+ * tno_mf.h -- C ABI of the B200 matched-filter trajectory search.
+ *
+ * The operation (BASELINE.json:north_star; paper: Ganapathi, arXiv 2209.09848, section 3.2,
+ * PAPER.md:L104-118, Eq. 5 "S = D * F" at L110, thresholding at L122): for a stack of
+ * background-subtracted residual frames R_t and a bank of trajectory hypotheses k, score every
+ * start pixel (x, y) with the matched filter "trajectory line convolved with the pixel response
+ * function" (L106), evaluated sparsely (the paper's own suggestion of a "sparse convolution CUDA
+ * kernel", L118):
+ *
+ *     c_t  = (x, y) + v (t - t0) + a (t - t0)^2              position at frame t
+ *     N    = sum_t sum_{p in 5x5 window at round(c_t)} g(p - c_t) R_t(p) / sigma_t^2
+ *     D    = sum_t sum_p g(p - c_t)^2 / sigma_t^2            taps outside the frame are
+ *     SNR_k(x, y) = N / sqrt(D),  0 where D = 0              dropped from N and from D
+ *
+ * g(u) = exp(-|u|^2 / (2 prf_sigma^2)) (peak 1, sampled at pixel centres); round() is applied to
+ * the displacement alone, round(c_t) = (x, y) + floor(d_t + 1/2), ties up (readings
+ * c1-c8).  Outputs: the SNR maps and, per trajectory, the top-K pixels with SNR >= threshold
+ * ordered by (SNR descending, y ascending, x ascending).
+ *
+ * Conventions
+ *   - DEVICE pointers are CUDA device memory owned by the caller (e.g. a torch tensor's
+ *     data_ptr()); HOST pointers are ordinary process memory.  Nothing passed in is retained
+ *     after the call returns, and inputs are never written (except tno_mf_inject's frames).
+ *   - tno_mf_search and tno_mf_inject validate on the host, enqueue their work on the context's
+ *     stream and return without synchronising the device; results are valid once the caller
+ *     synchronises that stream.  Host arrays are consumed before return.
+ *   - Every function returns 0 on success or a negative TNO_MF_E* code; no exceptions, no
+ *     exit().  After a failure tno_mf_last_error(ctx) describes it; outputs are unspecified.
+ *   - A context is not thread-safe; distinct contexts are independent.  No global state.
+ *   - There is no CPU fallback: without a CUDA device of compute capability 10.x,
+ *     tno_mf_create fails with TNO_MF_EUNSUPPORTED / TNO_MF_ECUDA.
+ *   - Behaviour for non-finite PIXELS is unspecified (pixels are not scanned).
+ */
+#ifndef TNO_MF_H
+#define TNO_MF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TNO_MF_OK            0
+#define TNO_MF_EINVAL       (-1)   /* bad argument (see each function) */
+#define TNO_MF_ENOMEM       (-2)   /* host or device allocation failed */
+#define TNO_MF_ECUDA        (-3)   /* CUDA runtime/driver error; text in tno_mf_last_error */
+#define TNO_MF_EUNSUPPORTED (-4)   /* device is not sm_100-class, or no device */
+
+typedef struct tno_mf_ctx tno_mf_ctx;                        /* opaque */
+
+/* One trajectory hypothesis: velocity in px/frame, parallax term in px/frame^2
+ * (north_star: "linear (vx,vy) or linear plus parallax term (ax,ay)"). */
+typedef struct { float vx, vy, ax, ay; } tno_mf_traj;
+
+/* One candidate.  Unused tail records are {-INFINITY, -1, -1, k}. */
+typedef struct { float snr; int32_t x, y, k; } tno_mf_cand;  /* 16 bytes */
+
+/* One source to inject: trajectory, start pixel at the reference epoch t0, amplitude in the
+ * frames' flux units. */
+typedef struct { tno_mf_traj traj; int32_t x, y; float amplitude; } tno_mf_source;  /* 28 bytes */
+
+typedef struct {
+    int32_t device;          /* CUDA device ordinal */
+    void   *stream;          /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream);
+                                NULL = the legacy default stream */
+    int32_t topk;            /* K of the per-trajectory candidate list, >= 0; 0 = no list */
+    float   snr_threshold;   /* candidate iff snr >= threshold; -INFINITY disables the cut */
+    int32_t force_generic;   /* 0 = pick the fastest kernel that applies (normal use);
+                                1 = always use the generic (non-TMA) kernel -- for tests */
+    int32_t reserved[3];     /* must be 0 */
+} tno_mf_config;
+
+/* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
+ * reserved != 0), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
+int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
+
+/* The search (formula above).
+ *   frames        DEVICE  float32 [T][H][W], x fastest.  Read only.
+ *   sigma_t       HOST    float32 [T], per-frame noise standard deviation, finite and > 0.
+ *   trajectories  HOST    [n_traj]; finite values.
+ *   prf_sigma     Gaussian PRF width in px, finite and > 0.   t0: reference epoch (frame units).
+ *   out_snr       DEVICE  float32 [n_traj][H][W] (map k at out_snr + k*H*W), or NULL = no maps.
+ *   out_topk      DEVICE  [n_traj][topk] records, or NULL (or topk == 0) = no lists.
+ * Errors: EINVAL (NULL frames/sigma_t/trajectories, T/H/W/n_traj < 1, bad prf_sigma, sigma_t,
+ * trajectory or t0 values, both outputs absent, shapes whose shifts do not fit 32-bit pixel
+ * arithmetic), ENOMEM, ECUDA.
+ * Any H, W >= 1 is computed correctly; the TMA kernel needs W % 4 == 0 and 16-byte aligned
+ * frames, other shapes take the generic kernel.  All element offsets are 64-bit. */
+int tno_mf_search(tno_mf_ctx *ctx,
+                  const float *frames, int32_t T, int32_t H, int32_t W,
+                  const float *sigma_t,
+                  const tno_mf_traj *trajectories, int32_t n_traj,
+                  float prf_sigma, float t0,
+                  float *out_snr,
+                  tno_mf_cand *out_topk);
+
+/* Signal injection ("signal injection corresponds to adding a filter times a flux
+ * to the raw data"): for each source m in order and every frame t,
+ *     R_t(p) <- (float)((double)R_t(p) + amplitude_m * g(p - c_t))  on the 25 window taps,
+ * taps outside the frame skipped.  Deterministic (sources are applied sequentially per frame).
+ *   frames   DEVICE float32 [T][H][W], modified in place.     sources  HOST [n_sources].
+ * Errors: EINVAL, ECUDA. */
+int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W,
+                  const tno_mf_source *sources, int32_t n_sources,
+                  float prf_sigma, float t0);
+
+/* Host-only planning query (no device work; ctx may be NULL): how the search would group
+ * `trajectories` into batches that share one x-motion (vx, ax) -- the unit of work of the
+ * separable kernel.  Writes, for each trajectory, its batch index and slot
+ * within the batch to out_batch[n_traj] / out_slot[n_traj] (either may be NULL) and returns the
+ * number of batches (>= 1), or a negative error.  max_entries: slots per batch (1..16);
+ * max_spread: largest allowed difference of integer y-shifts inside a batch at any frame. */
+int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, float t0,
+                int32_t max_entries, int32_t max_spread,
+                int32_t *out_batch, int32_t *out_slot);
+
+/* Counters of the last tno_mf_search on this context (host values, valid after the call
+ * returns): number of kernel launches enqueued, and which search kernel was used
+ * (0 = generic, 1 = separable TMA kernel).  NULL pointers are skipped. */
+int tno_mf_last_stats(const tno_mf_ctx *ctx, int32_t *out_launches, int32_t *out_kernel);
+
+/* Release the context and its workspace.  The caller must have synchronised the stream.
+ * NULL is accepted. */
+int tno_mf_destroy(tno_mf_ctx *ctx);
+
+/* Text of the last error on this context (or of the last failed tno_mf_create when ctx is
+ * NULL).  Never NULL; valid until the next call on the same context. */
+const char *tno_mf_last_error(const tno_mf_ctx *ctx);
+
+/* Library version string, e.g. "tno_mf 0.1 (sm_100a)". */
+const char *tno_mf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TNO_MF_H */

@@ -1,0 +1,9 @@
+"""B200-native matched-filter trajectory search (hot path of arXiv 2209.09848).
+
+The product is the C-ABI library ``libtno_mf.so`` (CUDA, sm_100a; sources in ``csrc/``, interface
+in ``include/tno_mf.h``).  This package is its thin Python binding plus a small convenience class.
+"""
+from .binding import (CAND_DTYPE, SOURCE_DTYPE, TRAJ_DTYPE, TnoMfError, make_sources,  # noqa: F401
+                      tno_mf_create, tno_mf_destroy, tno_mf_inject, tno_mf_last_error,
+                      tno_mf_last_stats, tno_mf_plan, tno_mf_search, tno_mf_version)
+from .search import MatchedFilter  # noqa: F401

@@ -1,0 +1,166 @@
+"""ctypes binding of libtno_mf.so -- argument marshalling only; every step of the search runs in
+the library's CUDA kernels (include/tno_mf.h).  torch is used for device memory and streams.
+
+The functions carry the names of the C ABI (tno_mf_create, tno_mf_search, tno_mf_inject,
+tno_mf_plan, tno_mf_last_stats, tno_mf_destroy, tno_mf_last_error, tno_mf_version).  There is no
+CPU fallback: loading fails loudly if the library is missing and tno_mf_create fails without an
+sm_100 device.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtno_mf.so")
+
+TNO_MF_OK, TNO_MF_EINVAL, TNO_MF_ENOMEM, TNO_MF_ECUDA, TNO_MF_EUNSUPPORTED = 0, -1, -2, -3, -4
+
+TRAJ_DTYPE = np.dtype([("vx", np.float32), ("vy", np.float32), ("ax", np.float32), ("ay", np.float32)])
+CAND_DTYPE = np.dtype([("snr", np.float32), ("x", np.int32), ("y", np.int32), ("k", np.int32)])
+SOURCE_DTYPE = np.dtype([("vx", np.float32), ("vy", np.float32), ("ax", np.float32), ("ay", np.float32),
+                         ("x", np.int32), ("y", np.int32), ("amplitude", np.float32)])
+assert TRAJ_DTYPE.itemsize == 16 and CAND_DTYPE.itemsize == 16 and SOURCE_DTYPE.itemsize == 28
+
+
+class tno_mf_config(ctypes.Structure):
+    _fields_ = [("device", ctypes.c_int32), ("stream", ctypes.c_void_p), ("topk", ctypes.c_int32),
+                ("snr_threshold", ctypes.c_float), ("force_generic", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 3)]
+
+
+class TnoMfError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__("tno_mf error %d: %s" % (code, text))
+        self.code = code
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s is missing: build it with `python -m paper_2209_09848_b200.build` "
+            "(nvcc, sm_100a).  There is no CPU fallback." % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_float
+    lib.tno_mf_create.restype = ctypes.c_int
+    lib.tno_mf_create.argtypes = [ctypes.POINTER(tno_mf_config), ctypes.POINTER(vp)]
+    lib.tno_mf_search.restype = ctypes.c_int
+    lib.tno_mf_search.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_inject.restype = ctypes.c_int
+    lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
+    lib.tno_mf_plan.restype = ctypes.c_int
+    lib.tno_mf_plan.argtypes = [vp, i32, i32, f32, i32, i32, vp, vp]
+    lib.tno_mf_last_stats.restype = ctypes.c_int
+    lib.tno_mf_last_stats.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32)]
+    lib.tno_mf_destroy.restype = ctypes.c_int
+    lib.tno_mf_destroy.argtypes = [vp]
+    lib.tno_mf_last_error.restype = ctypes.c_char_p
+    lib.tno_mf_last_error.argtypes = [vp]
+    lib.tno_mf_version.restype = ctypes.c_char_p
+    lib.tno_mf_version.argtypes = []
+    return lib
+
+
+_lib = _load()
+
+
+def _check(rc: int, ctx) -> None:
+    if rc != 0:
+        raise TnoMfError(rc, _lib.tno_mf_last_error(ctx).decode())
+
+
+def tno_mf_version() -> str:
+    return _lib.tno_mf_version().decode()
+
+
+def tno_mf_last_error(ctx=None) -> str:
+    return _lib.tno_mf_last_error(ctx).decode()
+
+
+def tno_mf_create(device: int = 0, stream: Optional[int] = None, topk: int = 0,
+                  snr_threshold: float = float("-inf"), force_generic: bool = False):
+    """Returns an opaque context handle.  `stream` is a raw cudaStream_t (int) or None."""
+    cfg = tno_mf_config(device=int(device), stream=ctypes.c_void_p(stream or 0), topk=int(topk),
+                        snr_threshold=float(snr_threshold), force_generic=int(bool(force_generic)))
+    ctx = ctypes.c_void_p()
+    _check(_lib.tno_mf_create(ctypes.byref(cfg), ctypes.byref(ctx)), None)
+    return ctx
+
+
+def tno_mf_destroy(ctx) -> None:
+    _check(_lib.tno_mf_destroy(ctx), None)
+
+
+def _traj_array(trajectories) -> np.ndarray:
+    a = np.ascontiguousarray(trajectories, dtype=np.float32)
+    if a.ndim != 2 or a.shape[1] != 4:
+        raise ValueError("trajectories must be [n, 4] (vx, vy, ax, ay)")
+    return a
+
+
+def tno_mf_search(ctx, frames, sigma_t, trajectories, prf_sigma: float, t0: float,
+                  out_snr=None, out_topk=None) -> None:
+    """frames: CUDA float32 tensor [T, H, W] (contiguous); sigma_t: host float32 [T];
+    trajectories: host [n, 4]; out_snr: CUDA float32 tensor [n, H, W] or None; out_topk: CUDA
+    uint8/int32 tensor with n*topk*16 bytes or None.  Enqueues on the context's stream."""
+    assert frames.is_cuda and frames.dtype.is_floating_point and frames.element_size() == 4
+    assert frames.is_contiguous() and frames.dim() == 3
+    T, H, W = frames.shape
+    sig = np.ascontiguousarray(sigma_t, dtype=np.float32)
+    if sig.shape != (T,):
+        raise ValueError("sigma_t must have shape [T]")
+    tr = _traj_array(trajectories)
+    n = tr.shape[0]
+    p_snr = None
+    if out_snr is not None:
+        assert out_snr.is_cuda and out_snr.is_contiguous() and out_snr.element_size() == 4
+        assert out_snr.numel() == n * H * W
+        p_snr = out_snr.data_ptr()
+    p_top = None
+    if out_topk is not None:
+        assert out_topk.is_cuda and out_topk.is_contiguous()
+        p_top = out_topk.data_ptr()
+    _check(_lib.tno_mf_search(ctx, frames.data_ptr(), T, H, W, sig.ctypes.data, tr.ctypes.data, n,
+                              float(prf_sigma), float(t0), p_snr, p_top), ctx)
+
+
+def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float) -> None:
+    """frames: CUDA float32 tensor [T, H, W], modified in place; sources: SOURCE_DTYPE array."""
+    assert frames.is_cuda and frames.is_contiguous() and frames.dim() == 3 and frames.element_size() == 4
+    T, H, W = frames.shape
+    src = np.ascontiguousarray(sources, dtype=SOURCE_DTYPE)
+    _check(_lib.tno_mf_inject(ctx, frames.data_ptr(), T, H, W, src.ctypes.data, src.shape[0],
+                              float(prf_sigma), float(t0)), ctx)
+
+
+def tno_mf_plan(trajectories, T: int, t0: float, max_entries: int, max_spread: int
+                ) -> Tuple[int, np.ndarray, np.ndarray]:
+    """Host-only: (n_batches, batch index per trajectory, slot per trajectory)."""
+    tr = _traj_array(trajectories)
+    n = tr.shape[0]
+    ob = np.full(n, -1, dtype=np.int32)
+    os_ = np.full(n, -1, dtype=np.int32)
+    rc = _lib.tno_mf_plan(tr.ctypes.data, n, int(T), float(t0), int(max_entries), int(max_spread),
+                          ob.ctypes.data, os_.ctypes.data)
+    if rc < 0:
+        raise TnoMfError(rc, "tno_mf_plan: invalid argument")
+    return rc, ob, os_
+
+
+def tno_mf_last_stats(ctx) -> Tuple[int, int]:
+    """(kernel launches of the last search, 1 if the separable TMA kernel was used else 0)."""
+    a, b = ctypes.c_int32(), ctypes.c_int32()
+    _check(_lib.tno_mf_last_stats(ctx, ctypes.byref(a), ctypes.byref(b)), None)
+    return a.value, b.value
+
+
+def make_sources(trajs, xs, ys, amps) -> np.ndarray:
+    """Pack per-source arrays into SOURCE_DTYPE records."""
+    tr = _traj_array(trajs)
+    out = np.zeros(tr.shape[0], dtype=SOURCE_DTYPE)
+    out["vx"], out["vy"], out["ax"], out["ay"] = tr[:, 0], tr[:, 1], tr[:, 2], tr[:, 3]
+    out["x"], out["y"], out["amplitude"] = xs, ys, amps
+    return out

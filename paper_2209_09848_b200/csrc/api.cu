@@ -1,0 +1,453 @@
+// C ABI of libtno_mf.so (include/tno_mf.h): context, validation, planning, launches.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.h"
+#include "plan.h"
+
+using namespace tno;
+
+namespace {
+
+thread_local std::string g_create_error = "";
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+}  // namespace
+
+struct tno_mf_ctx {
+    tno_mf_config cfg;
+    cudaStream_t stream = nullptr;
+    int32_t n_sm = 0;
+    void *encode_fn = nullptr;
+    std::string err;
+    int32_t last_launches = 0, last_kernel = 0;
+    // grow-only device workspace
+    DevBuf meta, shift, g, gd, ab, rsd, stage_tab, scratch, keys, counts, tmp_maps, src;
+};
+
+namespace {
+
+int fail(tno_mf_ctx *ctx, int code, const char *fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define CU_TRY(ctx, expr)                                                                   \
+    do {                                                                                    \
+        cudaError_t e_ = (expr);                                                            \
+        if (e_ != cudaSuccess)                                                              \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? TNO_MF_ENOMEM : TNO_MF_ECUDA, \
+                        "%s: %s", #expr, cudaGetErrorString(e_));                           \
+    } while (0)
+
+// Grow-only buffer.  cudaFree synchronises the device, so replacing a buffer that earlier work on
+// the stream may still read is safe.
+int reserve(tno_mf_ctx *ctx, DevBuf &b, size_t bytes) {
+    if (bytes <= b.cap) return TNO_MF_OK;
+    if (b.p) { cudaFree(b.p); b.p = nullptr; b.cap = 0; }
+    const size_t want = bytes + bytes / 8 + 256;
+    cudaError_t e = cudaMalloc(&b.p, want);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        e = cudaMalloc(&b.p, bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            b.p = nullptr;
+            return fail(ctx, TNO_MF_ENOMEM, "device allocation of %zu bytes failed: %s", bytes,
+                        cudaGetErrorString(e));
+        }
+        b.cap = bytes;
+        return TNO_MF_OK;
+    }
+    b.cap = want;
+    return TNO_MF_OK;
+}
+
+// host blob with 16-byte aligned sections, uploaded with one copy
+struct Blob {
+    std::vector<unsigned char> bytes;
+    size_t add(const void *src, size_t n) {
+        const size_t off = (bytes.size() + 15) & ~(size_t)15;
+        bytes.resize(off + n);
+        if (n) memcpy(bytes.data() + off, src, n);
+        return off;
+    }
+};
+
+AxisBorder make_border(const AxisClass &c, int32_t L) {
+    AxisBorder b;
+    b.lo = std::max(0, 2 - c.smin);
+    b.hi = std::max(0, c.smax + 2);
+    // lo/hi larger than the axis mean every pixel is clipped somewhere: fall back to identity
+    if ((int64_t)b.lo + 1 + (int64_t)b.hi >= (int64_t)L) {
+        b.identity = 1;
+        b.n = L;
+        b.lo = b.hi = 0;
+    } else {
+        b.identity = 0;
+        b.n = b.lo + 1 + b.hi;
+    }
+    return b;
+}
+
+bool finite_f(float v) { return std::isfinite(v); }
+
+}  // namespace
+
+extern "C" {
+
+const char *tno_mf_version(void) { return "tno_mf 0.1 (sm_100a)"; }
+
+const char *tno_mf_last_error(const tno_mf_ctx *ctx) {
+    return ctx ? ctx->err.c_str() : g_create_error.c_str();
+}
+
+int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
+    if (!cfg || !out_ctx) return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: NULL argument");
+    *out_ctx = nullptr;
+    if (cfg->topk < 0 || cfg->topk > kMaxTopk)
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
+    if (std::isnan(cfg->snr_threshold))
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
+    if (cfg->reserved[0] || cfg->reserved[1] || cfg->reserved[2])
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: reserved fields must be 0");
+    int n_dev = 0;
+    cudaError_t e = cudaGetDeviceCount(&n_dev);
+    if (e != cudaSuccess || n_dev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, TNO_MF_EUNSUPPORTED, "tno_mf_create: no CUDA device (%s); there is no CPU fallback",
+                    e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    if (cfg->device < 0 || cfg->device >= n_dev)
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: device %d out of range [0, %d)", cfg->device, n_dev);
+    cudaDeviceProp prop;
+    CU_TRY(nullptr, cudaGetDeviceProperties(&prop, cfg->device));
+    if (prop.major != 10)
+        return fail(nullptr, TNO_MF_EUNSUPPORTED,
+                    "tno_mf_create: device %d is sm_%d%d; this library is built for sm_100a only",
+                    cfg->device, prop.major, prop.minor);
+    CU_TRY(nullptr, cudaSetDevice(cfg->device));
+    tno_mf_ctx *ctx = new (std::nothrow) tno_mf_ctx();
+    if (!ctx) return fail(nullptr, TNO_MF_ENOMEM, "tno_mf_create: out of host memory");
+    ctx->cfg = *cfg;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cfg->stream);
+    ctx->n_sm = prop.multiProcessorCount;
+    cudaDriverEntryPointQueryResult qres;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !ctx->encode_fn) {
+        cudaGetLastError();
+        delete ctx;
+        return fail(nullptr, TNO_MF_ECUDA, "tno_mf_create: cuTensorMapEncodeTiled not available in the driver");
+    }
+    *out_ctx = ctx;
+    return TNO_MF_OK;
+}
+
+int tno_mf_destroy(tno_mf_ctx *ctx) {
+    if (!ctx) return TNO_MF_OK;
+    cudaSetDevice(ctx->cfg.device);
+    DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
+                      &ctx->scratch, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src};
+    for (DevBuf *b : bufs)
+        if (b->p) cudaFree(b->p);
+    delete ctx;
+    return TNO_MF_OK;
+}
+
+int tno_mf_last_stats(const tno_mf_ctx *ctx, int32_t *out_launches, int32_t *out_kernel) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (out_launches) *out_launches = ctx->last_launches;
+    if (out_kernel) *out_kernel = ctx->last_kernel;
+    return TNO_MF_OK;
+}
+
+int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, float t0,
+                int32_t max_entries, int32_t max_spread, int32_t *out_batch, int32_t *out_slot) {
+    if (!trajectories || n_traj < 1 || T < 1 || max_entries < 1 || max_entries > 16 || max_spread < 0 ||
+        !finite_f(t0))
+        return TNO_MF_EINVAL;
+    for (int32_t k = 0; k < n_traj; ++k)
+        if (!finite_f(trajectories[k].vx) || !finite_f(trajectories[k].vy) ||
+            !finite_f(trajectories[k].ax) || !finite_f(trajectories[k].ay))
+            return TNO_MF_EINVAL;
+    Plan plan;
+    const int rc = build_classes(trajectories, n_traj, T, (double)t0, &plan);
+    if (rc != TNO_MF_OK) return rc;
+    build_batches(&plan, max_entries, max_spread);
+    for (size_t b = 0; b < plan.batches.size(); ++b)
+        for (size_t s = 0; s < plan.batches[b].traj.size(); ++s) {
+            if (out_batch) out_batch[plan.batches[b].traj[s]] = (int32_t)b;
+            if (out_slot) out_slot[plan.batches[b].traj[s]] = (int32_t)s;
+        }
+    return (int)plan.batches.size();
+}
+
+int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W,
+                  const tno_mf_source *sources, int32_t n_sources, float prf_sigma, float t0) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (!frames || !sources || T < 1 || H < 1 || W < 1 || n_sources < 0)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: NULL pointer or non-positive size");
+    if (!(prf_sigma > 0.f) || !finite_f(prf_sigma) || !finite_f(t0))
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: prf_sigma must be finite and > 0, t0 finite");
+    if (n_sources == 0) return TNO_MF_OK;
+    std::vector<SourceDev> host(n_sources);
+    for (int32_t m = 0; m < n_sources; ++m) {
+        const tno_mf_source &s = sources[m];
+        if (!finite_f(s.traj.vx) || !finite_f(s.traj.vy) || !finite_f(s.traj.ax) || !finite_f(s.traj.ay) ||
+            !finite_f(s.amplitude))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: source %d has a non-finite value", m);
+        host[m] = {s.traj.vx, s.traj.vy, s.traj.ax, s.traj.ay, s.x, s.y, s.amplitude};
+    }
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc = reserve(ctx, ctx->src, host.size() * sizeof(SourceDev));
+    if (rc) return rc;
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->src.p, host.data(), host.size() * sizeof(SourceDev),
+                                cudaMemcpyHostToDevice, ctx->stream));
+    launch_inject(ctx->stream, frames, T, H, W, static_cast<const SourceDev *>(ctx->src.p), n_sources,
+                  (double)prf_sigma, (double)t0);
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
+}
+
+int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
+                  const float *sigma_t, const tno_mf_traj *trajectories, int32_t n_traj,
+                  float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
+    if (!ctx) return TNO_MF_EINVAL;
+    ctx->last_launches = 0;
+    // ------------------------------------------------------------------ validation
+    if (!frames || !sigma_t || !trajectories)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: NULL frames, sigma_t or trajectories");
+    if (T < 1 || H < 1 || W < 1 || n_traj < 1)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: T, H, W and n_traj must be >= 1");
+    if (n_traj > 65535) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: at most 65535 trajectories per call");
+    if ((int64_t)H * W > (int64_t)1 << 31)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: H*W must not exceed 2^31 pixels");
+    if (!(prf_sigma > 0.f) || !finite_f(prf_sigma))
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: prf_sigma must be finite and > 0");
+    if (!finite_f(t0)) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: t0 must be finite");
+    const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
+    if (!out_snr && !want_topk)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: no output requested (out_snr NULL and no top-K)");
+    for (int32_t t = 0; t < T; ++t)
+        if (!(sigma_t[t] > 0.f) || !finite_f(sigma_t[t]))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: sigma_t[%d] must be finite and > 0", t);
+    for (int32_t k = 0; k < n_traj; ++k)
+        if (!finite_f(trajectories[k].vx) || !finite_f(trajectories[k].vy) ||
+            !finite_f(trajectories[k].ax) || !finite_f(trajectories[k].ay))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: trajectory %d has a non-finite value", k);
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = ctx->stream;
+
+    // ------------------------------------------------------------------ planning (host)
+    Plan plan;
+    if (build_classes(trajectories, n_traj, T, (double)t0, &plan) != TNO_MF_OK)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: a trajectory displacement exceeds 1e9 px");
+    const int32_t n_x = (int32_t)plan.xcls.size(), n_y = (int32_t)plan.ycls.size();
+    const int32_t n_cls = n_x + n_y;
+    if (n_cls > 65535) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: too many distinct axis motions");
+
+    const bool use_sep = !ctx->cfg.force_generic && (W % 4 == 0) &&
+                         ((reinterpret_cast<uintptr_t>(frames) & 15u) == 0) && W >= 4;
+    int32_t variant = -1;
+    if (use_sep) {
+        double best = 0.0;
+        Plan trial = plan;
+        for (int32_t v = 0; v < sep_num_variants(); ++v) {
+            const SepVariant sv = sep_variant(v);
+            build_batches(&trial, sv.nb, sv.max_spread);
+            const double cost = (double)trial.batches.size() * (sv.nb + 1.5);
+            if (variant < 0 || cost < best) {
+                best = cost;
+                variant = v;
+                plan.batches = trial.batches;
+            }
+        }
+    }
+    ctx->last_kernel = use_sep ? 1 : 0;
+
+    // ------------------------------------------------------------------ host metadata blob
+    std::vector<float> cls_v(n_cls), cls_a(n_cls);
+    std::vector<AxisBorder> border(n_cls);
+    std::vector<int64_t> ab_off(n_cls);
+    int64_t ab_total = 0;
+    int32_t max_n = 0;
+    for (int32_t c = 0; c < n_cls; ++c) {
+        const AxisClass &ac = c < n_x ? plan.xcls[c] : plan.ycls[c - n_x];
+        cls_v[c] = ac.v;
+        cls_a[c] = ac.a;
+        border[c] = make_border(ac, c < n_x ? W : H);
+        ab_off[c] = ab_total;
+        ab_total += (int64_t)border[c].n * T;
+        max_n = std::max(max_n, border[c].n);
+    }
+    std::vector<float> qf(T);
+    std::vector<double> qd(T);
+    for (int32_t t = 0; t < T; ++t) {
+        const double s = (double)sigma_t[t];
+        qd[t] = 1.0 / (s * s);
+        qf[t] = (float)qd[t];
+    }
+    std::vector<TrajInfo> tinfo(n_traj);
+    int64_t rsd_total = 0, max_cells = 0;
+    for (int32_t k = 0; k < n_traj; ++k) {
+        TrajInfo &ti = tinfo[k];
+        ti.xc = plan.traj_xc[k];
+        ti.yc = plan.traj_yc[k];
+        ti.bx = border[ti.xc];
+        ti.by = border[n_x + ti.yc];
+        ti.rsd_off = rsd_total;
+        const int64_t cells = (int64_t)ti.bx.n * ti.by.n;
+        rsd_total += cells;
+        max_cells = std::max(max_cells, cells);
+    }
+    SepVariant sv = {0, 0, 0};
+    int32_t n_batches = 0;
+    std::vector<int32_t> batch_xc, batch_yc, batch_traj;
+    if (use_sep) {
+        sv = sep_variant(variant);
+        n_batches = (int32_t)plan.batches.size();
+        batch_xc.resize(n_batches);
+        batch_yc.assign((size_t)n_batches * sv.nb, -1);
+        batch_traj.assign((size_t)n_batches * sv.nb, -1);
+        for (int32_t b = 0; b < n_batches; ++b) {
+            const Batch &bt = plan.batches[b];
+            batch_xc[b] = bt.xcls;
+            for (size_t s = 0; s < bt.traj.size(); ++s) {
+                batch_traj[(size_t)b * sv.nb + s] = bt.traj[s];
+                batch_yc[(size_t)b * sv.nb + s] = plan.traj_yc[bt.traj[s]];
+            }
+        }
+    }
+    Blob blob;
+    const size_t o_v = blob.add(cls_v.data(), cls_v.size() * 4);
+    const size_t o_a = blob.add(cls_a.data(), cls_a.size() * 4);
+    const size_t o_qf = blob.add(qf.data(), qf.size() * 4);
+    const size_t o_qd = blob.add(qd.data(), qd.size() * 8);
+    const size_t o_bd = blob.add(border.data(), border.size() * sizeof(AxisBorder));
+    const size_t o_off = blob.add(ab_off.data(), ab_off.size() * 8);
+    const size_t o_ti = blob.add(tinfo.data(), tinfo.size() * sizeof(TrajInfo));
+    const size_t o_bx = blob.add(batch_xc.data(), batch_xc.size() * 4);
+    const size_t o_by = blob.add(batch_yc.data(), batch_yc.size() * 4);
+    const size_t o_bt = blob.add(batch_traj.data(), batch_traj.size() * 4);
+
+    // ------------------------------------------------------------------ workspace
+    int rc;
+    const size_t ct = (size_t)n_cls * T;
+    if ((rc = reserve(ctx, ctx->meta, blob.bytes.size()))) return rc;
+    if ((rc = reserve(ctx, ctx->shift, ct * 4))) return rc;
+    if ((rc = reserve(ctx, ctx->g, ct * 5 * 4))) return rc;
+    if ((rc = reserve(ctx, ctx->gd, ct * 5 * 8))) return rc;
+    if ((rc = reserve(ctx, ctx->ab, (size_t)ab_total * 8))) return rc;
+    if ((rc = reserve(ctx, ctx->rsd, (size_t)rsd_total * 4))) return rc;
+    const int32_t tile_h = use_sep ? sv.tile_h : kCollectTile;
+    const int32_t ntx = (W + 63) / 64, nty = (H + tile_h - 1) / tile_h;
+    const int64_t n_tiles = (int64_t)ntx * nty;
+    if (want_topk) {
+        if ((rc = reserve(ctx, ctx->keys, (size_t)n_tiles * n_traj * ctx->cfg.topk * 8))) return rc;
+        if ((rc = reserve(ctx, ctx->counts, (size_t)n_tiles * n_traj * 4))) return rc;
+    }
+    if (use_sep) {
+        if ((rc = reserve(ctx, ctx->stage_tab, (size_t)n_batches * T * sep_table_words(variant) * 4))) return rc;
+        if ((rc = reserve(ctx, ctx->scratch, (size_t)ctx->n_sm * sep_scratch_floats_per_cta(variant) * 4))) return rc;
+    }
+    unsigned char *meta = static_cast<unsigned char *>(ctx->meta.p);
+    CU_TRY(ctx, cudaMemcpyAsync(meta, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st));
+
+    ClassTables tab;
+    tab.shift = static_cast<const int32_t *>(ctx->shift.p);
+    tab.g = static_cast<const float *>(ctx->g.p);
+    tab.gd = static_cast<const double *>(ctx->gd.p);
+    tab.qf = reinterpret_cast<const float *>(meta + o_qf);
+    tab.qd = reinterpret_cast<const double *>(meta + o_qd);
+    tab.n_x = n_x;
+    tab.T = T;
+    const TrajInfo *d_ti = reinterpret_cast<const TrajInfo *>(meta + o_ti);
+    const int64_t *d_off = reinterpret_cast<const int64_t *>(meta + o_off);
+    float *d_rsd = static_cast<float *>(ctx->rsd.p);
+
+    // ------------------------------------------------------------------ table kernels
+    launch_class_tables(st, reinterpret_cast<const float *>(meta + o_v), reinterpret_cast<const float *>(meta + o_a),
+                        n_cls, T, (double)t0, (double)prf_sigma, static_cast<int32_t *>(ctx->shift.p),
+                        static_cast<float *>(ctx->g.p), static_cast<double *>(ctx->gd.p));
+    launch_border_tables(st, tab.shift, tab.gd, tab.qd, reinterpret_cast<const AxisBorder *>(meta + o_bd), d_off,
+                         n_cls, n_x, max_n, T, W, H, static_cast<double *>(ctx->ab.p));
+    launch_rsd_tables(st, d_ti, n_traj, max_cells, static_cast<const double *>(ctx->ab.p), d_off, n_x, T, d_rsd);
+    ctx->last_launches += 3;
+    CU_TRY(ctx, cudaGetLastError());
+
+    TopkSlots slots;
+    slots.keys = want_topk ? static_cast<uint64_t *>(ctx->keys.p) : nullptr;
+    slots.counts = want_topk ? static_cast<int32_t *>(ctx->counts.p) : nullptr;
+    slots.ktop = ctx->cfg.topk;
+    slots.K = n_traj;
+    slots.threshold = ctx->cfg.snr_threshold;
+
+    // ------------------------------------------------------------------ search
+    if (use_sep) {
+        launch_sep_tables(st, variant, tab, reinterpret_cast<const int32_t *>(meta + o_bx),
+                          reinterpret_cast<const int32_t *>(meta + o_by), n_batches,
+                          static_cast<float *>(ctx->stage_tab.p));
+        ctx->last_launches += 1;
+        CU_TRY(ctx, cudaGetLastError());
+        SepArgs a;
+        a.frames = frames; a.T = T; a.H = H; a.W = W;
+        a.stage_tab = static_cast<const float *>(ctx->stage_tab.p);
+        a.batch_traj = reinterpret_cast<const int32_t *>(meta + o_bt);
+        a.n_batches = n_batches;
+        a.traj = d_ti;
+        a.rsd = d_rsd;
+        a.out_snr = out_snr;
+        a.slots = slots;
+        a.scratch = static_cast<float *>(ctx->scratch.p);
+        a.n_sm = ctx->n_sm;
+        int32_t grid = 0;
+        const char *err = "";
+        if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
+            return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
+        ctx->last_launches += 1;
+    } else {
+        // generic path: maps are always materialised (caller's buffer, or a workspace chunk)
+        const int64_t map_px = (int64_t)H * W;
+        int32_t chunk = n_traj;
+        float *maps = out_snr;
+        if (!out_snr) {
+            const int64_t budget = (int64_t)1 << 29;   // floats (2 GiB)
+            chunk = (int32_t)std::max<int64_t>(1, std::min<int64_t>(n_traj, budget / map_px));
+            if ((rc = reserve(ctx, ctx->tmp_maps, (size_t)chunk * map_px * 4))) return rc;
+            maps = static_cast<float *>(ctx->tmp_maps.p);
+        }
+        for (int32_t k0 = 0; k0 < n_traj; k0 += chunk) {
+            const int32_t kc = std::min(chunk, n_traj - k0);
+            float *dst = out_snr ? out_snr + (int64_t)k0 * map_px : maps;
+            launch_search_generic(st, frames, T, H, W, tab, d_ti, d_rsd, k0, kc, dst);
+            ctx->last_launches += 1;
+            if (want_topk) {
+                launch_collect_from_map(st, dst, H, W, k0, kc, slots);
+                ctx->last_launches += 1;
+            }
+        }
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    if (want_topk) {
+        launch_topk_merge(st, slots, (int32_t)n_tiles, W, out_topk);
+        ctx->last_launches += 1;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    return TNO_MF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,49 @@
+// Signal injection: R_t(p) <- (float)((double)R_t(p) + A g(p - c_t)) on the 25
+// window taps of every frame.  One thread per frame applies the sources in order, so overlapping
+// sources give a deterministic result.
+#include "kernels.h"
+
+namespace tno {
+
+__device__ __forceinline__ void axis_pos(double v, double a, double dt, int32_t *s, double *ph) {
+    const double d = __dadd_rn(__dmul_rn(v, dt), __dmul_rn(__dmul_rn(a, dt), dt));
+    const double f = floor(__dadd_rn(d, 0.5));
+    *s = (int32_t)f;
+    *ph = __dsub_rn(d, f);
+}
+
+__global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32_t W,
+                         const SourceDev *__restrict__ src, int32_t n_src, double prf_sigma,
+                         double t0) {
+    const int32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= T) return;
+    const double dt = (double)t - t0;
+    const double inv = 1.0 / (2.0 * prf_sigma * prf_sigma);
+    float *f = frames + (int64_t)t * H * W;
+    for (int32_t m = 0; m < n_src; ++m) {
+        const SourceDev s = src[m];
+        int32_t sx, sy;
+        double phx, phy;
+        axis_pos((double)s.vx, (double)s.ax, dt, &sx, &phx);
+        axis_pos((double)s.vy, (double)s.ay, dt, &sy, &phy);
+        for (int j = -2; j <= 2; ++j) {
+            const int32_t py = s.y + sy + j;
+            if (py < 0 || py >= H) continue;
+            for (int i = -2; i <= 2; ++i) {
+                const int32_t px = s.x + sx + i;
+                if (px < 0 || px >= W) continue;
+                const double ux = (double)i - phx, uy = (double)j - phy;
+                const double g = exp(-(ux * ux + uy * uy) * inv);
+                float *p = f + (int64_t)py * W + px;
+                *p = (float)((double)*p + (double)s.amp * g);
+            }
+        }
+    }
+}
+
+void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,
+                   const SourceDev *src, int32_t n_src, double prf_sigma, double t0) {
+    k_inject<<<(unsigned)((T + 63) / 64), 64, 0, st>>>(frames, T, H, W, src, n_src, prf_sigma, t0);
+}
+
+}  // namespace tno

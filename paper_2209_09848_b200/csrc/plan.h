@@ -1,0 +1,49 @@
+// Host planner of the matched-filter search (no CUDA in this file).
+//
+// The filter of PAPER.md:L106 ("convolving the line of the trajectory with the pixel response
+// function") is separable per frame: its x part depends only on the trajectory's x-motion
+// (vx, ax), its y part only on (vy, ay).  The planner groups trajectories into AXIS CLASSES
+// (distinct x-motions, distinct y-motions) and packs them into BATCHES that share one x-class,
+// so that the x-pass of the separable kernel is computed once per batch.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include "../../include/tno_mf.h"
+
+namespace tno {
+
+// floor(d + 1/2) of d = v*dt + a*dt*dt, all in IEEE double without contraction
+// (BASELINE.json:north_star "5x5 window at round(c_t)"; reading c1 in DESIGN.md: ties go up).
+// Returns false if the shift does not fit comfortably in 32 bits.
+bool axis_shift(double v, double a, double dt, int32_t *shift);
+
+struct AxisClass {
+    float v, a;                  // px/frame, px/frame^2 (exact float32 values of the ABI)
+    int32_t smin, smax;          // extreme integer shifts over t = 0..T-1
+    std::vector<int32_t> shift;  // [T]
+};
+
+struct Batch {
+    int32_t xcls;                // x-class shared by every entry
+    std::vector<int32_t> traj;   // trajectory index of each entry (size <= max_entries)
+    int32_t max_spread;          // max over t of (max_e sy - min_e sy)
+};
+
+struct Plan {
+    int32_t T = 0;
+    double t0 = 0.0;
+    std::vector<AxisClass> xcls, ycls;
+    std::vector<int32_t> traj_xc, traj_yc;   // [n_traj]
+    std::vector<Batch> batches;
+};
+
+// Group trajectories into axis classes.  Returns TNO_MF_OK or TNO_MF_EINVAL (shift overflow).
+int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0, Plan *plan);
+
+// Pack the trajectories of each x-class into batches of at most max_entries entries whose integer
+// y-shifts never differ by more than max_spread in any frame.  Entries are ordered by (vy, ay) so
+// that neighbours move alike.  A single trajectory always fits (spread 0).
+void build_batches(Plan *plan, int32_t max_entries, int32_t max_spread);
+
+}  // namespace tno

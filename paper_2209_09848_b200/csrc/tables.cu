@@ -1,0 +1,95 @@
+// Table kernels: everything that depends on (trajectory class, frame) but not on the pixel.
+//   k_class_tables   shift, phase, PRF taps per (class, t)        -- the sparse form of the filter
+//                    of PAPER.md:L106 (trajectory line (x) PRF), 5 + 5 taps instead of R x C
+//   k_border_tables  per-axis clipped sums of squared taps per (class, t, border class)
+//   k_rsd_tables     D^(-1/2) per (trajectory, border class y, border class x)
+// D = sum_t sum_p g(p - c_t)^2 / sigma_t^2 with off-frame taps dropped (BASELINE.json:north_star)
+// is separable per frame, D = sum_t q_t Ax_t(x) Ay_t(y); it is evaluated in float64.
+#include "kernels.h"
+
+namespace tno {
+
+__global__ void k_class_tables(const float *__restrict__ cls_v, const float *__restrict__ cls_a,
+                               int32_t n_cls, int32_t T, double t0, double prf_sigma,
+                               int32_t *__restrict__ shift, float *__restrict__ g,
+                               double *__restrict__ gd) {
+    const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (int64_t)n_cls * T) return;
+    const int32_t c = (int32_t)(id / T), t = (int32_t)(id % T);
+    const double v = (double)cls_v[c], a = (double)cls_a[c];
+    const double dt = (double)t - t0;
+    // d = v*dt + a*dt*dt evaluated left to right, every operation separately rounded
+    const double d = __dadd_rn(__dmul_rn(v, dt), __dmul_rn(__dmul_rn(a, dt), dt));
+    const double f = floor(__dadd_rn(d, 0.5));
+    const double ph = __dsub_rn(d, f);
+    shift[id] = (int32_t)f;
+    const double inv = 1.0 / (2.0 * prf_sigma * prf_sigma);
+#pragma unroll
+    for (int i = 0; i < 5; ++i) {
+        const double u = (double)(i - 2) - ph;
+        const double w = exp(-(u * u) * inv);
+        g[id * 5 + i] = (float)w;
+        gd[id * 5 + i] = w;
+    }
+}
+
+// out[off[c] + t * n + j] = (scale_q ? q_t : 1) * sum_{i : 0 <= rep(j) + s + i - 2 < L} gd[c][t][i]^2
+__global__ void k_border_tables(const int32_t *__restrict__ shift, const double *__restrict__ gd,
+                                const double *__restrict__ qd, const AxisBorder *__restrict__ border,
+                                const int64_t *__restrict__ off, int32_t n_x, int32_t T, int32_t W,
+                                int32_t H, double *__restrict__ out) {
+    const int32_t c = blockIdx.y;
+    const AxisBorder b = border[c];
+    const int32_t L = (c < n_x) ? W : H;
+    const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (int64_t)b.n * T) return;
+    const int32_t t = (int32_t)(id / b.n), j = (int32_t)(id % b.n);
+    const int32_t p = border_rep(j, b, L) + shift[(int64_t)c * T + t] - 2;
+    const double *w = gd + ((int64_t)c * T + t) * 5;
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 5; ++i)
+        if (p + i >= 0 && p + i < L) s += w[i] * w[i];
+    if (c < n_x) s *= qd[t];
+    out[off[c] + id] = s;
+}
+
+// rsd[k][cy][cx] = 1 / sqrt(sum_t AX[xc][t][cx] * AY[yc][t][cy])   (0 where the sum is 0)
+__global__ void k_rsd_tables(const TrajInfo *__restrict__ traj, const double *__restrict__ ab,
+                             const int64_t *__restrict__ off, int32_t n_x, int32_t T,
+                             float *__restrict__ rsd) {
+    const TrajInfo ti = traj[blockIdx.y];
+    const int32_t ncx = ti.bx.n, ncy = ti.by.n;
+    const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (int64_t)ncx * ncy) return;
+    const int32_t cy = (int32_t)(id / ncx), cx = (int32_t)(id % ncx);
+    const double *ax = ab + off[ti.xc] + cx;
+    const double *ay = ab + off[n_x + ti.yc] + cy;
+    double D = 0.0;
+    for (int32_t t = 0; t < T; ++t) D += ax[(int64_t)t * ncx] * ay[(int64_t)t * ncy];
+    rsd[ti.rsd_off + id] = (D > 0.0) ? (float)(1.0 / sqrt(D)) : 0.0f;
+}
+
+void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a, int32_t n_cls,
+                         int32_t T, double t0, double prf_sigma, int32_t *shift, float *g,
+                         double *gd) {
+    const int64_t n = (int64_t)n_cls * T;
+    k_class_tables<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cls_v, cls_a, n_cls, T, t0,
+                                                                 prf_sigma, shift, g, gd);
+}
+
+void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,
+                          const AxisBorder *border, const int64_t *off, int32_t n_cls, int32_t n_x,
+                          int32_t max_n, int32_t T, int32_t W, int32_t H, double *out) {
+    const int64_t n = (int64_t)max_n * T;
+    dim3 grid((unsigned)((n + 255) / 256), (unsigned)n_cls);
+    k_border_tables<<<grid, 256, 0, st>>>(shift, gd, qd, border, off, n_x, T, W, H, out);
+}
+
+void launch_rsd_tables(cudaStream_t st, const TrajInfo *traj, int32_t n_traj, int64_t max_cells,
+                       const double *ab, const int64_t *off, int32_t n_x, int32_t T, float *rsd) {
+    dim3 grid((unsigned)((max_cells + 127) / 128), (unsigned)n_traj);
+    k_rsd_tables<<<grid, 128, 0, st>>>(traj, ab, off, n_x, T, rsd);
+}
+
+}  // namespace tno

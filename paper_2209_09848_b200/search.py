@@ -1,0 +1,65 @@
+"""Convenience wrapper: allocates the output tensors with torch and calls the C ABI."""
+from __future__ import annotations
+
+from typing import Optional, Tuple
+
+import numpy as np
+
+from . import binding as B
+
+
+class MatchedFilter:
+    """One library context bound to the current torch CUDA stream of `device`."""
+
+    def __init__(self, device: int = 0, topk: int = 0, snr_threshold: float = float("-inf"),
+                 force_generic: bool = False):
+        import torch
+        self._torch = torch
+        self.device = torch.device("cuda", device)
+        self.topk = int(topk)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic)
+
+    def close(self) -> None:
+        if self.ctx is not None:
+            self._torch.cuda.synchronize(self.device)
+            B.tno_mf_destroy(self.ctx)
+            self.ctx = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def search(self, frames, sigma_t, trajectories, prf_sigma: float, t0: float,
+               want_maps: bool = True, out_snr=None, out_topk=None):
+        """Returns (snr maps tensor [n, H, W] or None, candidate tensor or None); asynchronous."""
+        torch = self._torch
+        n = np.asarray(trajectories).shape[0]
+        T, H, W = frames.shape
+        if want_maps and out_snr is None:
+            out_snr = torch.empty((n, H, W), dtype=torch.float32, device=frames.device)
+        if self.topk > 0 and out_topk is None:
+            out_topk = torch.empty((n, self.topk, 4), dtype=torch.int32, device=frames.device)
+        B.tno_mf_search(self.ctx, frames, sigma_t, trajectories, prf_sigma, t0,
+                        out_snr if want_maps else None, out_topk if self.topk > 0 else None)
+        return (out_snr if want_maps else None), (out_topk if self.topk > 0 else None)
+
+    def inject(self, frames, trajs, xs, ys, amps, prf_sigma: float, t0: float) -> None:
+        B.tno_mf_inject(self.ctx, frames, B.make_sources(trajs, xs, ys, amps), prf_sigma, t0)
+
+    @staticmethod
+    def candidates_to_numpy(out_topk) -> np.ndarray:
+        """[n, topk] structured array (snr, x, y, k) from the int32 [n, topk, 4] device tensor."""
+        a = out_topk.cpu().numpy()
+        return a.view(B.CAND_DTYPE).reshape(a.shape[0], a.shape[1])
+
+    def stats(self) -> Tuple[int, int]:
+        return B.tno_mf_last_stats(self.ctx)

@@ -1,0 +1,170 @@
+"""GPU parity: the CUDA library (through its C ABI) against the CPU oracle, element by element.
+Run on a B200 with `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import oracle
+import tno_synth
+from helpers import TOL, check_topk, check_topk_vs_own_map, cpu_inputs, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+def _compare_full(cfg, force_generic):
+    torch = _torch()
+    p, f = cpu_inputs(cfg)
+    om = oracle.snr_map(f, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0)
+    fd = torch.from_numpy(f).cuda()
+    gm, gc, stats = run_gpu(fd, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0, cfg.topk, cfg.threshold,
+                            force_generic=force_generic)
+    assert stats[1] == (0 if force_generic else 1)
+    assert stats[0] >= 5
+    err = np.abs(gm.astype(np.float64) - om)
+    assert err.max() <= TOL, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    for k in range(cfg.n_traj):
+        check_topk(gc[k], om[k], k, cfg.topk, cfg.threshold)
+        check_topk_vs_own_map(gc[k], gm[k], k, cfg.topk, cfg.threshold)
+    # injected sources are where the oracle says they are
+    for i in range(len(p.src_k)):
+        k, x, y = int(p.src_k[i]), int(p.src_x[i]), int(p.src_y[i])
+        assert abs(float(gm[k, y, x]) - om[k, y, x]) <= TOL
+    return err.max()
+
+
+@pytest.mark.parametrize("force_generic", [False, True])
+def test_config1_full_maps_and_topk(force_generic):
+    _compare_full(tno_synth.CONFIGS[1], force_generic)
+
+
+@pytest.mark.parametrize("force_generic", [False, True])
+def test_config2_full_maps_and_topk(force_generic):
+    _compare_full(tno_synth.CONFIGS[2], force_generic)
+
+
+def test_config1_against_oracle_point_everywhere():
+    torch = _torch()
+    cfg = tno_synth.CONFIGS[1]
+    p, f = cpu_inputs(cfg)
+    gm, _, _ = run_gpu(torch.from_numpy(f).cuda(), p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0,
+                       cfg.topk, cfg.threshold)
+    for k in range(cfg.n_traj):
+        for y in range(0, cfg.H, 3):
+            for x in range(0, cfg.W, 3):
+                s, _, _ = oracle.point(f, p.sigma_t, p.traj[k], cfg.prf_sigma, cfg.t0, x, y)
+                assert abs(float(gm[k, y, x]) - s) <= TOL
+
+
+@pytest.mark.parametrize("shape,force_generic", [
+    ((7, 64, 64), False), ((3, 70, 132), False), ((5, 130, 68), False), ((1, 8, 8), False),
+    ((4, 33, 47), True), ((2, 1, 1), True), ((3, 5, 9), True), ((6, 65, 4), False),
+    ((70, 40, 72), False),
+])
+def test_ragged_shapes_and_mixed_trajectories(shape, force_generic):
+    """Sizes that are not multiples of the tile, tiny frames, T < pipeline depth, T > one flush
+    segment; trajectories with shared and unshared x-motions, accelerations, exact ties."""
+    torch = _torch()
+    T, H, W = shape
+    rng = np.random.default_rng(T * 10007 + H * 101 + W)
+    f = rng.standard_normal(shape).astype(np.float32)
+    f[T // 2, H // 2, W // 2] += 40.0
+    sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
+    traj = np.array([[0.3, -0.2, 0, 0], [0.3, 0.45, 0, 0], [0.3, 0.0, 0, 0.01], [-1.25, 0.5, 0, 0],
+                     [0.5, 0.5, 0, 0], [-0.5, 0.25, 0, 0], [0, 0, 0, 0], [2.0, -3.0, 0.1, 0],
+                     [0.3, -0.2, 0, 0], [0.11, 0.9, -0.02, 0.03], [0.3, 7.0, 0, 0]], dtype=np.float32)
+    t0 = float(T // 2)
+    om = oracle.snr_map(f, sigma, traj, 1.0, t0)
+    gm, gc, stats = run_gpu(torch.from_numpy(f).cuda(), sigma, traj, 1.0, t0, 7, 2.5,
+                            force_generic=force_generic)
+    if W % 4 != 0:
+        assert stats[1] == 0        # shapes the TMA kernel does not take go to the generic kernel
+    err = np.abs(gm.astype(np.float64) - om)
+    assert err.max() <= TOL, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    for k in range(traj.shape[0]):
+        check_topk(gc[k], om[k], k, 7, 2.5)
+        check_topk_vs_own_map(gc[k], gm[k], k, 7, 2.5)
+
+
+def test_zero_frames_and_threshold_edges():
+    torch = _torch()
+    T, H, W = 5, 64, 64
+    z = torch.zeros((T, H, W), device="cuda")
+    sigma = np.ones(T, np.float32)
+    traj = np.array([[0.2, 0.1, 0, 0], [7.0, 0, 0, 0]], np.float32)
+    gm, gc, _ = run_gpu(z, sigma, traj, 1.0, 2.0, 4, 5.0)
+    assert np.all(gm == 0.0)
+    assert np.all(gc["x"] == -1) and np.all(np.isneginf(gc["snr"]))
+    # threshold -inf: every pixel competes; lists are full and start at pixel (0, 0) on all-zero maps
+    gm, gc, _ = run_gpu(z, sigma, traj, 1.0, 2.0, 4, float("-inf"))
+    assert gc["x"][0].tolist() == [0, 1, 2, 3] and gc["y"][0].tolist() == [0, 0, 0, 0]
+    # maps only / lists only
+    gm, gc, _ = run_gpu(z, sigma, traj, 1.0, 2.0, 0, 5.0)
+    assert gc is None and gm.shape == (2, H, W)
+    gm, gc, _ = run_gpu(z, sigma, traj, 1.0, 2.0, 3, 5.0, want_maps=False)
+    assert gm is None and gc.shape == (2, 3)
+
+
+def test_many_candidates_per_tile_and_exact_ties():
+    """More candidates than K in one tile (tile-level selection), exact ties across tiles."""
+    torch = _torch()
+    T, H, W = 3, 128, 192
+    f = np.zeros((T, H, W), np.float32)
+    f[:, 10:50, 5:60] = 3.0                      # a bright plateau: hundreds of candidates, many ties
+    f[:, 100, 150] = 9.0
+    f[:, 100, 20] = 9.0                          # exact tie with the previous one, another tile
+    sigma = np.ones(T, np.float32)
+    traj = np.zeros((2, 4), np.float32)
+    traj[1, 0] = 1.0
+    om = oracle.snr_map(f, sigma, traj, 1.0, 1.0)
+    for generic in (False, True):
+        gm, gc, _ = run_gpu(torch.from_numpy(f).cuda(), sigma, traj, 1.0, 1.0, 50, 1.0,
+                            force_generic=generic)
+        assert np.abs(gm - om).max() <= TOL
+        for k in range(2):
+            check_topk_vs_own_map(gc[k], gm[k], k, 50, 1.0)
+            check_topk(gc[k], om[k], k, 50, 1.0)
+
+
+def test_inject_matches_oracle_renderer():
+    torch = _torch()
+    from paper_2209_09848_b200 import MatchedFilter
+    cfg = tno_synth.CONFIGS[2]
+    p = tno_synth.make_params(cfg)
+    base = tno_synth.stack_numpy(p)
+    a = base.copy()
+    oracle.inject(a, p.traj[p.src_k], p.src_x, p.src_y, p.src_amp, cfg.prf_sigma, cfg.t0)
+    d = torch.from_numpy(base).cuda()
+    with MatchedFilter(0) as mf:
+        mf.inject(d, p.traj[p.src_k], p.src_x, p.src_y, p.src_amp, cfg.prf_sigma, cfg.t0)
+        torch.cuda.synchronize()
+    b = d.cpu().numpy()
+    changed = a != base
+    assert np.array_equal(b != base, changed) or np.count_nonzero((b != base) ^ changed) < 10
+    # identical up to one float32 rounding of exp()
+    assert np.max(np.abs(a - b)) <= 1e-6 * max(1.0, float(np.abs(a).max()))
+    assert np.count_nonzero(a != b) <= 0.01 * np.count_nonzero(changed)
+
+
+def test_errors_are_reported():
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    ctx = P.tno_mf_create(0, None, 3, 5.0)
+    f = torch.zeros((2, 8, 8), device="cuda")
+    out = torch.empty((1, 8, 8), device="cuda")
+    with pytest.raises(P.TnoMfError) as e:
+        P.tno_mf_search(ctx, f, np.array([1.0, -1.0], np.float32), np.zeros((1, 4), np.float32), 1.0, 0.0, out)
+    assert e.value.code == -1 and "sigma_t" in str(e.value)
+    with pytest.raises(P.TnoMfError):
+        P.tno_mf_search(ctx, f, np.ones(2, np.float32), np.zeros((1, 4), np.float32), 0.0, 0.0, out)
+    with pytest.raises(P.TnoMfError):
+        P.tno_mf_search(ctx, f, np.ones(2, np.float32), np.array([[np.nan, 0, 0, 0]], np.float32), 1.0, 0.0, out)
+    with pytest.raises(P.TnoMfError):
+        P.tno_mf_search(ctx, f, np.ones(2, np.float32), np.zeros((1, 4), np.float32), 1.0, 0.0, None, None)
+    P.tno_mf_search(ctx, f, np.ones(2, np.float32), np.zeros((1, 4), np.float32), 1.0, 0.0, out)
+    torch.cuda.synchronize()
+    P.tno_mf_destroy(ctx)
