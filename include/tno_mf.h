@@ -68,7 +68,9 @@ typedef struct {
     float   snr_threshold;   /* candidate iff snr >= threshold; -INFINITY disables the cut */
     int32_t force_generic;   /* 0 = pick the fastest kernel that applies (normal use);
                                 1 = always use the generic (non-TMA) kernel -- for tests */
-    int32_t reserved[3];     /* must be 0 */
+    int32_t record_events;   /* != 0: bracket the main search kernel with CUDA events on the stream
+                                so that tno_mf_last_kernel_ms can report its duration */
+    int32_t reserved[2];     /* must be 0 */
 } tno_mf_config;
 
 /* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
@@ -119,6 +121,17 @@ int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, floa
  * returns): number of kernel launches enqueued, and which search kernel was used
  * (0 = generic, 1 = separable TMA kernel).  NULL pointers are skipped. */
 int tno_mf_last_stats(const tno_mf_ctx *ctx, int32_t *out_launches, int32_t *out_kernel);
+
+/* Duration in milliseconds of the main search kernel of the last tno_mf_search, measured with
+ * CUDA events recorded on the context's stream around that launch.  Needs
+ * cfg.record_events != 0 (else EINVAL).  Blocks the host until the kernel has finished. */
+int tno_mf_last_kernel_ms(tno_mf_ctx *ctx, float *out_ms);
+
+/* Work of the last tno_mf_search in FP32 multiply-adds of the formulation it executed
+ * (DESIGN.md "roofline"): the shared x-pass (5 per staged pixel and batch, halo rows included) and
+ * the per-trajectory y-pass (5 per trajectory x frame x pixel).  The generic kernel reports
+ * x = 0, y = 25 per evaluation.  NULL pointers are skipped. */
+int tno_mf_last_work(const tno_mf_ctx *ctx, double *out_fma_xpass, double *out_fma_ypass);
 
 /* Release the context and its workspace.  The caller must have synchronised the stream.
  * NULL is accepted. */

@@ -29,7 +29,7 @@ assert TRAJ_DTYPE.itemsize == 16 and CAND_DTYPE.itemsize == 16 and SOURCE_DTYPE.
 class tno_mf_config(ctypes.Structure):
     _fields_ = [("device", ctypes.c_int32), ("stream", ctypes.c_void_p), ("topk", ctypes.c_int32),
                 ("snr_threshold", ctypes.c_float), ("force_generic", ctypes.c_int32),
-                ("reserved", ctypes.c_int32 * 3)]
+                ("record_events", ctypes.c_int32), ("reserved", ctypes.c_int32 * 2)]
 
 
 class TnoMfError(RuntimeError):
@@ -55,6 +55,10 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_plan.argtypes = [vp, i32, i32, f32, i32, i32, vp, vp]
     lib.tno_mf_last_stats.restype = ctypes.c_int
     lib.tno_mf_last_stats.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32)]
+    lib.tno_mf_last_kernel_ms.restype = ctypes.c_int
+    lib.tno_mf_last_kernel_ms.argtypes = [vp, ctypes.POINTER(f32)]
+    lib.tno_mf_last_work.restype = ctypes.c_int
+    lib.tno_mf_last_work.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.tno_mf_destroy.restype = ctypes.c_int
     lib.tno_mf_destroy.argtypes = [vp]
     lib.tno_mf_last_error.restype = ctypes.c_char_p
@@ -81,10 +85,12 @@ def tno_mf_last_error(ctx=None) -> str:
 
 
 def tno_mf_create(device: int = 0, stream: Optional[int] = None, topk: int = 0,
-                  snr_threshold: float = float("-inf"), force_generic: bool = False):
+                  snr_threshold: float = float("-inf"), force_generic: bool = False,
+                  record_events: bool = False):
     """Returns an opaque context handle.  `stream` is a raw cudaStream_t (int) or None."""
     cfg = tno_mf_config(device=int(device), stream=ctypes.c_void_p(stream or 0), topk=int(topk),
-                        snr_threshold=float(snr_threshold), force_generic=int(bool(force_generic)))
+                        snr_threshold=float(snr_threshold), force_generic=int(bool(force_generic)),
+                        record_events=int(bool(record_events)))
     ctx = ctypes.c_void_p()
     _check(_lib.tno_mf_create(ctypes.byref(cfg), ctypes.byref(ctx)), None)
     return ctx
@@ -154,6 +160,20 @@ def tno_mf_last_stats(ctx) -> Tuple[int, int]:
     """(kernel launches of the last search, 1 if the separable TMA kernel was used else 0)."""
     a, b = ctypes.c_int32(), ctypes.c_int32()
     _check(_lib.tno_mf_last_stats(ctx, ctypes.byref(a), ctypes.byref(b)), None)
+    return a.value, b.value
+
+
+def tno_mf_last_kernel_ms(ctx) -> float:
+    """Duration (ms) of the main search kernel of the last search (needs record_events)."""
+    ms = ctypes.c_float()
+    _check(_lib.tno_mf_last_kernel_ms(ctx, ctypes.byref(ms)), ctx)
+    return ms.value
+
+
+def tno_mf_last_work(ctx) -> Tuple[float, float]:
+    """(x-pass, y-pass) FP32 multiply-adds of the formulation the last search executed."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.tno_mf_last_work(ctx, ctypes.byref(a), ctypes.byref(b)), None)
     return a.value, b.value
 
 

@@ -30,6 +30,9 @@ struct tno_mf_ctx {
     void *encode_fn = nullptr;
     std::string err;
     int32_t last_launches = 0, last_kernel = 0;
+    double last_fma_x = 0.0, last_fma_y = 0.0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
     // grow-only device workspace
     DevBuf meta, shift, g, gd, ab, rsd, stage_tab, scratch, keys, counts, tmp_maps, src;
 };
@@ -123,7 +126,7 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
     if (std::isnan(cfg->snr_threshold))
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
-    if (cfg->reserved[0] || cfg->reserved[1] || cfg->reserved[2])
+    if (cfg->reserved[0] || cfg->reserved[1])
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: reserved fields must be 0");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
@@ -153,7 +156,30 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         delete ctx;
         return fail(nullptr, TNO_MF_ECUDA, "tno_mf_create: cuTensorMapEncodeTiled not available in the driver");
     }
+    if (cfg->record_events) {
+        if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) {
+            cudaGetLastError();
+            delete ctx;
+            return fail(nullptr, TNO_MF_ECUDA, "tno_mf_create: cudaEventCreate failed");
+        }
+    }
     *out_ctx = ctx;
+    return TNO_MF_OK;
+}
+
+int tno_mf_last_kernel_ms(tno_mf_ctx *ctx, float *out_ms) {
+    if (!ctx || !out_ms) return TNO_MF_EINVAL;
+    if (!ctx->ev0 || !ctx->ev_valid)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_last_kernel_ms: no recorded search (cfg.record_events = 0?)");
+    CU_TRY(ctx, cudaEventSynchronize(ctx->ev1));
+    CU_TRY(ctx, cudaEventElapsedTime(out_ms, ctx->ev0, ctx->ev1));
+    return TNO_MF_OK;
+}
+
+int tno_mf_last_work(const tno_mf_ctx *ctx, double *out_fma_xpass, double *out_fma_ypass) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (out_fma_xpass) *out_fma_xpass = ctx->last_fma_x;
+    if (out_fma_ypass) *out_fma_ypass = ctx->last_fma_y;
     return TNO_MF_OK;
 }
 
@@ -164,6 +190,8 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
                       &ctx->scratch, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
     return TNO_MF_OK;
 }
@@ -416,9 +444,25 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
         a.n_sm = ctx->n_sm;
         int32_t grid = 0;
         const char *err = "";
+        if (ctx->ev0) CU_TRY(ctx, cudaEventRecord(ctx->ev0, st));
         if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
             return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
+        if (ctx->ev0) { CU_TRY(ctx, cudaEventRecord(ctx->ev1, st)); ctx->ev_valid = true; }
         ctx->last_launches += 1;
+        // work of the formulation: x-pass over staged rows (halo included), y-pass per entry
+        double rows_sum = 0.0;
+        for (const Batch &bt : plan.batches) {
+            for (int32_t t = 0; t < T; ++t) {
+                int32_t lo = INT32_MAX, hi = INT32_MIN;
+                for (int32_t k : bt.traj) {
+                    const int32_t s = plan.ycls[plan.traj_yc[k]].shift[t];
+                    lo = std::min(lo, s); hi = std::max(hi, s);
+                }
+                rows_sum += (double)(sv.tile_h + 4 + (hi - lo));
+            }
+        }
+        ctx->last_fma_x = 5.0 * rows_sum * 64.0 * (double)n_tiles;
+        ctx->last_fma_y = 5.0 * (double)n_traj * T * (double)H * W;
     } else {
         // generic path: maps are always materialised (caller's buffer, or a workspace chunk)
         const int64_t map_px = (int64_t)H * W;
@@ -430,6 +474,9 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
             if ((rc = reserve(ctx, ctx->tmp_maps, (size_t)chunk * map_px * 4))) return rc;
             maps = static_cast<float *>(ctx->tmp_maps.p);
         }
+        ctx->last_fma_x = 0.0;
+        ctx->last_fma_y = 25.0 * (double)n_traj * T * (double)H * W;
+        if (ctx->ev0) CU_TRY(ctx, cudaEventRecord(ctx->ev0, st));
         for (int32_t k0 = 0; k0 < n_traj; k0 += chunk) {
             const int32_t kc = std::min(chunk, n_traj - k0);
             float *dst = out_snr ? out_snr + (int64_t)k0 * map_px : maps;
@@ -440,6 +487,7 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
                 ctx->last_launches += 1;
             }
         }
+        if (ctx->ev0) { CU_TRY(ctx, cudaEventRecord(ctx->ev1, st)); ctx->ev_valid = true; }
         CU_TRY(ctx, cudaGetLastError());
     }
     if (want_topk) {

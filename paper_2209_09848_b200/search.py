@@ -12,13 +12,13 @@ class MatchedFilter:
     """One library context bound to the current torch CUDA stream of `device`."""
 
     def __init__(self, device: int = 0, topk: int = 0, snr_threshold: float = float("-inf"),
-                 force_generic: bool = False):
+                 force_generic: bool = False, record_events: bool = False):
         import torch
         self._torch = torch
         self.device = torch.device("cuda", device)
         self.topk = int(topk)
         stream = torch.cuda.current_stream(self.device).cuda_stream
-        self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic)
+        self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events)
 
     def close(self) -> None:
         if self.ctx is not None:
@@ -63,3 +63,9 @@ class MatchedFilter:
 
     def stats(self) -> Tuple[int, int]:
         return B.tno_mf_last_stats(self.ctx)
+
+    def kernel_ms(self) -> float:
+        return B.tno_mf_last_kernel_ms(self.ctx)
+
+    def work(self) -> Tuple[float, float]:
+        return B.tno_mf_last_work(self.ctx)
