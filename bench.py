@@ -165,7 +165,7 @@ def _workload(cfg):
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
-    from paper_2209_09848_b200 import MatchedFilter, make_sources  # noqa: F401
+    from paper_2209_09848_b200 import MatchedFilter, multi
 
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -178,11 +178,7 @@ def run_ours(args, cfg):
         dist.init_process_group("nccl", device_id=dev)
 
     # ---- inputs: one stack per rank (a different CCD each), generated on the device
-    rcfg = cfg if world == 1 else tno_synth.scaled(cfg)          # same shape; seed differs below
-    p = tno_synth.make_params(rcfg)
-    if world > 1:                                                 # decorrelate ranks: shift the noise seed
-        import dataclasses
-        p.cfg = dataclasses.replace(p.cfg, idx=cfg.idx + 10 * rank)
+    p = tno_synth.make_params(multi.rank_config(cfg, rank))       # rank-specific seed, same recipe
     frames = tno_synth.stack_torch(p, dev)
     mf = MatchedFilter(local, cfg.topk, cfg.threshold, record_events=True)
     mf.inject(frames, p.traj[p.src_k], p.src_x, p.src_y, p.src_amp, cfg.prf_sigma, cfg.t0)
@@ -217,13 +213,9 @@ def run_ours(args, cfg):
     if world > 1:
         dist.barrier()
     clocks = sampler.stop()
-    total_ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        tt = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = multi.max_over_ranks(ev0.elapsed_time(ev1), dev)
     ms_per_step = total_ms / args.steps
-    value = cfg.evals * world / (ms_per_step * 1e-3)
+    value = multi.aggregate_value(cfg.evals, world, ms_per_step)
 
     # ---- end to end through the C ABI with HOST buffers (H2D of the stack, D2H of the results)
     e2e = None
@@ -251,14 +243,10 @@ def run_ours(args, cfg):
                 host_snr.copy_(out_snr, non_blocking=True)
         e1.record()
         torch.cuda.synchronize()
-        e2e_ms = e0.elapsed_time(e1) / e2e_steps
-        if world > 1:
-            tt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_ms = float(tt.item())
+        e2e_ms = multi.max_over_ranks(e0.elapsed_time(e1) / e2e_steps, dev)
         h2d = frames.numel() * 4
         d2h = out_topk.numel() * 4 + (out_snr.numel() * 4 if cfg.want_maps else 0)
-        e2e = {"value": cfg.evals * world / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+        e2e = {"value": multi.aggregate_value(cfg.evals, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
                "steps": e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "host_memory": "pinned" if pinned else "pageable"}
         del host_frames, host_snr

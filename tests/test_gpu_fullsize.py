@@ -1,0 +1,151 @@
+"""GPU parity at BASELINE.json's full sizes (configs 3, 4, 5), in the launch configuration
+bench.py times.  The full oracle would take ~10 min - 1 h per config, so parity is checked on
+(i) full-T oracle maps of 256 x 256 crops (interior, edges, corner) for a spread of trajectories,
+(ii) oracle_point at every sampled GPU candidate, every injected source, hot pixels and random
+(k, x, y), (iii) the GPU candidate lists against a plain sort of the GPU's own maps.
+Needs a B200 with ~100 GB of free HBM and ~100 GB of host RAM (config 4).  `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import oracle
+import tno_synth
+from helpers import TOL, check_topk_vs_own_map
+
+pytestmark = pytest.mark.gpu
+
+
+def _setup(cfg):
+    import torch
+    from paper_2209_09848_b200 import MatchedFilter
+    assert torch.cuda.is_available()
+    dev = torch.device("cuda", 0)
+    p = tno_synth.make_params(cfg)
+    frames = tno_synth.stack_torch(p, dev)
+    mf = MatchedFilter(0, cfg.topk, cfg.threshold)
+    mf.inject(frames, p.traj[p.src_k], p.src_x, p.src_y, p.src_amp, cfg.prf_sigma, cfg.t0)
+    torch.cuda.synchronize()
+    return torch, mf, p, frames
+
+
+def _spread_trajs(p, n):
+    speed = np.hypot(p.traj[:, 0], p.traj[:, 1]) + 1e3 * np.hypot(p.traj[:, 2], p.traj[:, 3])
+    order = np.argsort(speed, kind="stable")
+    return np.unique(order[np.linspace(0, len(order) - 1, n).round().astype(int)])
+
+
+def _crops(cfg, size=256):
+    H, W = cfg.H, cfg.W
+    return [((W - size) // 2 + 37, (H - size) // 2 - 53),     # interior, not tile aligned
+            (0, (H - size) // 3),                             # left edge
+            ((W - size) // 3, 0),                             # top edge
+            (W - size, H - size)]                             # bottom-right corner
+
+
+def _check_points(host, p, cfg, pts, gpu_vals):
+    worst = 0.0
+    for (k, x, y), g in zip(pts, gpu_vals):
+        s, _, _ = oracle.point(host, p.sigma_t, p.traj[k], cfg.prf_sigma, cfg.t0, int(x), int(y))
+        worst = max(worst, abs(float(g) - s))
+        assert abs(float(g) - s) <= TOL, (k, x, y, float(g), s)
+    return worst
+
+
+def _fullsize_with_maps(cfg, n_crop_traj, n_random):
+    torch, mf, p, frames = _setup(cfg)
+    maps, cand = mf.search(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0)
+    torch.cuda.synchronize()
+    assert mf.stats()[1] == 1, "the separable TMA kernel must be the one bench.py times"
+    c = mf.candidates_to_numpy(cand)
+    host = frames.cpu().numpy()
+    del frames
+    rng = np.random.default_rng(cfg.seed)
+    # (i) crops against the hoisted oracle, evaluated against the full frames (real borders)
+    ks = _spread_trajs(p, n_crop_traj)
+    for (cx, cy) in _crops(cfg):
+        om = oracle.snr_map(host, p.sigma_t, p.traj[ks], cfg.prf_sigma, cfg.t0,
+                            region=(cx, cx + 256, cy, cy + 256))
+        gm = maps[torch.from_numpy(ks).cuda()][:, cy:cy + 256, cx:cx + 256].cpu().numpy()
+        err = np.abs(gm.astype(np.float64) - om)
+        assert err.max() <= TOL, (cx, cy, err.max(), np.unravel_index(err.argmax(), err.shape))
+    # (iii) candidate lists = plain sort of the GPU's own maps (all trajectories)
+    for k in range(cfg.n_traj):
+        check_topk_vs_own_map(c[k], maps[k].cpu().numpy(), k, cfg.topk, cfg.threshold)
+    # (ii) literal oracle at sampled candidates, all sources, hot pixels, random points
+    pts, vals = [], []
+    for k in ks:
+        for r in c[k][: min(cfg.topk, 25)]:
+            if r["x"] >= 0:
+                pts.append((int(k), int(r["x"]), int(r["y"])))
+                vals.append(r["snr"])
+    for k in range(cfg.n_traj):
+        if c[k]["x"][0] >= 0:
+            pts.append((k, int(c[k]["x"][0]), int(c[k]["y"][0])))
+            vals.append(c[k]["snr"][0])
+    for i in range(len(p.src_k)):
+        pts.append((int(p.src_k[i]), int(p.src_x[i]), int(p.src_y[i])))
+    for hp in p.hot_pos[:12]:
+        pts.append((int(ks[0]), int(hp % cfg.W), int(hp // cfg.W)))
+    for _ in range(n_random):
+        pts.append((int(rng.integers(cfg.n_traj)), int(rng.integers(cfg.W)), int(rng.integers(cfg.H))))
+    idx = torch.tensor([[k, y, x] for k, x, y in pts[len(vals):]], device="cuda")
+    vals += maps[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy().tolist()
+    _check_points(host, p, cfg, pts, vals)
+    # every injected source stands out at its own trajectory and start pixel
+    for i in range(len(p.src_k)):
+        s = float(maps[int(p.src_k[i]), int(p.src_y[i]), int(p.src_x[i])])
+        assert s > 0.5 * float(p.src_amp[i]) * np.sqrt(cfg.T * np.pi) / 1.2
+    mf.close()
+
+
+def test_config3_headline_sampled_parity():
+    _fullsize_with_maps(tno_synth.CONFIGS[3], n_crop_traj=8, n_random=3000)
+
+
+def test_config4_long_sector_sampled_parity():
+    _fullsize_with_maps(tno_synth.CONFIGS[4], n_crop_traj=6, n_random=600)
+
+
+def test_config5_curved_topk_only():
+    cfg = tno_synth.CONFIGS[5]
+    torch, mf, p, frames = _setup(cfg)
+    _, cand = mf.search(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0, want_maps=False)
+    torch.cuda.synchronize()
+    assert mf.stats()[1] == 1
+    c = mf.candidates_to_numpy(cand)
+    assert c.shape == (1024, 100) and np.all(c["k"] == np.arange(1024)[:, None])
+    # map mode on 16 trajectories covering the four accelerations: same kernel, maps visible
+    sub = np.array([0, 17, 100, 255, 256, 300, 400, 511, 512, 600, 700, 767, 768, 850, 900, 1023])
+    maps, cand_s = mf.search(frames, p.sigma_t, p.traj[sub], cfg.prf_sigma, cfg.t0)
+    torch.cuda.synchronize()
+    cs = mf.candidates_to_numpy(cand_s)
+    host = frames.cpu().numpy()
+    del frames
+    for j, k in enumerate(sub):
+        gm = maps[j].cpu().numpy()
+        check_topk_vs_own_map(cs[j], gm, j, cfg.topk, cfg.threshold)
+        # the list-only run returns the same candidates for this trajectory
+        assert np.array_equal(cs[j]["x"], c[k]["x"]) and np.array_equal(cs[j]["y"], c[k]["y"])
+        assert np.array_equal(cs[j]["snr"], c[k]["snr"])
+    # crops of the sub-run maps against the hoisted oracle
+    for (cx, cy) in _crops(cfg)[:2] + _crops(cfg)[3:]:
+        pick = [1, 6, 9, 15]
+        om = oracle.snr_map(host, p.sigma_t, p.traj[sub[pick]], cfg.prf_sigma, cfg.t0,
+                            region=(cx, cx + 256, cy, cy + 256))
+        gm = maps[pick][:, cy:cy + 256, cx:cx + 256].cpu().numpy()
+        assert np.abs(gm.astype(np.float64) - om).max() <= TOL
+    # literal oracle at returned candidates: all of 24 trajectories, the best 2 of every trajectory
+    pts, vals = [], []
+    for k in list(range(0, 1024, 43)):
+        for r in c[k]:
+            if r["x"] >= 0:
+                pts.append((k, int(r["x"]), int(r["y"]))); vals.append(r["snr"])
+    for k in range(1024):
+        for r in c[k][:2]:
+            if r["x"] >= 0:
+                pts.append((k, int(r["x"]), int(r["y"]))); vals.append(r["snr"])
+    assert len(pts) > 3000
+    _check_points(host, p, cfg, pts, vals)
+    for k in range(1024):                                   # lists are ordered and above threshold
+        v = c[k][c[k]["x"] >= 0]
+        assert np.all(v["snr"][:-1] >= v["snr"][1:]) and np.all(v["snr"] >= cfg.threshold)
+    mf.close()
