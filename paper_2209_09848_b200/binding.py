@@ -41,7 +41,7 @@ class TnoMfError(RuntimeError):
 def _load() -> ctypes.CDLL:
     if not os.path.exists(LIB_PATH):
         raise ImportError(
-            "%s is missing: build it with `python -m paper_2209_09848_b200.build` "
+            "%s is missing: build it with `python paper_2209_09848_b200/build.py` "
             "(nvcc, sm_100a).  There is no CPU fallback." % LIB_PATH)
     lib = ctypes.CDLL(LIB_PATH)
     vp, i32, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_float

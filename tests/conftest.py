@@ -10,3 +10,6 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on a B200)")
+    # a fresh checkout has no built libraries: compile them once (nvcc cross-compiles without a GPU)
+    import __graft_entry__
+    __graft_entry__.build()
