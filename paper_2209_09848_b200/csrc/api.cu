@@ -31,10 +31,10 @@ struct tno_mf_ctx {
     std::string err;
     int32_t last_launches = 0, last_kernel = 0;
     double last_fma_x = 0.0, last_fma_y = 0.0;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    bool ev_valid = false;
+    std::vector<cudaEvent_t> ev;      // pairs (before, after) around each main search kernel launch
+    int32_t ev_used = 0;              // events recorded by the last search
     // grow-only device workspace
-    DevBuf meta, shift, g, gd, ab, rsd, stage_tab, scratch, keys, counts, tmp_maps, src;
+    DevBuf meta, shift, g, gd, ab, rsd, stage_tab, pieces, keys, counts, tmp_maps, src;
 };
 
 namespace {
@@ -109,6 +109,25 @@ AxisBorder make_border(const AxisClass &c, int32_t L) {
 
 bool finite_f(float v) { return std::isfinite(v); }
 
+// Record the next event of the (before, after) pairs that bracket the main search kernels.
+int record_event(tno_mf_ctx *ctx) {
+    if (!ctx->cfg.record_events) return TNO_MF_OK;
+    if (ctx->ev_used == (int32_t)ctx->ev.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(ctx, TNO_MF_ECUDA, "cudaEventCreate failed");
+        }
+        ctx->ev.push_back(e);
+    }
+    if (cudaEventRecord(ctx->ev[ctx->ev_used], ctx->stream) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, TNO_MF_ECUDA, "cudaEventRecord failed");
+    }
+    ++ctx->ev_used;
+    return TNO_MF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -156,23 +175,22 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         delete ctx;
         return fail(nullptr, TNO_MF_ECUDA, "tno_mf_create: cuTensorMapEncodeTiled not available in the driver");
     }
-    if (cfg->record_events) {
-        if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) {
-            cudaGetLastError();
-            delete ctx;
-            return fail(nullptr, TNO_MF_ECUDA, "tno_mf_create: cudaEventCreate failed");
-        }
-    }
     *out_ctx = ctx;
     return TNO_MF_OK;
 }
 
 int tno_mf_last_kernel_ms(tno_mf_ctx *ctx, float *out_ms) {
     if (!ctx || !out_ms) return TNO_MF_EINVAL;
-    if (!ctx->ev0 || !ctx->ev_valid)
+    if (ctx->ev_used < 2)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_last_kernel_ms: no recorded search (cfg.record_events = 0?)");
-    CU_TRY(ctx, cudaEventSynchronize(ctx->ev1));
-    CU_TRY(ctx, cudaEventElapsedTime(out_ms, ctx->ev0, ctx->ev1));
+    float total = 0.f;
+    for (int32_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+        float ms = 0.f;
+        CU_TRY(ctx, cudaEventSynchronize(ctx->ev[i + 1]));
+        CU_TRY(ctx, cudaEventElapsedTime(&ms, ctx->ev[i], ctx->ev[i + 1]));
+        total += ms;
+    }
+    *out_ms = total;
     return TNO_MF_OK;
 }
 
@@ -187,11 +205,10 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     if (!ctx) return TNO_MF_OK;
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
-                      &ctx->scratch, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src};
+                      &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
-    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
-    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     delete ctx;
     return TNO_MF_OK;
 }
@@ -256,6 +273,7 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
                   float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
+    ctx->ev_used = 0;
     // ------------------------------------------------------------------ validation
     if (!frames || !sigma_t || !trajectories)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: NULL frames, sigma_t or trajectories");
@@ -288,22 +306,32 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
     const int32_t n_cls = n_x + n_y;
     if (n_cls > 65535) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: too many distinct axis motions");
 
-    const bool use_sep = !ctx->cfg.force_generic && (W % 4 == 0) &&
-                         ((reinterpret_cast<uintptr_t>(frames) & 15u) == 0) && W >= 4;
-    int32_t variant = -1;
+    // The separable kernel needs TMA-compatible frames (W % 4 == 0, 16-byte aligned) and a piece
+    // count (1 + ceil(y-shift range / tile height)) that stays small.
+    bool use_sep = !ctx->cfg.force_generic && (W % 4 == 0) &&
+                   ((reinterpret_cast<uintptr_t>(frames) & 15u) == 0) && W >= 4;
+    int32_t variant = -1, n_pieces = 1;
+    SepVariant sv = {0, 0};
     if (use_sep) {
+        // variant = batch capacity; cost = x-pass per batch + y-pass per entry (FFMA per pixel), ties
+        // go to the smaller capacity (fewer partially filled batches)
         double best = 0.0;
         Plan trial = plan;
         for (int32_t v = 0; v < sep_num_variants(); ++v) {
-            const SepVariant sv = sep_variant(v);
-            build_batches(&trial, sv.nb, sv.max_spread);
-            const double cost = (double)trial.batches.size() * (sv.nb + 1.5);
+            build_batches(&trial, sep_variant(v).nb, kUnlimitedSpread);
+            double cost = 0.0;
+            for (const Batch &bt : trial.batches) cost += 5.3 + 5.0 * (double)bt.traj.size();
             if (variant < 0 || cost < best) {
                 best = cost;
                 variant = v;
                 plan.batches = trial.batches;
             }
         }
+        sv = sep_variant(variant);
+        int64_t range = 0;
+        for (const AxisClass &c : plan.ycls) range = std::max<int64_t>(range, (int64_t)c.smax - c.smin);
+        const int64_t np = 1 + (range + sv.tile_h - 1) / sv.tile_h;
+        if (np > 64) use_sep = false; else n_pieces = (int32_t)np;
     }
     ctx->last_kernel = use_sep ? 1 : 0;
 
@@ -342,23 +370,28 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
         rsd_total += cells;
         max_cells = std::max(max_cells, cells);
     }
-    SepVariant sv = {0, 0, 0};
+    // planned order q: batches in order, entries in order (slots 0 .. n-1 of the batch)
     int32_t n_batches = 0;
-    std::vector<int32_t> batch_xc, batch_yc, batch_traj;
+    std::vector<int32_t> batch_xc, batch_yc, batch_q, perm, batch_q0;
     if (use_sep) {
-        sv = sep_variant(variant);
         n_batches = (int32_t)plan.batches.size();
         batch_xc.resize(n_batches);
         batch_yc.assign((size_t)n_batches * sv.nb, -1);
-        batch_traj.assign((size_t)n_batches * sv.nb, -1);
+        batch_q.assign((size_t)n_batches * sv.nb, -1);
+        batch_q0.resize(n_batches + 1);
+        perm.reserve(n_traj);
         for (int32_t b = 0; b < n_batches; ++b) {
             const Batch &bt = plan.batches[b];
             batch_xc[b] = bt.xcls;
-            for (size_t s = 0; s < bt.traj.size(); ++s) {
-                batch_traj[(size_t)b * sv.nb + s] = bt.traj[s];
-                batch_yc[(size_t)b * sv.nb + s] = plan.traj_yc[bt.traj[s]];
+            batch_q0[b] = (int32_t)perm.size();
+            for (size_t j = 0; j < bt.traj.size(); ++j) {
+                const size_t slot = j;
+                batch_q[(size_t)b * sv.nb + slot] = (int32_t)perm.size();
+                batch_yc[(size_t)b * sv.nb + slot] = plan.traj_yc[bt.traj[j]];
+                perm.push_back(bt.traj[j]);
             }
         }
+        batch_q0[n_batches] = (int32_t)perm.size();
     }
     Blob blob;
     const size_t o_v = blob.add(cls_v.data(), cls_v.size() * 4);
@@ -370,7 +403,8 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
     const size_t o_ti = blob.add(tinfo.data(), tinfo.size() * sizeof(TrajInfo));
     const size_t o_bx = blob.add(batch_xc.data(), batch_xc.size() * 4);
     const size_t o_by = blob.add(batch_yc.data(), batch_yc.size() * 4);
-    const size_t o_bt = blob.add(batch_traj.data(), batch_traj.size() * 4);
+    const size_t o_bq = blob.add(batch_q.data(), batch_q.size() * 4);
+    const size_t o_perm = blob.add(perm.data(), perm.size() * 4);
 
     // ------------------------------------------------------------------ workspace
     int rc;
@@ -381,16 +415,33 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
     if ((rc = reserve(ctx, ctx->gd, ct * 5 * 8))) return rc;
     if ((rc = reserve(ctx, ctx->ab, (size_t)ab_total * 8))) return rc;
     if ((rc = reserve(ctx, ctx->rsd, (size_t)rsd_total * 4))) return rc;
-    const int32_t tile_h = use_sep ? sv.tile_h : kCollectTile;
-    const int32_t ntx = (W + 63) / 64, nty = (H + tile_h - 1) / tile_h;
-    const int64_t n_tiles = (int64_t)ntx * nty;
+    const int32_t ntx = (W + kCollectTile - 1) / kCollectTile, nty = (H + kCollectTile - 1) / kCollectTile;
+    const int64_t n_tiles = (int64_t)ntx * nty;           // candidate tiles (64 x 64 start pixels)
     if (want_topk) {
         if ((rc = reserve(ctx, ctx->keys, (size_t)n_tiles * n_traj * ctx->cfg.topk * 8))) return rc;
         if ((rc = reserve(ctx, ctx->counts, (size_t)n_tiles * n_traj * 4))) return rc;
     }
+    // piece buffer: n_pieces partial-sum maps per entry; the bank is processed in chunks of whole
+    // batches when it does not fit the budget (<= 40 GB and <= 80 % of what the device has free)
+    const int64_t map_px = (int64_t)H * W;
+    int64_t chunk_cap = n_traj;                            // entries per chunk
     if (use_sep) {
         if ((rc = reserve(ctx, ctx->stage_tab, (size_t)n_batches * T * sep_table_words(variant) * 4))) return rc;
-        if ((rc = reserve(ctx, ctx->scratch, (size_t)ctx->n_sm * sep_scratch_floats_per_cta(variant) * 4))) return rc;
+        const size_t per_entry = (size_t)n_pieces * map_px * 4;
+        const size_t want = per_entry * n_traj;
+        if (want > ctx->pieces.cap) {
+            size_t free_b = 0, total_b = 0;
+            CU_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));
+            const size_t avail = (size_t)((double)(free_b + ctx->pieces.cap) * 0.8);
+            const size_t budget = std::min<size_t>(want, std::min<size_t>(avail, (size_t)40 << 30));
+            chunk_cap = (int64_t)(budget / per_entry);
+            if (chunk_cap < sv.nb && chunk_cap < n_traj)
+                return fail(ctx, TNO_MF_ENOMEM, "not enough device memory for the partial-sum buffer "
+                            "(%zu bytes per trajectory, %zu available)", per_entry, avail);
+            chunk_cap = std::min<int64_t>(chunk_cap, n_traj);
+            if ((rc = reserve(ctx, ctx->pieces, per_entry * (size_t)chunk_cap))) return rc;
+        }
+        chunk_cap = std::min<int64_t>((int64_t)(ctx->pieces.cap / per_entry), n_traj);
     }
     unsigned char *meta = static_cast<unsigned char *>(ctx->meta.p);
     CU_TRY(ctx, cudaMemcpyAsync(meta, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st));
@@ -401,6 +452,8 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
     tab.gd = static_cast<const double *>(ctx->gd.p);
     tab.qf = reinterpret_cast<const float *>(meta + o_qf);
     tab.qd = reinterpret_cast<const double *>(meta + o_qd);
+    tab.cls_v = reinterpret_cast<const float *>(meta + o_v);
+    tab.cls_a = reinterpret_cast<const float *>(meta + o_a);
     tab.n_x = n_x;
     tab.T = T;
     const TrajInfo *d_ti = reinterpret_cast<const TrajInfo *>(meta + o_ti);
@@ -431,41 +484,43 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
                           static_cast<float *>(ctx->stage_tab.p));
         ctx->last_launches += 1;
         CU_TRY(ctx, cudaGetLastError());
-        SepArgs a;
-        a.frames = frames; a.T = T; a.H = H; a.W = W;
-        a.stage_tab = static_cast<const float *>(ctx->stage_tab.p);
-        a.batch_traj = reinterpret_cast<const int32_t *>(meta + o_bt);
-        a.n_batches = n_batches;
-        a.traj = d_ti;
-        a.rsd = d_rsd;
-        a.out_snr = out_snr;
-        a.slots = slots;
-        a.scratch = static_cast<float *>(ctx->scratch.p);
-        a.n_sm = ctx->n_sm;
-        int32_t grid = 0;
-        const char *err = "";
-        if (ctx->ev0) CU_TRY(ctx, cudaEventRecord(ctx->ev0, st));
-        if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
-            return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
-        if (ctx->ev0) { CU_TRY(ctx, cudaEventRecord(ctx->ev1, st)); ctx->ev_valid = true; }
-        ctx->last_launches += 1;
-        // work of the formulation: x-pass over staged rows (halo included), y-pass per entry
-        double rows_sum = 0.0;
-        for (const Batch &bt : plan.batches) {
-            for (int32_t t = 0; t < T; ++t) {
-                int32_t lo = INT32_MAX, hi = INT32_MIN;
-                for (int32_t k : bt.traj) {
-                    const int32_t s = plan.ycls[plan.traj_yc[k]].shift[t];
-                    lo = std::min(lo, s); hi = std::max(hi, s);
-                }
-                rows_sum += (double)(sv.tile_h + 4 + (hi - lo));
-            }
+        const int32_t tabw = sep_table_words(variant);
+        for (int32_t b0 = 0; b0 < n_batches;) {
+            int32_t b1 = b0 + 1;
+            while (b1 < n_batches && batch_q0[b1 + 1] - batch_q0[b0] <= chunk_cap) ++b1;
+            const int32_t q0 = batch_q0[b0], qn = batch_q0[b1] - q0;
+            SepArgs a;
+            a.frames = frames; a.T = T; a.H = H; a.W = W;
+            a.stage_tab = static_cast<const float *>(ctx->stage_tab.p) + (size_t)b0 * T * tabw;
+            a.batch_q = reinterpret_cast<const int32_t *>(meta + o_bq) + (size_t)b0 * sv.nb;
+            a.n_batches = b1 - b0;
+            a.q0 = q0;
+            a.pieces = static_cast<float *>(ctx->pieces.p);
+            a.piece_stride = (int64_t)qn * map_px;
+            a.n_pieces = n_pieces;
+            a.n_sm = ctx->n_sm;
+            CU_TRY(ctx, cudaMemsetAsync(a.pieces, 0, (size_t)n_pieces * a.piece_stride * 4, st));
+            int32_t grid = 0;
+            const char *err = "";
+            if ((rc = record_event(ctx))) return rc;
+            if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
+                return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
+            if ((rc = record_event(ctx))) return rc;
+            launch_finish(st, a.pieces, n_pieces, a.piece_stride, reinterpret_cast<const int32_t *>(meta + o_perm),
+                          q0, qn, d_ti, d_rsd, H, W, out_snr, slots);
+            CU_TRY(ctx, cudaGetLastError());
+            ctx->last_launches += 3;                       // memset, search, finish
+            b0 = b1;
         }
-        ctx->last_fma_x = 5.0 * rows_sum * 64.0 * (double)n_tiles;
+        // work of the formulation: x-pass over the staged rows of every (tile, batch, frame),
+        // y-pass per trajectory x frame x start pixel
+        double rows = 0.0;
+        for (int32_t ty = 0; ty < sep_tile_rows(variant, H); ++ty)
+            rows += (double)(std::min(sv.tile_h, H + 2 - (ty * sv.tile_h - 2)) + 4);
+        ctx->last_fma_x = 5.0 * rows * 64.0 * (double)((W + 63) / 64) * (double)n_batches * T;
         ctx->last_fma_y = 5.0 * (double)n_traj * T * (double)H * W;
     } else {
         // generic path: maps are always materialised (caller's buffer, or a workspace chunk)
-        const int64_t map_px = (int64_t)H * W;
         int32_t chunk = n_traj;
         float *maps = out_snr;
         if (!out_snr) {
@@ -476,7 +531,7 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
         }
         ctx->last_fma_x = 0.0;
         ctx->last_fma_y = 25.0 * (double)n_traj * T * (double)H * W;
-        if (ctx->ev0) CU_TRY(ctx, cudaEventRecord(ctx->ev0, st));
+        if ((rc = record_event(ctx))) return rc;
         for (int32_t k0 = 0; k0 < n_traj; k0 += chunk) {
             const int32_t kc = std::min(chunk, n_traj - k0);
             float *dst = out_snr ? out_snr + (int64_t)k0 * map_px : maps;
@@ -487,7 +542,7 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
                 ctx->last_launches += 1;
             }
         }
-        if (ctx->ev0) { CU_TRY(ctx, cudaEventRecord(ctx->ev1, st)); ctx->ev_valid = true; }
+        if ((rc = record_event(ctx))) return rc;
         CU_TRY(ctx, cudaGetLastError());
     }
     if (want_topk) {

@@ -16,6 +16,8 @@ struct ClassTables {
     const double *gd;
     const float *qf;      // [T] 1 / sigma_t^2
     const double *qd;     // [T]
+    const float *cls_v;   // [n classes] velocity of the class (px/frame)
+    const float *cls_a;   // [n classes] parallax term (px/frame^2)
     int32_t n_x;          // number of x-classes (y-class j is class n_x + j)
     int32_t T;
 };

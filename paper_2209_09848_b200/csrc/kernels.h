@@ -41,32 +41,36 @@ void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t
 // ---- search_sep.cu ----
 struct SepVariant {
     int32_t nb;           // entries per batch
-    int32_t tile_h;       // output tile height (tile width is 64)
-    int32_t max_spread;   // largest y-shift spread a batch may have
+    int32_t tile_h;       // positions (frame rows) per tile; the tile width is 64 columns
 };
 int32_t sep_num_variants();
 SepVariant sep_variant(int32_t v);
-// per-(batch, frame) stage table size in 32-bit words for variant v
+// per-(batch, frame) stage table size in 32-bit words
 int32_t sep_table_words(int32_t v);
+// tile rows of the position space [-2, H + 2)
+int32_t sep_tile_rows(int32_t v, int32_t H);
 void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
                        const int32_t *batch_yc /* [n_batches][nb], -1 = empty */, int32_t n_batches,
                        float *stage_tab);
 struct SepArgs {
     const float *frames;
     int32_t T, H, W;
-    const float *stage_tab;       // [n_batches][T][table_words]
-    const int32_t *batch_traj;    // [n_batches][nb] trajectory index or -1
-    int32_t n_batches;
-    const TrajInfo *traj;
-    const float *rsd;
-    float *out_snr;               // may be NULL
-    TopkSlots slots;              // slots.keys may be NULL
-    float *scratch;               // [grid][tile_h*64*nb] partial sums
+    const float *stage_tab;       // [n_batches][T][table_words], first batch of the chunk
+    const int32_t *batch_q;       // [n_batches][nb] planned-order index q of each slot, or -1
+    int32_t n_batches;            // batches of the chunk
+    int32_t q0;                   // first planned-order index of the chunk
+    float *pieces;                // [n_pieces][chunk entries][H][W] partial sums, zero on entry
+    int64_t piece_stride;         // floats between pieces = chunk entries * H * W
+    int32_t n_pieces;
     int32_t n_sm;
 };
 // returns cudaError_t-like code (0 ok); *grid_out = number of CTAs used
 int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode_fn, int32_t *grid_out,
                       const char **err);
-size_t sep_scratch_floats_per_cta(int32_t v);
+// SNR = (sum of pieces) * D^(-1/2) for entries q0 .. q0 + q_count of the planned order (perm[q] =
+// trajectory); maps to out_snr (may be NULL), candidates to the 64 x 64 tile slots (keys may be NULL)
+void launch_finish(cudaStream_t st, const float *pieces, int32_t n_pieces, int64_t piece_stride,
+                   const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
+                   int32_t H, int32_t W, float *out_snr, const TopkSlots &slots);
 
 }  // namespace tno

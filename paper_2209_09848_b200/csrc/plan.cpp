@@ -83,6 +83,29 @@ void build_batches(Plan *plan, int32_t max_entries, int32_t max_spread) {
         Batch cur;
         cur.xcls = (int32_t)xc;
         cur.max_spread = 0;
+        if (max_spread >= kUnlimitedSpread) {
+            // no spread limit (the trajectory-following kernel): split the class into the fewest
+            // batches, of sizes that differ by at most one
+            const int32_t n = (int32_t)ks.size();
+            const int32_t nbt = (n + max_entries - 1) / max_entries;
+            int32_t pos = 0;
+            for (int32_t j = 0; j < nbt; ++j) {
+                const int32_t len = n / nbt + (j < n % nbt ? 1 : 0);
+                cur.traj.assign(ks.begin() + pos, ks.begin() + pos + len);
+                pos += len;
+                for (int32_t t = 0; t < T; ++t) {
+                    int32_t l = INT32_MAX, h = INT32_MIN;
+                    for (int32_t k : cur.traj) {
+                        const int32_t sh = plan->ycls[plan->traj_yc[k]].shift[t];
+                        l = std::min(l, sh); h = std::max(h, sh);
+                    }
+                    cur.max_spread = std::max(cur.max_spread, h - l);
+                }
+                plan->batches.push_back(cur);
+                cur.max_spread = 0;
+            }
+            continue;
+        }
         for (int32_t k : ks) {
             const std::vector<int32_t> &s = plan->ycls[plan->traj_yc[k]].shift;
             bool fits = !cur.traj.empty() && (int32_t)cur.traj.size() < max_entries;

@@ -44,6 +44,9 @@ int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0,
 // Pack the trajectories of each x-class into batches of at most max_entries entries whose integer
 // y-shifts never differ by more than max_spread in any frame.  Entries are ordered by (vy, ay) so
 // that neighbours move alike.  A single trajectory always fits (spread 0).
+// max_spread >= kUnlimitedSpread (what the search itself uses): no spread limit, and each x-class
+// is split into the fewest batches, of sizes that differ by at most one.
+constexpr int32_t kUnlimitedSpread = 1 << 30;
 void build_batches(Plan *plan, int32_t max_entries, int32_t max_spread);
 
 }  // namespace tno
