@@ -86,29 +86,35 @@ constexpr int kBoxW = 76;    // staged columns: 64 + 4 halo + up to 3 of alignme
 constexpr int kXP = 68;      // pitch of the X rows (words), = 4 mod 32
 constexpr int kSeg = 64;     // an entry's accumulators are flushed at least every kSeg frames
 constexpr int kHdr = 16;     // header words of a stage table entry
+constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per warpgroup)
 // stage table entry (32-bit words), one per (batch, frame t):
 //   [0] xo = 4*floor((sx - 2)/4), the 16-byte aligned x offset of the staged box relative to the tile
 //   [1] o = sx - 2 - xo in 0..3, the column of the box at which the 5-tap window of output 0 starts
 //   [2] number of entries of the batch (they occupy slots 0 .. n-1)
 //   [3] flush mask: bit e set if entry e must be flushed after this frame
 //   [4..8] gx[0..4]
-//   [9] xo of frame t + STAGES - 1 (look-ahead for the producer)
 //   [16 + 8e + 0..4] gy_e[0..4] / sigma_t^2   [16 + 8e + 5] d_{e,t}          (entry e; zeros if empty)
 
-template <int R_, int NB_, int RG_, int STAGES_>
+template <int R_, int NB_, int CW_, int SB_, int XR_>
 struct SepCfg {
-    static constexpr int R = R_, NB = NB_, RG = RG_, STAGES = STAGES_;
-    static constexpr int NW = RG;                  // warps: warp w owns positions w*R .. w*R + R - 1
-    static constexpr int NT = 32 * NW;
-    static constexpr int HT = R * RG;              // positions (rows) per tile
+    static constexpr int R = R_, NB = NB_, CW = CW_, SB = SB_, XR = XR_;
+    static constexpr int NT = 32 * (CW + kPW);     // consumer warps 0 .. CW-1, then the producer warpgroup
+    static constexpr int HT = R * CW;              // positions (rows) per tile: consumer warp w owns w*R ..
     static constexpr int XROWS = HT + 4;
+    static constexpr int TS = 16;                  // table stages, >= SB + XR + 2 (ring invariants in the kernel)
     static constexpr int TABW = kHdr + 8 * NB;
-    static constexpr int RBUF = (XROWS * kBoxW + 31) / 32 * 32;   // floats per stage (128-byte multiple)
+    static constexpr int RBUF = (XROWS * kBoxW + 31) / 32 * 32;   // floats per box stage (128-byte multiple)
     static constexpr int XBUF = XROWS * kXP;                      // floats per X buffer
     static constexpr uint32_t BOX_BYTES = XROWS * kBoxW * 4;
-    static constexpr size_t SMEM = (size_t)(STAGES * RBUF + 2 * XBUF + STAGES * TABW) * 4 + STAGES * 8 + 64;
+    static constexpr int NBAR = SB + 2 * XR + NB;
+    static constexpr size_t SMEM = (size_t)(SB * RBUF + XR * XBUF + TS * TABW) * 4 + NBAR * 8 + 64;
+    // register split: setmaxnreg moves registers between the warpgroups of the CTA, the total stays
+    // what the launch allocated (NT x 128 with __launch_bounds__(512, 1))
+    static constexpr int CREGS = 160, PREGS = 32;
+    static_assert((SB & (SB - 1)) == 0 && (XR & (XR - 1)) == 0 && (TS & (TS - 1)) == 0 && TS >= SB + XR + 2,
+                  "ring sizes are powers of two");
     static_assert((TABW * 4) % 16 == 0 && (XBUF * 4) % 16 == 0, "16-byte alignment of the sections");
-    static_assert(NW % 8 == 0, "the order of the two passes alternates between halves of each SM sub-partition");
+    static_assert(CW % 4 == 0 && NT == 512 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * 128, "register budget");
 };
 
 // Phase of an entry's periodic flush: a function of its y-motion alone, so that the summation order
@@ -138,8 +144,6 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
     outi[0] = align4(sxm2);
     outi[1] = sxm2 - align4(sxm2);
     for (int i = 0; i < 5; ++i) out[4 + i] = tab.g[((int64_t)xc * T + t) * 5 + i];
-    const int32_t f = t + C::STAGES - 1;
-    if (f < T) outi[9] = align4(tab.shift[(int64_t)xc * T + f] - 2);
     int32_t n = 0, fmask = 0;
     for (int e = 0; e < C::NB; ++e) {
         float *oe = out + kHdr + 8 * e;
@@ -162,85 +166,111 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
 }
 
 // ------------------------------------------------------------------------------------ main kernel
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// Warp-specialised, persistent.  Per CTA-local frame counter n (frames of all its work items in
+// sequence) three rings connect the roles:
+//   box[n % SB]  TMA -> producers      full_box  (tx bytes; also covers tab[n % TS])
+//   X[n % XR]    producers -> consumers x_full   (kPW arrivals),  x_empty (CW arrivals)
+//   tab[n % TS]  TMA -> producers (gx) and consumers (gy, d, masks)
+// The TMA of frame n + SB is issued by one producer thread once every producer warp has finished
+// frame n (named barrier 1).  Producers start frame n only after all consumers released frame
+// n - XR, so when frame n + SB is issued every consumer has finished frame n - XR - 1 completely:
+// TS >= SB + XR + 2 table stages suffice even though a consumer releases X before it runs the flush
+// of that frame (which still reads d from the table).
 template <class C>
 __global__ void __launch_bounds__(C::NT, 1)
 k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int32_t ntx,
              const int32_t nty) {
-    constexpr int R = C::R, NB = C::NB, NW = C::NW, HT = C::HT;
-    constexpr int S = C::STAGES, TABW = C::TABW;
+    constexpr int R = C::R, NB = C::NB, CW = C::CW, HT = C::HT;
+    constexpr int SB = C::SB, XR = C::XR, TS = C::TS, TABW = C::TABW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *Rbuf = reinterpret_cast<float *>(smem_raw);
-    float *Xbuf = Rbuf + S * C::RBUF;
-    float *Tab = Xbuf + 2 * C::XBUF;
-    uint64_t *bar = reinterpret_cast<uint64_t *>(Tab + S * TABW);
+    float *Xbuf = Rbuf + SB * C::RBUF;
+    float *Tab = Xbuf + XR * C::XBUF;
+    uint64_t *full_box = reinterpret_cast<uint64_t *>(Tab + TS * TABW);
+    uint64_t *x_full = full_box + SB;
+    uint64_t *x_empty = x_full + XR;
+    uint64_t *f_done = x_empty + XR;      // [NB] all consumer warps have finished their k-th flush of entry e
 
     const int32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int32_t r0 = warp * R;
     const int32_t T = a.T, H = a.H, W = a.W;
-    // Half of the warps of every SM sub-partition (warp % 4) run the y-pass before the x-pass, the
-    // other half after it, so that the latencies of one pass hide under the FFMAs of the other.
-    const bool y_first = (warp & 4) != 0;
+    const int32_t n_items = ntx * nty * a.n_batches;          // < 2^31 (checked by the host)
 
     if (tid == 0) {
-        for (int s = 0; s < S; ++s) mbar_init(&bar[s], 1);
+        for (int s = 0; s < SB; ++s) mbar_init(&full_box[s], 1);
+        for (int s = 0; s < XR; ++s) { mbar_init(&x_full[s], kPW); mbar_init(&x_empty[s], CW); }
+        for (int s = 0; s < NB; ++s) mbar_init(&f_done[s], CW);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    uint32_t phase = 0;   // bit s = parity to wait for on stage s
-    // x-pass roles: group g = (block of 8 rows, half of the 64 columns); a quarter-warp takes the
-    // 8 rows of the block at one 8-column chunk.  The last warps take the ragged tail.
-    const int32_t xrow_in = lane & 7, xq_in = lane >> 3;
-
-    const int32_t n_items = ntx * nty * a.n_batches;          // < 2^31 (checked by the host)
-    for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const int32_t b = item % a.n_batches;
-        const int32_t tile = item / a.n_batches;
-        const int32_t ty = tile / ntx;
-        const int32_t x0 = (tile % ntx) * kTileW, Y0 = ty * HT - 2;
-        // positions P >= H + 2 have no tap inside the frame: warps that hold only such positions
-        // and the X rows only they would read are skipped (rows past the frame arrive as zeros)
-        const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
-        const int32_t x = x0 + 2 * lane;
-
-        float2 acc[NB][R];
-#pragma unroll
-        for (int s = 0; s < NB; ++s)
-#pragma unroll
-            for (int i = 0; i < R; ++i) acc[s][i] = make_float2(0.f, 0.f);
-
-        auto issue = [&](int32_t f, int32_t xo) {
-            const int32_t st = f % S;
-            mbar_expect_tx(&bar[st], C::BOX_BYTES + TABW * 4);
-            tma_load_3d(Rbuf + st * C::RBUF, &map, x0 + xo, Y0 - 2, f, &bar[st]);
-            bulk_load(Tab + st * TABW, a.stage_tab + ((int64_t)b * T + f) * TABW, TABW * 4, &bar[st]);
+    if (warp >= CW) {
+        // =============================================================== producers: TMA + x-pass
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::PREGS));
+        const int32_t pw = warp - CW;
+        const bool issuer = (pw == 0) && (lane == 0);
+        // issue state (issuer thread only): the next frame to request
+        int32_t iss_item = blockIdx.x, iss_t = 0, iss_n = 0, iss_ts = 0, iss_x0 = 0, iss_y = 0, xo_next = 0;
+        const int32_t *iss_ptr = nullptr;
+        auto iss_setup = [&]() {
+            const int32_t b = iss_item % a.n_batches, tile = iss_item / a.n_batches;
+            iss_x0 = (tile % ntx) * kTileW;
+            iss_y = (tile / ntx) * HT - 4;
+            iss_ptr = reinterpret_cast<const int32_t *>(a.stage_tab + (int64_t)b * T * TABW);
+            xo_next = __ldg(iss_ptr);
         };
-
-        // ---------------- x-pass of frame fx: X[fx & 1] = row-wise 5-tap correlation of the staged box
-        auto x_pass = [&](int32_t fx, int32_t &nxo) {
-            const int32_t st = fx % S;
-            mbar_wait(&bar[st], (phase >> st) & 1u);
-            phase ^= 1u << st;
-            const float *tb = Tab + st * TABW;
-            const int32_t *tbi = reinterpret_cast<const int32_t *>(tb);
-            nxo = tbi[9];
-            const int32_t o = tbi[1];
-            const float g0 = tb[4], g1 = tb[5], g2 = tb[6], g3 = tb[7], g4 = tb[8];
-            const float *src = Rbuf + st * C::RBUF;
-            float *dst = Xbuf + (fx & 1) * C::XBUF;
-            const int32_t ngroups = 2 * ((xrows + 7) >> 3);
-            for (int32_t g = NW - 1 - warp; g < ngroups; g += NW) {
-                const int32_t row = 8 * (g >> 1) + xrow_in, q = 4 * (g & 1) + xq_in;
-                if (row < xrows) {
-                    const float4 *p4 = reinterpret_cast<const float4 *>(src + row * kBoxW + 8 * q);
-                    const float4 u0 = p4[0], u1 = p4[1], u2 = p4[2], u3 = p4[3];
-                    const float r[16] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w,
-                                         u2.x, u2.y, u2.z, u2.w, u3.x, u3.y, u3.z, u3.w};
-                    float v[8];
-#define TNO_TAPS(O)                                                                                   \
-    _Pragma("unroll") for (int c = 0; c < 8; ++c)                                                     \
-        v[c] = fmaf(g4, r[O + c + 4],                                                                 \
-                    fmaf(g3, r[O + c + 3], fmaf(g2, r[O + c + 2], fmaf(g1, r[O + c + 1], g0 * r[O + c]))));
+        auto iss_one = [&]() {          // request frame iss_n into box stage iss_n % SB, table stage iss_ts
+            const int32_t sb = iss_n & (SB - 1);
+            mbar_expect_tx(&full_box[sb], C::BOX_BYTES + TABW * 4);
+            tma_load_3d(Rbuf + sb * C::RBUF, &map, iss_x0 + xo_next, iss_y, iss_t, &full_box[sb]);
+            bulk_load(Tab + iss_ts * TABW, iss_ptr, TABW * 4, &full_box[sb]);
+            ++iss_n;
+            iss_ts = (iss_ts + 1) & (TS - 1);
+            iss_ptr += TABW;
+            if (++iss_t == T) {
+                iss_t = 0;
+                iss_item += gridDim.x;
+                if (iss_item < n_items) iss_setup();
+            } else {
+                xo_next = __ldg(iss_ptr);
+            }
+        };
+        if (issuer && iss_item < n_items) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            iss_setup();
+            for (int f = 0; f < SB && iss_item < n_items; ++f) iss_one();
+        }
+        // x-pass roles: group g = (block of 8 rows, 4 of the 16 column quads); a quarter-warp takes the
+        // 8 rows of a block at one quad: 32 distinct banks for the 16-byte loads (pitch 76) and for
+        // the 16-byte stores (pitch 68).  Producer warp pw owns quads 4 pw .. 4 pw + 3 of every block.
+        const int32_t row_in = lane & 7, quad = 4 * pw + (lane >> 3);
+        int32_t n = 0;
+        for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+            const int32_t Y0 = (item / a.n_batches / ntx) * HT - 2;
+            // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
+            const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
+            for (int32_t t = 0; t < T; ++t) {
+                const int32_t sb = n & (SB - 1), xr = n & (XR - 1);
+                mbar_wait(&full_box[sb], (n / SB) & 1);
+                if (n >= XR) mbar_wait(&x_empty[xr], ((n / XR) + 1) & 1);
+                const float *tb = Tab + (n & (TS - 1)) * TABW;
+                const int32_t o = reinterpret_cast<const int32_t *>(tb)[1];
+                const float g0 = tb[4], g1 = tb[5], g2 = tb[6], g3 = tb[7], g4 = tb[8];
+                const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 4 * quad;
+                float *dst = Xbuf + xr * C::XBUF + row_in * kXP + 4 * quad;
+                for (int32_t row = row_in; row < xrows; row += 8, src += 8 * kBoxW, dst += 8 * kXP) {
+                    const float4 *p4 = reinterpret_cast<const float4 *>(src);
+                    const float4 u0 = p4[0], u1 = p4[1], u2 = p4[2];
+                    const float r[12] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w, u2.x, u2.y, u2.z, u2.w};
+                    float4 v;
+#define TNO_TAPS(O)                                                                                        \
+    v.x = fmaf(g4, r[O + 4], fmaf(g3, r[O + 3], fmaf(g2, r[O + 2], fmaf(g1, r[O + 1], g0 * r[O]))));      \
+    v.y = fmaf(g4, r[O + 5], fmaf(g3, r[O + 4], fmaf(g2, r[O + 3], fmaf(g1, r[O + 2], g0 * r[O + 1]))));  \
+    v.z = fmaf(g4, r[O + 6], fmaf(g3, r[O + 5], fmaf(g2, r[O + 4], fmaf(g1, r[O + 3], g0 * r[O + 2]))));  \
+    v.w = fmaf(g4, r[O + 7], fmaf(g3, r[O + 6], fmaf(g2, r[O + 5], fmaf(g1, r[O + 4], g0 * r[O + 3]))));
                     switch (o) {                       // uniform across the CTA
                         case 0: TNO_TAPS(0) break;
                         case 1: TNO_TAPS(1) break;
@@ -248,96 +278,131 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                         default: TNO_TAPS(3) break;
                     }
 #undef TNO_TAPS
-                    float4 *d4 = reinterpret_cast<float4 *>(dst + row * kXP + 8 * q);
-                    d4[0] = make_float4(v[0], v[1], v[2], v[3]);
-                    d4[1] = make_float4(v[4], v[5], v[6], v[7]);
+                    *reinterpret_cast<float4 *>(dst) = v;
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&x_full[xr]);
+                asm volatile("bar.sync 1, %0;" ::"n"(kPW * 32) : "memory");   // all producers are done with box sb
+                if (issuer && iss_item < n_items) iss_one();
+                ++n;
             }
-        };
+        }
+    } else {
+        // =============================================================== consumers: y-pass + flush
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::CREGS));
+        const int32_t r0 = warp * R;
+        int32_t n = 0;
+        uint32_t fpar = 0;        // bit e = parity of the number of flushes of entry e so far
+        for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+            // else: positions without any tap in the frame
+            const bool y_active = r0 < min(HT, H + 4 - (item / a.n_batches / ntx) * HT);
 
-        // ---------------- y-pass of frame i: one register window of X for all entries of the batch
-        auto y_pass = [&](int32_t i) {
-            const float *th = Tab + (i % S) * TABW;
-            const float *tb = th + kHdr;
-            const float2 *xp = reinterpret_cast<const float2 *>(Xbuf + (i & 1) * C::XBUF + r0 * kXP) + lane;
-            float2 win[R + 4];
+            float2 acc[NB][R];
 #pragma unroll
-            for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
-            const int32_t n = reinterpret_cast<const int32_t *>(th)[2];
-            const int32_t fmask = reinterpret_cast<const int32_t *>(th)[3];
-#define TNO_ENTRY(s)                                                                                  \
-    {                                                                                                 \
-        const float4 wa = *reinterpret_cast<const float4 *>(tb + 8 * (s));                            \
-        const float w4 = tb[8 * (s) + 4];                                                             \
-        _Pragma("unroll") for (int r = 0; r < R; ++r) {                                               \
-            float2 c = acc[s][r];                                                                     \
-            c.x = fmaf(wa.x, win[r].x, c.x);     c.y = fmaf(wa.x, win[r].y, c.y);                     \
-            c.x = fmaf(wa.y, win[r + 1].x, c.x); c.y = fmaf(wa.y, win[r + 1].y, c.y);                 \
-            c.x = fmaf(wa.z, win[r + 2].x, c.x); c.y = fmaf(wa.z, win[r + 2].y, c.y);                 \
-            c.x = fmaf(wa.w, win[r + 3].x, c.x); c.y = fmaf(wa.w, win[r + 3].y, c.y);                 \
-            c.x = fmaf(w4, win[r + 4].x, c.x);   c.y = fmaf(w4, win[r + 4].y, c.y);                   \
-            acc[s][r] = c;                                                                            \
-        }                                                                                             \
+            for (int s = 0; s < NB; ++s)
+#pragma unroll
+                for (int i = 0; i < R; ++i) acc[s][i] = make_float2(0.f, 0.f);
+
+            for (int32_t t = 0; t < T; ++t) {
+                const int32_t xr = n & (XR - 1);
+                mbar_wait(&x_full[xr], (n / XR) & 1);
+                const float *th = Tab + (n & (TS - 1)) * TABW;
+                const float *tb = th + kHdr;
+                if (y_active) {
+                    // ---------------- y-pass: one register window of X for all entries of the batch
+                    const float2 *xp = reinterpret_cast<const float2 *>(Xbuf + xr * C::XBUF + r0 * kXP) + lane;
+                    float2 win[R + 4];
+#pragma unroll
+                    for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
+                    const int32_t nfill = reinterpret_cast<const int32_t *>(th)[2];
+#define TNO_FMAS(s)                                                                                   \
+    _Pragma("unroll") for (int r = 0; r < R; ++r) {                                                   \
+        float2 c = acc[s][r];                                                                         \
+        c.x = fmaf(wa.x, win[r].x, c.x);     c.y = fmaf(wa.x, win[r].y, c.y);                         \
+        c.x = fmaf(wa.y, win[r + 1].x, c.x); c.y = fmaf(wa.y, win[r + 1].y, c.y);                     \
+        c.x = fmaf(wa.z, win[r + 2].x, c.x); c.y = fmaf(wa.z, win[r + 2].y, c.y);                     \
+        c.x = fmaf(wa.w, win[r + 3].x, c.x); c.y = fmaf(wa.w, win[r + 3].y, c.y);                     \
+        c.x = fmaf(w4, win[r + 4].x, c.x);   c.y = fmaf(w4, win[r + 4].y, c.y);                       \
+        acc[s][r] = c;                                                                                \
     }
-            if (n == NB) {          // full batch: straight-line code
+                    if (nfill == NB) {
+                        // full batch: straight-line code, the weights of entry s + 1 are loaded
+                        // before the FFMAs of entry s (the empty asm keeps ptxas from hoisting more
+                        // loads than the register budget holds)
+                        float4 wa = *reinterpret_cast<const float4 *>(tb);
+                        float w4 = tb[4];
 #pragma unroll
-                for (int s = 0; s < NB; ++s) TNO_ENTRY(s)
-            } else {
-#pragma unroll
-                for (int s = 0; s < NB; ++s)
-                    if (s < n) TNO_ENTRY(s)
-            }
-#undef TNO_ENTRY
-            if (fmask != 0) {
-                // ---------------- flush: piece[ty mod NP][entry][P - d][x] += acc, acc = 0
-                float *pbase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride;
-                const int32_t *bq = a.batch_q + (int64_t)b * NB;
-#pragma unroll
-                for (int s = 0; s < NB; ++s) {
-                    if (fmask & (1 << s)) {
-                        const int32_t d = reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
-                        const int32_t yb = Y0 + r0 - d;
-                        const int64_t q = __ldg(bq + s) - a.q0;
-                        float *p0 = pbase + (q * H + yb) * (int64_t)W + x;
-                        float2 old[R];
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const bool in = (uint32_t)(yb + r) < (uint32_t)H && x < W;
-                            old[r] = in ? __ldcg(reinterpret_cast<const float2 *>(p0 + (int64_t)r * W))
-                                        : make_float2(0.f, 0.f);
+                        for (int s = 0; s < NB; ++s) {
+                            float4 wan = wa;
+                            float w4n = w4;
+                            if (s + 1 < NB) {
+                                wan = *reinterpret_cast<const float4 *>(tb + 8 * (s + 1));
+                                w4n = tb[8 * (s + 1) + 4];
+                            }
+                            TNO_FMAS(s)
+                            asm volatile("" ::: "memory");
+                            wa = wan;
+                            w4 = w4n;
                         }
+                    } else {
 #pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const bool in = (uint32_t)(yb + r) < (uint32_t)H && x < W;
-                            if (in)
-                                __stcg(reinterpret_cast<float2 *>(p0 + (int64_t)r * W),
-                                       make_float2(old[r].x + acc[s][r].x, old[r].y + acc[s][r].y));
-                            acc[s][r] = make_float2(0.f, 0.f);
+                        for (int s = 0; s < NB; ++s)
+                            if (s < nfill) {
+                                const float4 wa = *reinterpret_cast<const float4 *>(tb + 8 * s);
+                                const float w4 = tb[8 * s + 4];
+                                TNO_FMAS(s)
+                            }
+                    }
+#undef TNO_FMAS
+                }
+                const int32_t fmask = reinterpret_cast<const int32_t *>(th)[3];
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&x_empty[xr]);      // this warp no longer reads X[xr]
+                if (fmask != 0) {
+                    // ---------------- flush: piece[ty mod NP][entry][P - d][x] += acc, acc = 0
+                    // (rare path: the item's coordinates are recomputed here to keep registers free)
+                    const int32_t b = item % a.n_batches, tile = item / a.n_batches;
+                    const int32_t ty = tile / ntx;
+                    const int32_t x = (tile % ntx) * kTileW + 2 * lane, Y0 = ty * HT - 2;
+                    float *pbase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride;
+                    const int32_t *bq = a.batch_q + (int64_t)b * NB;
+#pragma unroll
+                    for (int s = 0; s < NB; ++s) {
+                        if (fmask & (1 << s)) {
+                            // The output rows a warp holds change with d, so successive flushes of an
+                            // entry touch the same addresses from different warps: flush k starts only
+                            // after every consumer warp has finished flush k - 1 of that entry (f_done;
+                            // release/acquire at CTA scope orders the global read-modify-writes).
+                            mbar_wait(&f_done[s], ((fpar >> s) & 1u) ^ 1u);
+                            fpar ^= 1u << s;
+                            if (y_active) {
+                                const int32_t d = reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
+                                const int32_t yb = Y0 + r0 - d;
+                                const int64_t q = __ldg(bq + s) - a.q0;
+                                float *p0 = pbase + (q * H + yb) * (int64_t)W + x;
+                                float2 old[R];
+#pragma unroll
+                                for (int r = 0; r < R; ++r) {
+                                    const bool in = (uint32_t)(yb + r) < (uint32_t)H && x < W;
+                                    old[r] = in ? __ldcg(reinterpret_cast<const float2 *>(p0 + (int64_t)r * W))
+                                                : make_float2(0.f, 0.f);
+                                }
+#pragma unroll
+                                for (int r = 0; r < R; ++r) {
+                                    const bool in = (uint32_t)(yb + r) < (uint32_t)H && x < W;
+                                    if (in)
+                                        __stcg(reinterpret_cast<float2 *>(p0 + (int64_t)r * W),
+                                               make_float2(old[r].x + acc[s][r].x, old[r].y + acc[s][r].y));
+                                    acc[s][r] = make_float2(0.f, 0.f);
+                                }
+                            }
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(&f_done[s]);
                         }
                     }
                 }
+                ++n;
             }
-        };
-
-        __syncthreads();    // every warp is done with the previous item's buffers
-        if (tid == 0) {
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            const int32_t *gi = reinterpret_cast<const int32_t *>(a.stage_tab + (int64_t)b * T * TABW);
-            for (int32_t f = 0; f < S && f < T; ++f) issue(f, __ldg(gi + (int64_t)f * TABW));
-        }
-
-        const bool y_active = r0 < xrows - 4;
-        for (int32_t i = -1; i < T; ++i) {
-            int32_t nxo = 0;
-            if (y_first) {
-                if (i >= 0 && y_active) y_pass(i);
-                if (i + 1 < T) x_pass(i + 1, nxo);
-            } else {
-                if (i + 1 < T) x_pass(i + 1, nxo);
-                if (i >= 0 && y_active) y_pass(i);
-            }
-            __syncthreads();
-            if (tid == 0 && i >= 0 && i + S < T) issue(i + S, nxo);
         }
     }
 }
@@ -406,9 +471,10 @@ k_finish(const float *__restrict__ pieces, int32_t n_pieces, int64_t piece_strid
 }
 
 // ------------------------------------------------------------------------------------ host side
-// (rows per thread, entries per batch, warps, stages): tile 64 positions x 64 columns, 512 threads
-using V0 = SepCfg<4, 8, 16, 5>;
-using V1 = SepCfg<4, 10, 16, 5>;
+// (rows per thread, entries per batch, consumer warps, box stages, X buffers): tile 60 positions x
+// 64 columns, 384 consumer + 128 producer threads
+using V0 = SepCfg<5, 8, 12, 4, 4>;
+using V1 = SepCfg<5, 10, 12, 4, 4>;
 
 int32_t sep_num_variants() { return 2; }
 SepVariant sep_variant(int32_t v) { return v == 0 ? SepVariant{V0::NB, V0::HT} : SepVariant{V1::NB, V1::HT}; }
