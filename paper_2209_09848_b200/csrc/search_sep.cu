@@ -16,8 +16,8 @@
 // does.  Just before that happens (and every kSeg frames, and after the last frame) the entry's
 // accumulators are added into the PIECE buffer piece[ty mod NP][entry][y][x] in global memory
 // (L2 resident while hot) and cleared.  Tile rows ty and ty' contribute to the same output row
-// only if |ty - ty'| < NP, so every piece address belongs to exactly one CTA and plain
-// read-modify-write is race free and deterministic.  k_finish sums the NP pieces in a fixed order,
+// only if |ty - ty'| < NP, so every piece address belongs to exactly one CTA; the adds are
+// red.global.add.v2.f32 (no read latency), issued in a fixed order per address, hence deterministic.  k_finish sums the NP pieces in a fixed order,
 // multiplies by D^(-1/2), stores the map and collects the candidates.  The segment flushes also
 // bound the FP32 rounding error of long sums (|dSNR| <= 1e-3 on bright tracks).
 //
@@ -316,14 +316,14 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                     for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
                     const int32_t nfill = reinterpret_cast<const int32_t *>(th)[2];
 #define TNO_FMAS(s)                                                                                   \
-    _Pragma("unroll") for (int r = 0; r < R; ++r) {                                                   \
-        float2 c = acc[s][r];                                                                         \
-        c.x = fmaf(wa.x, win[r].x, c.x);     c.y = fmaf(wa.x, win[r].y, c.y);                         \
-        c.x = fmaf(wa.y, win[r + 1].x, c.x); c.y = fmaf(wa.y, win[r + 1].y, c.y);                     \
-        c.x = fmaf(wa.z, win[r + 2].x, c.x); c.y = fmaf(wa.z, win[r + 2].y, c.y);                     \
-        c.x = fmaf(wa.w, win[r + 3].x, c.x); c.y = fmaf(wa.w, win[r + 3].y, c.y);                     \
-        c.x = fmaf(w4, win[r + 4].x, c.x);   c.y = fmaf(w4, win[r + 4].y, c.y);                       \
-        acc[s][r] = c;                                                                                \
+    {                                                                                                 \
+        const float2 w0 = make_float2(wa.x, wa.x), w1 = make_float2(wa.y, wa.y),                      \
+                     w2 = make_float2(wa.z, wa.z), w3 = make_float2(wa.w, wa.w), w5 = make_float2(w4, w4); \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w0, win[r], acc[s][r]);     \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w1, win[r + 1], acc[s][r]); \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w2, win[r + 2], acc[s][r]); \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w3, win[r + 3], acc[s][r]); \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w5, win[r + 4], acc[s][r]); \
     }
                     if (nfill == NB) {
                         // full batch: straight-line code, the weights of entry s + 1 are loaded
@@ -380,19 +380,12 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                                 const int32_t yb = Y0 + r0 - d;
                                 const int64_t q = __ldg(bq + s) - a.q0;
                                 float *p0 = pbase + (q * H + yb) * (int64_t)W + x;
-                                float2 old[R];
 #pragma unroll
                                 for (int r = 0; r < R; ++r) {
-                                    const bool in = (uint32_t)(yb + r) < (uint32_t)H && x < W;
-                                    old[r] = in ? __ldcg(reinterpret_cast<const float2 *>(p0 + (int64_t)r * W))
-                                                : make_float2(0.f, 0.f);
-                                }
-#pragma unroll
-                                for (int r = 0; r < R; ++r) {
-                                    const bool in = (uint32_t)(yb + r) < (uint32_t)H && x < W;
-                                    if (in)
-                                        __stcg(reinterpret_cast<float2 *>(p0 + (int64_t)r * W),
-                                               make_float2(old[r].x + acc[s][r].x, old[r].y + acc[s][r].y));
+                                    // red.global.add.v2.f32: no read latency; the piece address is
+                                    // owned by this CTA, and f_done orders the adds of successive flushes
+                                    if ((uint32_t)(yb + r) < (uint32_t)H && x < W)
+                                        atomicAdd(reinterpret_cast<float2 *>(p0 + (int64_t)r * W), acc[s][r]);
                                     acc[s][r] = make_float2(0.f, 0.f);
                                 }
                             }
