@@ -109,12 +109,13 @@ struct SepCfg {
     static constexpr int NBAR = SB + 2 * XR + NB;
     static constexpr size_t SMEM = (size_t)(SB * RBUF + XR * XBUF + TS * TABW) * 4 + NBAR * 8 + 64;
     // register split: setmaxnreg moves registers between the warpgroups of the CTA, the total stays
-    // what the launch allocated (NT x 128 with __launch_bounds__(512, 1))
-    static constexpr int CREGS = 160, PREGS = 32;
+    // what the launch allocated (NT x the per-thread count ptxas derives from __launch_bounds__)
+    static constexpr int LREGS = 65536 / NT / 8 * 8;
+    static constexpr int PREGS = 32, CREGS = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
+    static_assert(CW % 4 == 0 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * LREGS, "register budget");
     static_assert((SB & (SB - 1)) == 0 && (XR & (XR - 1)) == 0 && (TS & (TS - 1)) == 0 && TS >= SB + XR + 2,
                   "ring sizes are powers of two");
     static_assert((TABW * 4) % 16 == 0 && (XBUF * 4) % 16 == 0, "16-byte alignment of the sections");
-    static_assert(CW % 4 == 0 && NT == 512 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * 128, "register budget");
 };
 
 // Phase of an entry's periodic flush: a function of its y-motion alone, so that the summation order
@@ -294,8 +295,18 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         int32_t n = 0;
         uint32_t fpar = 0;        // bit e = parity of the number of flushes of entry e so far
         for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+            // flush coordinates of the item: entry s of the batch has planned index q_first + s, its
+            // piece map starts at ebase + s*H*W (this lane's two columns), and the accumulator row r
+            // of this warp holds output row yr0 + r - d
+            const int32_t b = item % a.n_batches, tile = item / a.n_batches;
+            const int32_t ty = tile / ntx;
+            const int32_t x = (tile % ntx) * kTileW + 2 * lane;
+            float *ebase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride +
+                           (int64_t)(__ldg(a.batch_q + (int64_t)b * NB) - a.q0) * H * W + x;
+            // columns past the frame: make every row test fail
+            const int32_t yr0 = (x < W) ? ty * HT - 2 + r0 : INT32_MIN / 2;
             // else: positions without any tap in the frame
-            const bool y_active = r0 < min(HT, H + 4 - (item / a.n_batches / ntx) * HT);
+            const bool y_active = r0 < min(HT, H + 4 - ty * HT);
 
             float2 acc[NB][R];
 #pragma unroll
@@ -360,12 +371,6 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 if (lane == 0) mbar_arrive(&x_empty[xr]);      // this warp no longer reads X[xr]
                 if (fmask != 0) {
                     // ---------------- flush: piece[ty mod NP][entry][P - d][x] += acc, acc = 0
-                    // (rare path: the item's coordinates are recomputed here to keep registers free)
-                    const int32_t b = item % a.n_batches, tile = item / a.n_batches;
-                    const int32_t ty = tile / ntx;
-                    const int32_t x = (tile % ntx) * kTileW + 2 * lane, Y0 = ty * HT - 2;
-                    float *pbase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride;
-                    const int32_t *bq = a.batch_q + (int64_t)b * NB;
 #pragma unroll
                     for (int s = 0; s < NB; ++s) {
                         if (fmask & (1 << s)) {
@@ -376,16 +381,14 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                             mbar_wait(&f_done[s], ((fpar >> s) & 1u) ^ 1u);
                             fpar ^= 1u << s;
                             if (y_active) {
-                                const int32_t d = reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
-                                const int32_t yb = Y0 + r0 - d;
-                                const int64_t q = __ldg(bq + s) - a.q0;
-                                float *p0 = pbase + (q * H + yb) * (int64_t)W + x;
+                                const int32_t yb = yr0 - reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
+                                float *p = ebase + (int64_t)(s * H + yb) * W;
 #pragma unroll
-                                for (int r = 0; r < R; ++r) {
+                                for (int r = 0; r < R; ++r, p += W) {
                                     // red.global.add.v2.f32: no read latency; the piece address is
                                     // owned by this CTA, and f_done orders the adds of successive flushes
-                                    if ((uint32_t)(yb + r) < (uint32_t)H && x < W)
-                                        atomicAdd(reinterpret_cast<float2 *>(p0 + (int64_t)r * W), acc[s][r]);
+                                    if ((uint32_t)(yb + r) < (uint32_t)H)
+                                        atomicAdd(reinterpret_cast<float2 *>(p), acc[s][r]);
                                     acc[s][r] = make_float2(0.f, 0.f);
                                 }
                             }
