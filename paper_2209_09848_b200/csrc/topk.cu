@@ -32,28 +32,98 @@ k_collect_from_map(const float *__restrict__ maps, int32_t H, int32_t W, int32_t
     tile_flush<256>(list, count, slots, tile, k, tid);
 }
 
-// One block per trajectory: stream all tile slots through a sorted buffer of the P best.
-__global__ void __launch_bounds__(256)
+// One block per trajectory: exact selection of the ktop largest keys among the candidates of all
+// tile slots (keys are unique: the pixel index is part of the key), then one small sort.
+//   1. N = sum of the tile counts; if N <= ktop every candidate is selected;
+//   2. else a most-significant-digit radix select (13-bit digits, shared-memory histogram) finds
+//      the ktop-th largest key; each pass reads the candidates (L2 resident) once;
+//   3. the selected keys are gathered into shared memory, sorted (bitonic, shuffles for strides
+//      < 32) and written as records.
+constexpr int kMergeThreads = 512;
+constexpr int kDigitBits = 13, kBins = 1 << kDigitBits;
+
+__global__ void __launch_bounds__(kMergeThreads)
 k_topk_merge(TopkSlots slots, int32_t n_tiles, int32_t W, int32_t P, tno_mf_cand *__restrict__ out) {
-    extern __shared__ uint64_t buf[];          // [0, P) best so far (sorted), [P, 2P) incoming
-    const int32_t tid = threadIdx.x, k = blockIdx.x, ktop = slots.ktop;
-    for (int32_t i = tid; i < P; i += 256) buf[i] = 0ull;
-    const int32_t G = P / ktop;                // tiles per round
-    for (int32_t tile0 = 0; tile0 < n_tiles; tile0 += G) {
-        int32_t any = 0;
-        for (int32_t i = tid; i < P; i += 256) {
-            const int32_t g = i / ktop, r = i - g * ktop;
-            const int64_t tile = (int64_t)tile0 + g;
-            uint64_t v = 0ull;
-            if (g < G && tile < n_tiles && r < slots.counts[tile * slots.K + k])
-                v = slots.keys[(tile * slots.K + k) * (int64_t)ktop + r];
-            buf[P + i] = v;
-            any |= (v != 0ull);
+    extern __shared__ uint64_t buf[];          // [0, P) selected keys
+    __shared__ uint32_t hist[kBins];
+    __shared__ uint32_t wsum[kMergeThreads / 32];
+    __shared__ uint32_t sel_bin, sel_before, total, fill;
+    const int32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, k = blockIdx.x, ktop = slots.ktop;
+    constexpr int NWARP = kMergeThreads / 32;
+
+    // visit every candidate key of trajectory k: warp per tile, lanes over the slot entries
+    auto for_each_key = [&](auto &&fn) {
+        for (int32_t tile = warp; tile < n_tiles; tile += NWARP) {
+            const int32_t c = slots.counts[(int64_t)tile * slots.K + k];
+            const uint64_t *src = slots.keys + ((int64_t)tile * slots.K + k) * (int64_t)ktop;
+            for (int32_t r = lane; r < c; r += 32) fn(src[r]);
         }
-        if (__syncthreads_or(any)) block_sort_desc<256>(buf, 2 * P, tid);
+    };
+
+    if (tid == 0) { total = 0; fill = 0; }
+    for (int32_t i = tid; i < P; i += kMergeThreads) buf[i] = 0ull;
+    __syncthreads();
+    {
+        uint32_t n = 0;
+        for (int32_t tile = tid; tile < n_tiles; tile += kMergeThreads) n += (uint32_t)slots.counts[(int64_t)tile * slots.K + k];
+        for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+        if (lane == 0 && n) atomicAdd(&total, n);
     }
     __syncthreads();
-    for (int32_t i = tid; i < ktop; i += 256) {
+    const uint32_t N = total;
+    uint64_t kth = 0ull;                       // select keys >= kth
+    if (N > (uint32_t)ktop) {
+        uint64_t prefix = 0ull;                // value of the digits fixed so far (high bits of kth)
+        uint32_t remaining = (uint32_t)ktop;   // rank of the wanted key among the keys matching prefix
+        int32_t shift = 64;
+        while (shift > 0) {
+            const int32_t bits = shift >= kDigitBits ? kDigitBits : shift;
+            const int32_t lo = shift - bits;   // digit = (key >> lo) & (2^bits - 1)
+            const int32_t nb = 1 << bits;
+            for (int32_t i = tid; i < nb; i += kMergeThreads) hist[i] = 0u;
+            __syncthreads();
+            for_each_key([&](uint64_t key) {
+                const bool match = (shift == 64) || ((key >> shift) == (prefix >> shift));
+                if (match) atomicAdd(&hist[(uint32_t)(key >> lo) & (uint32_t)(nb - 1)], 1u);
+            });
+            __syncthreads();
+            // find, from the top bin down, the bin in which the cumulative count reaches `remaining`
+            const int32_t per = nb / kMergeThreads;                 // bins per thread (>= 1: nb >= 512)
+            uint32_t local = 0;
+            for (int32_t j = 0; j < per; ++j) local += hist[nb - 1 - (tid * per + j)];
+            uint32_t incl = local;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            if (lane == 31) wsum[warp] = incl;
+            __syncthreads();
+            uint32_t before = incl - local;
+            for (int32_t w = 0; w < warp; ++w) before += wsum[w];
+            if (before < remaining && remaining <= before + local) {
+                uint32_t acc = before;
+                for (int32_t j = 0; j < per; ++j) {
+                    const int32_t bin = nb - 1 - (tid * per + j);
+                    if (remaining <= acc + hist[bin]) { sel_bin = (uint32_t)bin; sel_before = acc; break; }
+                    acc += hist[bin];
+                }
+            }
+            __syncthreads();
+            prefix |= (uint64_t)sel_bin << lo;
+            remaining -= sel_before;
+            const uint32_t in_bin = hist[sel_bin];
+            shift = lo;
+            __syncthreads();
+            if (in_bin == remaining) break;    // every key with this prefix is selected
+        }
+        kth = prefix;                          // digits below `shift` are zero: keys >= kth are exactly the ktop best
+    }
+    for_each_key([&](uint64_t key) {
+        if (key >= kth) buf[atomicAdd(&fill, 1u)] = key;
+    });
+    __syncthreads();
+    block_sort_desc<kMergeThreads>(buf, P, tid);
+    for (int32_t i = tid; i < ktop; i += kMergeThreads) {
         const uint64_t key = buf[i];
         tno_mf_cand c;
         if (key != 0ull) {
@@ -78,10 +148,10 @@ void launch_collect_from_map(cudaStream_t st, const float *maps, int32_t H, int3
 
 void launch_topk_merge(cudaStream_t st, const TopkSlots &slots, int32_t n_tiles, int32_t W,
                        tno_mf_cand *out_topk) {
-    int32_t P = 512;
+    int32_t P = 32;
     while (P < slots.ktop) P <<= 1;
-    const size_t smem = (size_t)2 * P * sizeof(uint64_t);
-    k_topk_merge<<<(unsigned)slots.K, 256, smem, st>>>(slots, n_tiles, W, P, out_topk);
+    const size_t smem = (size_t)P * sizeof(uint64_t);
+    k_topk_merge<<<(unsigned)slots.K, kMergeThreads, smem, st>>>(slots, n_tiles, W, P, out_topk);
 }
 
 }  // namespace tno
