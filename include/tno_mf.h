@@ -70,11 +70,15 @@ typedef struct {
                                 1 = always use the generic (non-TMA) kernel -- for tests */
     int32_t record_events;   /* != 0: bracket the main search kernel with CUDA events on the stream
                                 so that tno_mf_last_kernel_ms can report its duration */
-    int32_t reserved[2];     /* must be 0 */
+    int32_t workspace_limit_mb; /* 0 = default (<= 40 GB and <= 80 % of the free device memory);
+                                > 0: cap, in MiB, of the partial-sum workspace of the separable
+                                kernel -- a bank that needs more is searched in chunks of whole
+                                batches (same results) */
+    int32_t reserved;        /* must be 0 */
 } tno_mf_config;
 
 /* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
- * reserved != 0), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
+ * workspace_limit_mb < 0, reserved != 0), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
 int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
 
 /* The search (formula above).

@@ -145,8 +145,8 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
     if (std::isnan(cfg->snr_threshold))
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
-    if (cfg->reserved[0] || cfg->reserved[1])
-        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: reserved fields must be 0");
+    if (cfg->reserved || cfg->workspace_limit_mb < 0)
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: reserved must be 0 and workspace_limit_mb >= 0");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess || n_dev == 0) {
@@ -429,19 +429,23 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
         if ((rc = reserve(ctx, ctx->stage_tab, (size_t)n_batches * T * sep_table_words(variant) * 4))) return rc;
         const size_t per_entry = (size_t)n_pieces * map_px * 4;
         const size_t want = per_entry * n_traj;
-        if (want > ctx->pieces.cap) {
+        const size_t limit = ctx->cfg.workspace_limit_mb > 0 ? (size_t)ctx->cfg.workspace_limit_mb << 20
+                                                             : (size_t)40 << 30;
+        size_t have = std::min(ctx->pieces.cap, limit);
+        if (want > have) {
             size_t free_b = 0, total_b = 0;
             CU_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));
             const size_t avail = (size_t)((double)(free_b + ctx->pieces.cap) * 0.8);
-            const size_t budget = std::min<size_t>(want, std::min<size_t>(avail, (size_t)40 << 30));
-            chunk_cap = (int64_t)(budget / per_entry);
-            if (chunk_cap < sv.nb && chunk_cap < n_traj)
+            const size_t budget = std::min<size_t>(want, std::min<size_t>(avail, limit));
+            // a chunk holds at least one batch
+            const size_t need = std::max<size_t>(budget, per_entry * (size_t)std::min<int64_t>(sv.nb, n_traj));
+            if (need > avail)
                 return fail(ctx, TNO_MF_ENOMEM, "not enough device memory for the partial-sum buffer "
                             "(%zu bytes per trajectory, %zu available)", per_entry, avail);
-            chunk_cap = std::min<int64_t>(chunk_cap, n_traj);
-            if ((rc = reserve(ctx, ctx->pieces, per_entry * (size_t)chunk_cap))) return rc;
+            if ((rc = reserve(ctx, ctx->pieces, need))) return rc;
+            have = need;
         }
-        chunk_cap = std::min<int64_t>((int64_t)(ctx->pieces.cap / per_entry), n_traj);
+        chunk_cap = std::min<int64_t>((int64_t)(have / per_entry), n_traj);
     }
     unsigned char *meta = static_cast<unsigned char *>(ctx->meta.p);
     CU_TRY(ctx, cudaMemcpyAsync(meta, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st));

@@ -17,19 +17,25 @@
 // accumulators are added into the PIECE buffer piece[ty mod NP][entry][y][x] in global memory
 // (L2 resident while hot) and cleared.  Tile rows ty and ty' contribute to the same output row
 // only if |ty - ty'| < NP, so every piece address belongs to exactly one CTA; the adds are
-// red.global.add.v2.f32 (no read latency), issued in a fixed order per address, hence deterministic.  k_finish sums the NP pieces in a fixed order,
-// multiplies by D^(-1/2), stores the map and collects the candidates.  The segment flushes also
-// bound the FP32 rounding error of long sums (|dSNR| <= 1e-3 on bright tracks).
+// red.global.add.v2.f32 (no read latency), issued in a fixed order per address, hence
+// deterministic.  k_finish sums the NP pieces in a fixed order, multiplies by D^(-1/2), stores the
+// map and collects the candidates.  The segment flushes also bound the FP32 rounding error of long
+// sums (|dSNR| <= 1e-3 on bright tracks).
 //
 // Structure:
 //   * persistent CTAs, one per SM, walk (tile, batch) work items batch-fastest, so the batches of
 //     one tile run on neighbouring CTAs at the same time and share the frame tiles in L2;
+//   * warp-specialised: one producer warpgroup (32 registers per thread after setmaxnreg) issues
+//     the TMA loads and runs the x-pass, 12 consumer warps (160 registers) run the y-pass; the
+//     roles are linked by mbarrier rings only, there is no CTA-wide barrier in the frame loop;
 //   * frame tiles of (HT + 4) rows x 76 columns are staged by TMA (cp.async.bulk.tensor.3d, zero
-//     fill outside the frame = "dropped from N") into a STAGES-deep shared-memory ring together
-//     with the per-(batch, frame) table (cp.async.bulk), completion on mbarriers;
-//   * x-pass: 8 outputs per thread from four 16-byte shared loads; the row pitches (76 and 68
+//     fill outside the frame = "dropped from N") into a ring of box stages together with the
+//     per-(batch, frame) table (cp.async.bulk), completion on mbarriers;
+//   * x-pass: 4 outputs per thread from three 16-byte shared loads; the row pitches (76 and 68
 //     words) make a quarter-warp of 8 rows hit 32 distinct banks on both the loads and the stores;
-//   * y-pass: R rows x 2 columns x NBW entries per thread in FP32 registers.
+//   * y-pass: R rows x 2 columns x NB entries per thread in FP32 registers, packed FFMA2
+//     (fma.rn.f32x2: two columns per instruction), which halves the issue slots of the y-pass and
+//     leaves room for the producer warps on the same schedulers.
 #include <cstdio>
 
 #include "kernels.h"

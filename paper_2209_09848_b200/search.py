@@ -12,13 +12,14 @@ class MatchedFilter:
     """One library context bound to the current torch CUDA stream of `device`."""
 
     def __init__(self, device: int = 0, topk: int = 0, snr_threshold: float = float("-inf"),
-                 force_generic: bool = False, record_events: bool = False):
+                 force_generic: bool = False, record_events: bool = False, workspace_limit_mb: int = 0):
         import torch
         self._torch = torch
         self.device = torch.device("cuda", device)
         self.topk = int(topk)
         stream = torch.cuda.current_stream(self.device).cuda_stream
-        self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events)
+        self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events,
+                                   workspace_limit_mb)
 
     def close(self) -> None:
         if self.ctx is not None:

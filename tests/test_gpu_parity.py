@@ -168,3 +168,70 @@ def test_errors_are_reported():
     P.tno_mf_search(ctx, f, np.ones(2, np.float32), np.zeros((1, 4), np.float32), 1.0, 0.0, out)
     torch.cuda.synchronize()
     P.tno_mf_destroy(ctx)
+
+
+def _bank_case(T, H, W, seed):
+    rng = np.random.default_rng(seed)
+    f = rng.standard_normal((T, H, W)).astype(np.float32)
+    f[:, H // 3, W // 3] += 6.0
+    sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
+    return f, sigma
+
+
+def test_chunked_workspace_gives_identical_results():
+    """A workspace cap smaller than the bank's partial-sum buffer makes the library search the bank
+    in chunks of whole batches; maps and lists must be bitwise those of the one-chunk search."""
+    torch = _torch()
+    from paper_2209_09848_b200 import MatchedFilter
+    T, H, W = 40, 128, 128
+    f, sigma = _bank_case(T, H, W, 11)
+    vs = np.linspace(-0.3, 0.3, 6).astype(np.float32)
+    traj = np.array([[vx, vy, 0, 0] for vx in vs for vy in vs], np.float32)      # 6 x-classes x 6 entries
+    d = torch.from_numpy(f).cuda()
+    outs = []
+    for limit in (0, 1):           # 1 MiB: one batch (6 entries x 1-2 pieces x 64 KiB) per chunk
+        with MatchedFilter(0, 9, 3.0, workspace_limit_mb=limit) as mf:
+            maps, cand = mf.search(d, sigma, traj, 1.0, T / 2.0)
+            torch.cuda.synchronize()
+            launches, kernel = mf.stats()
+            outs.append((maps.cpu().numpy(), mf.candidates_to_numpy(cand), launches))
+        assert kernel == 1
+    assert outs[1][2] > outs[0][2], "the capped search must have used more launches (chunks)"
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert np.array_equal(outs[0][1], outs[1][1])
+    om = oracle.snr_map(f, sigma, traj, 1.0, T / 2.0)
+    assert np.abs(outs[1][0] - om).max() <= TOL
+
+
+def test_fast_trajectories_need_many_pieces():
+    """y-shift ranges of several tile heights (many partial-sum pieces per output row), shifts that
+    jump by more than one pixel per frame, accelerations that make the track come back."""
+    torch = _torch()
+    T, H, W = 60, 200, 64
+    f, sigma = _bank_case(T, H, W, 12)
+    traj = np.array([[0.0, 3.7, 0, 0], [0.0, -2.2, 0, 0], [0.0, 0.4, 0, 0.12], [0.25, 1.0, 0, -0.05],
+                     [0.25, 0.0, 0, 0], [0.0, 0.0, 0, 0]], np.float32)
+    om = oracle.snr_map(f, sigma, traj, 1.0, 30.0)
+    gm, gc, stats = run_gpu(torch.from_numpy(f).cuda(), sigma, traj, 1.0, 30.0, 5, 3.0)
+    assert stats[1] == 1
+    assert np.abs(gm.astype(np.float64) - om).max() <= TOL
+    for k in range(traj.shape[0]):
+        check_topk(gc[k], om[k], k, 5, 3.0)
+        check_topk_vs_own_map(gc[k], gm[k], k, 5, 3.0)
+
+
+def test_results_are_reproducible_and_independent_of_the_bank():
+    """Bitwise identical maps from run to run, and the map of a trajectory does not depend on which
+    other trajectories are searched with it (summation order is a function of the trajectory)."""
+    torch = _torch()
+    T, H, W = 130, 96, 128
+    f, sigma = _bank_case(T, H, W, 13)
+    vs = np.linspace(-0.2, 0.2, 5).astype(np.float32)
+    traj = np.array([[vx, vy, 0, 0] for vx in vs[:2] for vy in vs], np.float32)
+    d = torch.from_numpy(f).cuda()
+    a, _, _ = run_gpu(d, sigma, traj, 1.0, 65.0, 4, 3.0)
+    b, _, _ = run_gpu(d, sigma, traj, 1.0, 65.0, 4, 3.0)
+    assert np.array_equal(a, b)
+    sub = np.array([0, 3, 7])
+    c, _, _ = run_gpu(d, sigma, traj[sub], 1.0, 65.0, 4, 3.0)
+    assert np.array_equal(a[sub], c)

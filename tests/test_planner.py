@@ -72,3 +72,22 @@ def test_bad_arguments():
         tno_mf_plan(traj, 10, 0.0, 8, 60)
     with pytest.raises(TnoMfError):                          # displacement beyond 1e9 px
         tno_mf_plan(np.array([[3e8, 0, 0, 0]], np.float32), 100, 0.0, 8, 60)
+
+
+def test_unlimited_spread_splits_evenly():
+    """max_spread >= 2^30 is what the search itself uses: no spread limit, each x-motion is split into
+    the fewest batches, of sizes that differ by at most one."""
+    unlimited = 1 << 30
+    traj = np.array([[0.1, v, 0, 0] for v in np.linspace(-3, 3, 23)] +
+                    [[0.2, v, 0, 0] for v in np.linspace(-1, 1, 10)] + [[0.3, 0, 0, 0]], dtype=np.float32)
+    n, batch, slot = tno_mf_plan(traj, 100, 50.0, 10, unlimited)
+    assert n == 3 + 1 + 1
+    sizes = sorted(np.bincount(batch).tolist())
+    assert sizes == [1, 7, 8, 8, 10]
+    for b in range(n):
+        ks = np.nonzero(batch == b)[0]
+        assert len({float(traj[k, 0]) for k in ks}) == 1
+        assert sorted(slot[ks].tolist()) == list(range(len(ks)))
+    for idx, nb, expect in ((3, 10, 10), (5, 8, 128), (5, 10, 128), (4, 8, 8)):
+        cfg = tno_synth.CONFIGS[idx]
+        assert tno_mf_plan(tno_synth.trajectories(cfg), cfg.T, cfg.t0, nb, unlimited)[0] == expect
