@@ -117,7 +117,7 @@ struct SepCfg {
     // register split: setmaxnreg moves registers between the warpgroups of the CTA, the total stays
     // what the launch allocated (NT x the per-thread count ptxas derives from __launch_bounds__)
     static constexpr int LREGS = 65536 / NT / 8 * 8;
-    static constexpr int PREGS = 32, CREGS = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
+    static constexpr int PREGS = 56, CREGS = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
     static_assert(CW % 4 == 0 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * LREGS, "register budget");
     static_assert((SB & (SB - 1)) == 0 && (XR & (XR - 1)) == 0 && (TS & (TS - 1)) == 0 && TS >= SB + XR + 2,
                   "ring sizes are powers of two");
