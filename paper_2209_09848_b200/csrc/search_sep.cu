@@ -99,6 +99,7 @@ constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per
 //   [2] number of entries of the batch (they occupy slots 0 .. n-1)
 //   [3] flush mask: bit e set if entry e must be flushed after this frame
 //   [4..8] gx[0..4]
+//   [10] wait mask: bit e set if the previous flush of entry e is at most XR frames back
 //   [16 + 8e + 0..4] gy_e[0..4] / sigma_t^2   [16 + 8e + 5] d_{e,t}          (entry e; zeros if empty)
 
 template <int R_, int NB_, int CW_, int SB_, int XR_>
@@ -151,7 +152,7 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
     outi[0] = align4(sxm2);
     outi[1] = sxm2 - align4(sxm2);
     for (int i = 0; i < 5; ++i) out[4 + i] = tab.g[((int64_t)xc * T + t) * 5 + i];
-    int32_t n = 0, fmask = 0;
+    int32_t n = 0, fmask = 0, fwait = 0;
     for (int e = 0; e < C::NB; ++e) {
         float *oe = out + kHdr + 8 * e;
         int32_t *oi = reinterpret_cast<int32_t *>(oe);
@@ -166,10 +167,19 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
         // the last frame
         const bool fl = (t == T - 1) || (tab.shift[ci + 1] != tab.shift[ci]) ||
                         ((t + 1 + seg_phase(tab.cls_v[c], tab.cls_a[c])) % kSeg == 0);
-        if (fl) fmask |= 1 << e;
+        if (fl) {
+            fmask |= 1 << e;
+            // was the entry also flushed after one of the frames t - XR .. t - 1 ?  (t < XR: the
+            // last frame of the CTA's previous work item, where every entry is flushed, is that close)
+            const int32_t ph = seg_phase(tab.cls_v[c], tab.cls_a[c]);
+            if (t < C::XR) fwait |= 1 << e;
+            for (int32_t u = max(t - C::XR, 0); u < t; ++u)
+                if (tab.shift[ci - t + u + 1] != tab.shift[ci - t + u] || (u + 1 + ph) % kSeg == 0) fwait |= 1 << e;
+        }
     }
     outi[2] = n;
     outi[3] = fmask;
+    outi[10] = fwait;
 }
 
 // ------------------------------------------------------------------------------------ main kernel
@@ -373,6 +383,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 #undef TNO_FMAS
                 }
                 const int32_t fmask = reinterpret_cast<const int32_t *>(th)[3];
+                const int32_t fwait = reinterpret_cast<const int32_t *>(th)[10];
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&x_empty[xr]);      // this warp no longer reads X[xr]
                 if (fmask != 0) {
@@ -382,9 +393,13 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                         if (fmask & (1 << s)) {
                             // The output rows a warp holds change with d, so successive flushes of an
                             // entry touch the same addresses from different warps: flush k starts only
-                            // after every consumer warp has finished flush k - 1 of that entry (f_done;
-                            // release/acquire at CTA scope orders the global read-modify-writes).
-                            mbar_wait(&f_done[s], ((fpar >> s) & 1u) ^ 1u);
+                            // after every consumer warp has finished flush k - 1 of that entry, which
+                            // fixes the order of the float adds per address.  If flush k - 1 is more
+                            // than XR frames back that is already implied by X[n] being there (the
+                            // producers waited for every consumer to release frame n - XR, which each
+                            // did after its flushes of the frames before); otherwise wait on f_done --
+                            // also needed so that no warp arrives twice in one phase of f_done.
+                            if (fwait & (1 << s)) mbar_wait(&f_done[s], ((fpar >> s) & 1u) ^ 1u);
                             fpar ^= 1u << s;
                             if (y_active) {
                                 const int32_t yb = yr0 - reinterpret_cast<const int32_t *>(tb)[8 * s + 5];

@@ -235,3 +235,23 @@ def test_results_are_reproducible_and_independent_of_the_bank():
     sub = np.array([0, 3, 7])
     c, _, _ = run_gpu(d, sigma, traj[sub], 1.0, 65.0, 4, 3.0)
     assert np.array_equal(a[sub], c)
+
+
+@pytest.mark.timeout(180)
+def test_many_work_items_per_cta_with_early_flushes():
+    """More (tile, batch) work items than SMs, so every CTA walks several items, with trajectories whose
+    shift changes within the first frames of an item: the per-entry flush barriers must keep counting
+    correctly across item boundaries (a missed wait there once dead-locked the full-size runs)."""
+    torch = _torch()
+    T, H, W = 12, 1024, 1024
+    rng = np.random.default_rng(14)
+    f = rng.standard_normal((T, H, W)).astype(np.float32)
+    sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
+    traj = np.array([[0.0, 0.45, 0, 0], [0.0, -0.3, 0, 0], [0.0, 0.26, 0, 0.01], [0.0, 0.0, 0, 0],
+                     [0.2, 0.5, 0, 0]], np.float32)
+    om = oracle.snr_map(f, sigma, traj, 1.0, 0.0)
+    gm, gc, stats = run_gpu(torch.from_numpy(f).cuda(), sigma, traj, 1.0, 0.0, 6, 4.5)
+    assert stats[1] == 1
+    assert np.abs(gm.astype(np.float64) - om).max() <= TOL
+    for k in range(traj.shape[0]):
+        check_topk_vs_own_map(gc[k], gm[k], k, 6, 4.5)
