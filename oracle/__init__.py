@@ -138,3 +138,40 @@ def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0) -> None:
                                 ys.ctypes.data_as(_i32p), amps.ctypes.data_as(_f32p), n,
                                 float(prf_sigma), float(t0))
     assert rc == 0
+
+
+# ---- interpreting scores (section 3.3): max over the bank, local-sigma units ----------
+_lib.tno_oracle_best.restype = ctypes.c_int
+_lib.tno_oracle_best.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f32p, _i32p]
+for _name in ("tno_oracle_local_z", "tno_oracle_local_z_sep"):
+    getattr(_lib, _name).restype = ctypes.c_int
+    getattr(_lib, _name).argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f64p, _f64p]
+
+
+def best(snr):
+    """(max over trajectories float32 [H, W], argmax int32 [H, W], smallest k on ties) of float32
+    maps [K, H, W] (PAPER.md:L112)."""
+    snr = _f32(snr)
+    K, H, W = snr.shape
+    m = np.empty((H, W), np.float32)
+    a = np.empty((H, W), np.int32)
+    rc = _lib.tno_oracle_best(snr.ctypes.data_as(_f32p), K, H, W, m.ctypes.data_as(_f32p),
+                              a.ctypes.data_as(_i32p))
+    if rc != 0:
+        raise ValueError("tno_oracle_best failed (%d)" % rc)
+    return m, a
+
+
+def local_z(m, box: int = 255, literal: bool = False):
+    """(Z = M / sigma_box float64 [H, W], sigma_box float64 [H, W]): scores in units of the standard
+    deviation of the scores in the box x box square centred on each pixel, clipped to the frame
+    (PAPER.md:L124).  literal=True evaluates the two-pass definition pixel by pixel (small maps)."""
+    m = _f32(m)
+    H, W = m.shape
+    z = np.empty((H, W), np.float64)
+    s = np.empty((H, W), np.float64)
+    fn = _lib.tno_oracle_local_z if literal else _lib.tno_oracle_local_z_sep
+    rc = fn(m.ctypes.data_as(_f32p), H, W, int(box), z.ctypes.data_as(_f64p), s.ctypes.data_as(_f64p))
+    if rc != 0:
+        raise ValueError("tno_oracle_local_z failed (%d)" % rc)
+    return z, s

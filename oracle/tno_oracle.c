@@ -220,3 +220,105 @@ int tno_oracle_inject(float *frames, int T, int H, int W,
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Interpreting scores (section 3.3, L112 and L122-124; readings e1-e4).
+ *
+ * tno_oracle_best: "We take the maximum score across the filter bank, which then tells us the
+ * most likely trajectory, along with the score of that trajectory" (L112):
+ *     M(x, y) = max_k S_k(x, y),   A(x, y) = the smallest k that attains it.
+ * Scores are float32 (they are the product's output format); comparisons are exact.
+ *
+ * tno_oracle_local_z: "we compute the standard deviation sigma of the scores in the 255 x 255
+ * square centered on a pixel. We represent our scores in units of sigma" (L124):
+ *     B(x, y)   = the pixels (x', y') of the frame with |x' - x| <= h and |y' - y| <= h, h = (box-1)/2
+ *     mean      = sum_B M / |B|,   var = sum_B (M - mean)^2 / |B|      (population variance)
+ *     Z(x, y)   = M(x, y) / sqrt(var)   if var > 0 else 0
+ * The two-pass definition is evaluated literally for every pixel (O(H W box^2): small maps only).
+ * tno_oracle_local_z_sep uses the separability of the box sums of M and M^2 (row sums, then
+ * column sums of those, all float64, var = sum2/|B| - (sum/|B|)^2) and is pinned against the
+ * literal form by tests/test_oracle_pins.py; it is what full-size maps are checked against.
+ */
+int tno_oracle_best(const float *snr, int K, int H, int W, float *out_max, int *out_argk) {
+    if (!snr || K < 1 || H < 1 || W < 1 || !out_max || !out_argk) return -2;
+    for (long p = 0; p < (long)H * W; ++p) {
+        float m = snr[p];
+        int a = 0;
+        for (int k = 1; k < K; ++k) {
+            const float v = snr[(long)k * H * W + p];
+            if (v > m) { m = v; a = k; }
+        }
+        out_max[p] = m;
+        out_argk[p] = a;
+    }
+    return 0;
+}
+
+int tno_oracle_local_z(const float *m, int H, int W, int box, double *out_z, double *out_sigma) {
+    if (!m || H < 1 || W < 1 || box < 1 || (box & 1) == 0 || !out_z) return -2;
+    const int h = (box - 1) / 2;
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            const int y0 = y - h < 0 ? 0 : y - h, y1 = y + h >= H ? H - 1 : y + h;
+            const int x0 = x - h < 0 ? 0 : x - h, x1 = x + h >= W ? W - 1 : x + h;
+            const double n = (double)(y1 - y0 + 1) * (double)(x1 - x0 + 1);
+            double s = 0.0;
+            for (int yy = y0; yy <= y1; ++yy)
+                for (int xx = x0; xx <= x1; ++xx) s += (double)m[(long)yy * W + xx];
+            const double mean = s / n;
+            double v = 0.0;
+            for (int yy = y0; yy <= y1; ++yy)
+                for (int xx = x0; xx <= x1; ++xx) {
+                    const double d = (double)m[(long)yy * W + xx] - mean;
+                    v += d * d;
+                }
+            v /= n;
+            const double sd = v > 0.0 ? sqrt(v) : 0.0;
+            if (out_sigma) out_sigma[(long)y * W + x] = sd;
+            out_z[(long)y * W + x] = sd > 0.0 ? (double)m[(long)y * W + x] / sd : 0.0;
+        }
+    return 0;
+}
+
+int tno_oracle_local_z_sep(const float *m, int H, int W, int box, double *out_z, double *out_sigma) {
+    if (!m || H < 1 || W < 1 || box < 1 || (box & 1) == 0 || !out_z) return -2;
+    const int h = (box - 1) / 2;
+    double *r1 = (double *)malloc(sizeof(double) * (size_t)H * W);
+    double *r2 = (double *)malloc(sizeof(double) * (size_t)H * W);
+    if (!r1 || !r2) { free(r1); free(r2); return -3; }
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            const int x0 = x - h < 0 ? 0 : x - h, x1 = x + h >= W ? W - 1 : x + h;
+            double s = 0.0, q = 0.0;
+            for (int xx = x0; xx <= x1; ++xx) {
+                const double v = (double)m[(long)y * W + xx];
+                s += v;
+                q += v * v;
+            }
+            r1[(long)y * W + x] = s;
+            r2[(long)y * W + x] = q;
+        }
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            const int y0 = y - h < 0 ? 0 : y - h, y1 = y + h >= H ? H - 1 : y + h;
+            const int x0 = x - h < 0 ? 0 : x - h, x1 = x + h >= W ? W - 1 : x + h;
+            const double n = (double)(y1 - y0 + 1) * (double)(x1 - x0 + 1);
+            double s = 0.0, q = 0.0;
+            for (int yy = y0; yy <= y1; ++yy) {
+                s += r1[(long)yy * W + x];
+                q += r2[(long)yy * W + x];
+            }
+            const double mean = s / n;
+            double v = q / n - mean * mean;
+            if (v < 0.0) v = 0.0;
+            const double sd = v > 0.0 ? sqrt(v) : 0.0;
+            if (out_sigma) out_sigma[(long)y * W + x] = sd;
+            out_z[(long)y * W + x] = sd > 0.0 ? (double)m[(long)y * W + x] / sd : 0.0;
+        }
+    free(r1);
+    free(r2);
+    return 0;
+}

@@ -434,3 +434,70 @@ def test_config1_golden_regression():
         s, _, _ = oracle.point(f, p.sigma_t, p.traj[int(k)], p.cfg.prf_sigma, p.cfg.t0,
                                int(x), int(y))
         assert s == pytest.approx(float(val), rel=1e-12, abs=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------
+# Interpreting scores (section 3.3): max over the filter bank (L112), scores in units of
+# the standard deviation of the scores in the box centred on a pixel (L124).
+def test_best_is_max_and_first_argmax():
+    rng = np.random.default_rng(5)
+    s = rng.integers(-3, 4, size=(7, 9, 11)).astype(np.float32)      # many exact ties
+    m, a = oracle.best(s)
+    assert np.array_equal(m, s.max(axis=0))
+    assert np.array_equal(a, s.argmax(axis=0))                         # numpy: first maximal index
+    one = rng.standard_normal((1, 4, 5)).astype(np.float32)
+    m, a = oracle.best(one)
+    assert np.array_equal(m, one[0]) and np.all(a == 0)
+
+
+def test_local_z_literal_against_numpy_slices():
+    rng = np.random.default_rng(6)
+    m = rng.standard_normal((9, 13)).astype(np.float32)
+    for box in (1, 3, 5, 31):                                          # 31 > the map: every box is the whole map
+        z, sd = oracle.local_z(m, box, literal=True)
+        h = (box - 1) // 2
+        for y in range(9):
+            for x in range(13):
+                blk = m[max(0, y - h):y + h + 1, max(0, x - h):x + h + 1].astype(np.float64)
+                ref = np.std(blk)                                      # population standard deviation
+                assert sd[y, x] == pytest.approx(ref, rel=1e-12, abs=1e-15)
+                assert z[y, x] == pytest.approx(float(m[y, x]) / ref if ref > 0 else 0.0, rel=1e-12)
+    z, sd = oracle.local_z(m, 1, literal=True)
+    assert np.all(sd == 0) and np.all(z == 0)                          # a single pixel has no spread
+
+
+def test_local_z_separable_form_matches_literal():
+    rng = np.random.default_rng(7)
+    m = (rng.standard_normal((61, 77)) * 3 + 10).astype(np.float32)   # offset: tests the variance formula
+    for box in (3, 11, 255):
+        z1, s1 = oracle.local_z(m, box, literal=True)
+        z2, s2 = oracle.local_z(m, box)
+        assert np.max(np.abs(s1 - s2)) <= 1e-9 and np.max(np.abs(z1 - z2)) <= 1e-7
+
+
+def test_local_z_closed_forms_and_invariances():
+    H = W = 40
+    assert np.all(oracle.local_z(np.full((H, W), 2.5, np.float32), 7)[0] == 0)      # constant map
+    yy, xx = np.mgrid[0:H, 0:W]
+    cb = np.where((yy + xx) % 2 == 0, 1.0, -1.0).astype(np.float32)
+    n = 7
+    z, sd = oracle.local_z(cb, n)
+    # interior: (n^2 + 1)/2 pixels of the centre's sign, mean = +-1/n^2, variance = 1 - 1/n^4
+    assert np.allclose(sd[5:-5, 5:-5], math.sqrt(1.0 - 1.0 / n ** 4), rtol=0, atol=1e-12)
+    assert np.allclose(z[5:-5, 5:-5], cb[5:-5, 5:-5].astype(np.float64) / math.sqrt(1.0 - 1.0 / n ** 4), rtol=0, atol=1e-12)
+    # corner (0, 0): a 4 x 4 block with 8 pixels of each sign -> variance 1
+    assert sd[0, 0] == pytest.approx(1.0, abs=1e-12)
+    rng = np.random.default_rng(8)
+    m = rng.standard_normal((H, W)).astype(np.float32)
+    z1 = oracle.local_z(m, 9)[0]
+    assert np.allclose(oracle.local_z(4.0 * m, 9)[0], z1, rtol=1e-12)             # units of sigma
+    assert np.allclose(oracle.local_z(-m, 9)[0], -z1, rtol=1e-12)
+    assert np.allclose(oracle.local_z(m[::-1, ::-1].copy(), 9)[0], z1[::-1, ::-1], rtol=1e-12)
+
+
+def test_local_sigma_of_unit_noise_is_one():
+    rng = np.random.default_rng(9)
+    m = rng.standard_normal((300, 300)).astype(np.float32)
+    _, sd = oracle.local_z(m, 255)
+    assert abs(sd[150, 150] - 1.0) < 4.0 / math.sqrt(2 * 255 * 255)
+    assert abs(sd[0, 0] - 1.0) < 4.0 / math.sqrt(2 * 128 * 128)
