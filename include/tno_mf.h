@@ -111,6 +111,25 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
                   const tno_mf_source *sources, int32_t n_sources,
                   float prf_sigma, float t0);
 
+/* Interpreting scores (section 3.3): "We take the maximum score across the filter bank, which
+ * then tells us the most likely trajectory, along with the score of that trajectory" (L112), and "we
+ * compute the standard deviation sigma of the scores in the 255 x 255 square centered on a pixel. We
+ * represent our scores in units of sigma" (L124):
+ *     M(x, y) = max_k snr[k][y][x],  A(x, y) = the smallest k that attains it
+ *     Z(x, y) = M(x, y) / sigma_box(x, y), sigma_box = population standard deviation of M over the
+ *               pixels of the frame within (box-1)/2 of (x, y) in both axes; 0 where it vanishes
+ *   snr       DEVICE float32 [n_traj][H][W] (e.g. out_snr of tno_mf_search).  Read only.
+ *   box       odd, >= 1 (the paper uses 255).
+ *   out_max   DEVICE float32 [H][W].                  out_argk  DEVICE int32 [H][W], or NULL.
+ *   out_z     DEVICE float32 [H][W], or NULL.
+ *   out_topk  DEVICE [topk] records of the pixels with the largest Z >= cfg.snr_threshold (now in
+ *             units of sigma_box), ordered (Z descending, y, x ascending), record.snr = Z, record.k =
+ *             A(x, y); unused tail {-INFINITY, -1, -1, -1}; or NULL (or topk == 0).
+ * sigma_box is evaluated in float64 from summed-area tables; a variance below 1e-12 of the box's mean
+ * square counts as zero.  Errors: EINVAL (NULL snr/out_max, sizes < 1, even box), ENOMEM, ECUDA. */
+int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, int32_t box,
+                float *out_max, int32_t *out_argk, float *out_z, tno_mf_cand *out_topk);
+
 /* Host-only planning query (no device work; ctx may be NULL): how the search would group
  * `trajectories` into batches that share one x-motion (vx, ax) -- the unit of work of the
  * separable kernel.  Writes, for each trajectory, its batch index and slot

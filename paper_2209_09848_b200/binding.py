@@ -50,6 +50,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_create.argtypes = [ctypes.POINTER(tno_mf_config), ctypes.POINTER(vp)]
     lib.tno_mf_search.restype = ctypes.c_int
     lib.tno_mf_search.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_best.restype = ctypes.c_int
+    lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
     lib.tno_mf_plan.restype = ctypes.c_int
@@ -132,6 +134,25 @@ def tno_mf_search(ctx, frames, sigma_t, trajectories, prf_sigma: float, t0: floa
         p_top = out_topk.data_ptr()
     _check(_lib.tno_mf_search(ctx, frames.data_ptr(), T, H, W, sig.ctypes.data, tr.ctypes.data, n,
                               float(prf_sigma), float(t0), p_snr, p_top), ctx)
+
+
+def tno_mf_best(ctx, snr, box: int, out_max, out_argk=None, out_z=None, out_topk=None) -> None:
+    """snr: CUDA float32 tensor [n, H, W]; out_max / out_z: CUDA float32 [H, W]; out_argk: CUDA int32
+    [H, W]; out_topk: CUDA tensor with topk*16 bytes.  Enqueues on the context's stream."""
+    assert snr.is_cuda and snr.is_contiguous() and snr.dim() == 3 and snr.element_size() == 4
+    n, H, W = snr.shape
+    ptrs = []
+    for t, es in ((out_max, 4), (out_argk, 4), (out_z, 4)):
+        if t is None:
+            ptrs.append(None)
+            continue
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == es and t.numel() == H * W
+        ptrs.append(t.data_ptr())
+    p_top = None
+    if out_topk is not None:
+        assert out_topk.is_cuda and out_topk.is_contiguous()
+        p_top = out_topk.data_ptr()
+    _check(_lib.tno_mf_best(ctx, snr.data_ptr(), n, H, W, int(box), ptrs[0], ptrs[1], ptrs[2], p_top), ctx)
 
 
 def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float) -> None:

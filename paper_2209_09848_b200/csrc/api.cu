@@ -34,7 +34,7 @@ struct tno_mf_ctx {
     std::vector<cudaEvent_t> ev;      // pairs (before, after) around each main search kernel launch
     int32_t ev_used = 0;              // events recorded by the last search
     // grow-only device workspace
-    DevBuf meta, shift, g, gd, ab, rsd, stage_tab, pieces, keys, counts, tmp_maps, src;
+    DevBuf meta, shift, g, gd, ab, rsd, stage_tab, pieces, keys, counts, tmp_maps, src, sat, ztmp;
 };
 
 namespace {
@@ -205,7 +205,7 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     if (!ctx) return TNO_MF_OK;
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
-                      &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src};
+                      &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -264,6 +264,56 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
                                 cudaMemcpyHostToDevice, ctx->stream));
     launch_inject(ctx->stream, frames, T, H, W, static_cast<const SourceDev *>(ctx->src.p), n_sources,
                   (double)prf_sigma, (double)t0);
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
+}
+
+int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, int32_t box,
+                float *out_max, int32_t *out_argk, float *out_z, tno_mf_cand *out_topk) {
+    if (!ctx) return TNO_MF_EINVAL;
+    ctx->last_launches = 0;
+    if (!snr || !out_max) return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: NULL snr or out_max");
+    if (n_traj < 1 || H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 31)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: n_traj, H, W must be >= 1 and H*W <= 2^31");
+    if (box < 1 || (box & 1) == 0) return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: box must be odd and >= 1");
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = ctx->stream;
+    const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
+    int rc;
+    int32_t *argk = out_argk;
+    const size_t px = (size_t)H * W;
+    if (want_topk && !argk) {          // the records carry the arg-max trajectory
+        if ((rc = reserve(ctx, ctx->tmp_maps, px * 4))) return rc;
+        argk = static_cast<int32_t *>(ctx->tmp_maps.p);
+    }
+    launch_max_map(st, snr, n_traj, H, W, out_max, argk, ctx->n_sm);
+    ctx->last_launches += 1;
+    if (out_z || want_topk) {
+        float *z = out_z;
+        if (!z) {
+            if ((rc = reserve(ctx, ctx->ztmp, px * 4))) return rc;
+            z = static_cast<float *>(ctx->ztmp.p);
+        }
+        if ((rc = reserve(ctx, ctx->sat, px * 16))) return rc;
+        launch_local_z(st, out_max, H, W, box, ctx->sat.p, z);
+        ctx->last_launches += 3;
+        if (want_topk) {
+            const int32_t ntx = (W + kCollectTile - 1) / kCollectTile, nty = (H + kCollectTile - 1) / kCollectTile;
+            const int64_t n_tiles = (int64_t)ntx * nty;
+            if ((rc = reserve(ctx, ctx->keys, (size_t)n_tiles * ctx->cfg.topk * 8))) return rc;
+            if ((rc = reserve(ctx, ctx->counts, (size_t)n_tiles * 4))) return rc;
+            TopkSlots slots;
+            slots.keys = static_cast<uint64_t *>(ctx->keys.p);
+            slots.counts = static_cast<int32_t *>(ctx->counts.p);
+            slots.ktop = ctx->cfg.topk;
+            slots.K = 1;
+            slots.threshold = ctx->cfg.snr_threshold;
+            launch_collect_from_map(st, z, H, W, 0, 1, slots);
+            launch_topk_merge(st, slots, (int32_t)n_tiles, W, out_topk);
+            launch_set_argk(st, out_topk, ctx->cfg.topk, argk, W);
+            ctx->last_launches += 3;
+        }
+    }
     CU_TRY(ctx, cudaGetLastError());
     return TNO_MF_OK;
 }

@@ -1,0 +1,156 @@
+// Interpreting scores (section 3.3):
+//   k_max_map    M(x,y) = max_k S_k(x,y) and the smallest k that attains it -- "We take the maximum
+//                score across the filter bank, which then tells us the most likely trajectory" (L112)
+//   k_sat_rows / k_sat_cols   float64 summed-area tables of M and M^2
+//   k_local_z    Z = M / sigma_box, sigma_box = population standard deviation of M in the box x box
+//                square centred on the pixel, clipped to the frame -- "we compute the standard
+//                deviation of the scores in the 255 x 255 square centered on a pixel. We represent
+//                our scores in units of sigma" (L124)
+//   k_set_argk   writes the arg-max trajectory into the candidate records of the Z map
+// All of it is HBM-bound streaming work: K maps read once, then a few passes over one map.
+#include "kernels.h"
+
+namespace tno {
+
+// grid-stride over groups of 4 pixels (n_px % 4 == 0 is not required: scalar tail)
+__global__ void __launch_bounds__(256)
+k_max_map(const float *__restrict__ snr, int32_t K, int64_t n_px, float *__restrict__ out_max,
+          int32_t *__restrict__ out_argk) {
+    const int64_t n4 = n_px / 4;
+    const bool vec = (reinterpret_cast<uintptr_t>(snr) & 15u) == 0 && (n_px % 4) == 0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vec) {
+        for (int64_t i = id; i < n4; i += stride) {
+            float4 m = __ldcs(reinterpret_cast<const float4 *>(snr) + i);
+            int4 a = make_int4(0, 0, 0, 0);
+            for (int32_t k = 1; k < K; ++k) {
+                const float4 v = __ldcs(reinterpret_cast<const float4 *>(snr + (int64_t)k * n_px) + i);
+                if (v.x > m.x) { m.x = v.x; a.x = k; }
+                if (v.y > m.y) { m.y = v.y; a.y = k; }
+                if (v.z > m.z) { m.z = v.z; a.z = k; }
+                if (v.w > m.w) { m.w = v.w; a.w = k; }
+            }
+            reinterpret_cast<float4 *>(out_max)[i] = m;
+            if (out_argk) reinterpret_cast<int4 *>(out_argk)[i] = a;
+        }
+    } else {
+        for (int64_t i = id; i < n_px; i += stride) {
+            float m = snr[i];
+            int32_t a = 0;
+            for (int32_t k = 1; k < K; ++k) {
+                const float v = snr[(int64_t)k * n_px + i];
+                if (v > m) { m = v; a = k; }
+            }
+            out_max[i] = m;
+            if (out_argk) out_argk[i] = a;
+        }
+    }
+}
+
+// One block per row: inclusive prefix sums along x of (M, M^2) in float64.
+__global__ void __launch_bounds__(256)
+k_sat_rows(const float *__restrict__ m, int32_t W, double2 *__restrict__ sat) {
+    __shared__ double2 wsum[8];
+    const int32_t y = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int32_t per = (W + 255) / 256;
+    const int32_t x0 = tid * per, x1 = min(W, x0 + per);
+    const float *row = m + (int64_t)y * W;
+    double2 loc = make_double2(0.0, 0.0);
+    for (int32_t x = x0; x < x1; ++x) {
+        const double v = (double)row[x];
+        loc.x += v;
+        loc.y += v * v;
+    }
+    double2 inc = loc;
+    for (int o = 1; o < 32; o <<= 1) {
+        const double a = __shfl_up_sync(0xffffffffu, inc.x, o), b = __shfl_up_sync(0xffffffffu, inc.y, o);
+        if (lane >= o) { inc.x += a; inc.y += b; }
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    double2 run = make_double2(inc.x - loc.x, inc.y - loc.y);
+    for (int32_t w = 0; w < warp; ++w) { run.x += wsum[w].x; run.y += wsum[w].y; }
+    double2 *out = sat + (int64_t)y * W;
+    for (int32_t x = x0; x < x1; ++x) {
+        const double v = (double)row[x];
+        run.x += v;
+        run.y += v * v;
+        out[x] = run;
+    }
+}
+
+// One block per 32 columns, 32 warps: warp w walks the rows [w*chunk, (w+1)*chunk) of its columns
+// (lanes across columns: 512-byte coalesced rows of double2), in place.
+__global__ void __launch_bounds__(1024)
+k_sat_cols(double2 *__restrict__ sat, int32_t H, int32_t W) {
+    __shared__ double2 tot[32][33];
+    const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int32_t x = blockIdx.x * 32 + lane;
+    const int32_t chunk = (H + 31) / 32;
+    const int32_t y0 = warp * chunk, y1 = min(H, y0 + chunk);
+    double2 s = make_double2(0.0, 0.0);
+    if (x < W)
+        for (int32_t y = y0; y < y1; ++y) {
+            const double2 v = sat[(int64_t)y * W + x];
+            s.x += v.x;
+            s.y += v.y;
+        }
+    tot[warp][lane] = s;
+    __syncthreads();
+    double2 run = make_double2(0.0, 0.0);
+    for (int32_t w = 0; w < warp; ++w) { run.x += tot[w][lane].x; run.y += tot[w][lane].y; }
+    if (x < W)
+        for (int32_t y = y0; y < y1; ++y) {
+            double2 v = sat[(int64_t)y * W + x];
+            run.x += v.x;
+            run.y += v.y;
+            sat[(int64_t)y * W + x] = run;
+        }
+}
+
+__global__ void __launch_bounds__(256)
+k_local_z(const float *__restrict__ m, const double2 *__restrict__ sat, int32_t H, int32_t W, int32_t h,
+          float *__restrict__ z) {
+    const int32_t x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
+    if (x >= W || y >= H) return;
+    const int32_t x0 = max(0, x - h), x1 = min(W - 1, x + h), y0 = max(0, y - h), y1 = min(H - 1, y + h);
+    auto at = [&](int32_t yy, int32_t xx) -> double2 {
+        if (yy < 0 || xx < 0) return make_double2(0.0, 0.0);
+        return sat[(int64_t)yy * W + xx];
+    };
+    const double2 a = at(y1, x1), b = at(y1, x0 - 1), c = at(y0 - 1, x1), d = at(y0 - 1, x0 - 1);
+    const double n = (double)(y1 - y0 + 1) * (double)(x1 - x0 + 1);
+    const double s = ((a.x - b.x) - c.x) + d.x, q = ((a.y - b.y) - c.y) + d.y;
+    const double mean = s / n;
+    const double var = q / n - mean * mean;
+    // differences of large sums: a variance below this relative floor is rounding noise of a constant box
+    const double floor_v = 1e-12 * (q / n);
+    z[(int64_t)y * W + x] = var > floor_v ? (float)((double)m[(int64_t)y * W + x] / sqrt(var)) : 0.0f;
+}
+
+__global__ void k_set_argk(tno_mf_cand *__restrict__ cand, int32_t n, const int32_t *__restrict__ argk, int32_t W) {
+    const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    tno_mf_cand c = cand[i];
+    c.k = (c.x >= 0) ? argk[(int64_t)c.y * W + c.x] : -1;
+    cand[i] = c;
+}
+
+void launch_max_map(cudaStream_t st, const float *snr, int32_t K, int32_t H, int32_t W, float *out_max,
+                    int32_t *out_argk, int32_t n_sm) {
+    k_max_map<<<(unsigned)(n_sm * 8), 256, 0, st>>>(snr, K, (int64_t)H * W, out_max, out_argk);
+}
+
+void launch_local_z(cudaStream_t st, const float *m, int32_t H, int32_t W, int32_t box, void *sat_ws, float *z) {
+    double2 *sat = static_cast<double2 *>(sat_ws);
+    k_sat_rows<<<(unsigned)H, 256, 0, st>>>(m, W, sat);
+    k_sat_cols<<<(unsigned)((W + 31) / 32), 1024, 0, st>>>(sat, H, W);
+    dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4));
+    k_local_z<<<grid, 256, 0, st>>>(m, sat, H, W, (box - 1) / 2, z);
+}
+
+void launch_set_argk(cudaStream_t st, tno_mf_cand *cand, int32_t n, const int32_t *argk, int32_t W) {
+    k_set_argk<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(cand, n, argk, W);
+}
+
+}  // namespace tno

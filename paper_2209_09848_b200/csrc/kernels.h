@@ -33,6 +33,13 @@ void launch_collect_from_map(cudaStream_t st, const float *maps, int32_t H, int3
 void launch_topk_merge(cudaStream_t st, const TopkSlots &slots, int32_t n_tiles, int32_t W,
                        tno_mf_cand *out_topk);
 
+// ---- best.cu ---- (section 3.3: max over the filter bank, scores in local-sigma units)
+void launch_max_map(cudaStream_t st, const float *snr, int32_t K, int32_t H, int32_t W, float *out_max,
+                    int32_t *out_argk /* may be NULL */, int32_t n_sm);
+// sat_ws: H*W*16 bytes of workspace (float64 summed-area tables of M and M^2)
+void launch_local_z(cudaStream_t st, const float *m, int32_t H, int32_t W, int32_t box, void *sat_ws, float *z);
+void launch_set_argk(cudaStream_t st, tno_mf_cand *cand, int32_t n, const int32_t *argk, int32_t W);
+
 // ---- inject.cu ----
 struct SourceDev { float vx, vy, ax, ay; int32_t x, y; float amp; };
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,

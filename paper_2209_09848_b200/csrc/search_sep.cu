@@ -25,8 +25,8 @@
 // Structure:
 //   * persistent CTAs, one per SM, walk (tile, batch) work items batch-fastest, so the batches of
 //     one tile run on neighbouring CTAs at the same time and share the frame tiles in L2;
-//   * warp-specialised: one producer warpgroup (32 registers per thread after setmaxnreg) issues
-//     the TMA loads and runs the x-pass, 12 consumer warps (160 registers) run the y-pass; the
+//   * warp-specialised: one producer warpgroup (56 registers per thread after setmaxnreg) issues
+//     the TMA loads and runs the x-pass, 12 consumer warps (152 registers) run the y-pass; the
 //     roles are linked by mbarrier rings only, there is no CTA-wide barrier in the frame loop;
 //   * frame tiles of (HT + 4) rows x 76 columns are staged by TMA (cp.async.bulk.tensor.3d, zero
 //     fill outside the frame = "dropped from N") into a ring of box stages together with the

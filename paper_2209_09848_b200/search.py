@@ -53,6 +53,18 @@ class MatchedFilter:
                         out_snr if want_maps else None, out_topk if self.topk > 0 else None)
         return (out_snr if want_maps else None), (out_topk if self.topk > 0 else None)
 
+    def best(self, snr, box: int = 255):
+        """PAPER.md section 3.3 on SNR maps [n, H, W]: (max over trajectories, arg-max trajectory, Z =
+        max / local sigma of the box, top-K records of Z or None); asynchronous."""
+        torch = self._torch
+        n, H, W = snr.shape
+        mx = torch.empty((H, W), dtype=torch.float32, device=snr.device)
+        ak = torch.empty((H, W), dtype=torch.int32, device=snr.device)
+        z = torch.empty((H, W), dtype=torch.float32, device=snr.device)
+        top = torch.empty((self.topk, 4), dtype=torch.int32, device=snr.device) if self.topk > 0 else None
+        B.tno_mf_best(self.ctx, snr, box, mx, ak, z, top)
+        return mx, ak, z, top
+
     def inject(self, frames, trajs, xs, ys, amps, prf_sigma: float, t0: float) -> None:
         B.tno_mf_inject(self.ctx, frames, B.make_sources(trajs, xs, ys, amps), prf_sigma, t0)
 
