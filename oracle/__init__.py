@@ -39,6 +39,25 @@ _lib.tno_oracle_inject.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_i
 CAND_DTYPE = np.dtype([("snr", np.float64), ("x", np.int32), ("y", np.int32), ("k", np.int32)])
 
 
+_lib.tno_oracle_point_ex.restype = ctypes.c_int
+_lib.tno_oracle_point_ex.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, _f32p, _f32p, ctypes.c_float,
+                                     ctypes.c_float, ctypes.c_int, ctypes.c_int, _f64p, _f64p, _f64p]
+_lib.tno_oracle_map_ex.restype = ctypes.c_int
+_lib.tno_oracle_map_ex.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, _f32p, _f32p, ctypes.c_int,
+                                   ctypes.c_float, ctypes.c_float] + [ctypes.c_int] * 4 + [_f64p] * 3
+_lib.tno_oracle_inject_ex.restype = ctypes.c_int
+_lib.tno_oracle_inject_ex.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f32p, _f32p, _f32p,
+                                      _i32p, _i32p, _f32p, ctypes.c_int, ctypes.c_float, ctypes.c_float]
+
+
+def _opt(a, shape):
+    """Optional float32 array -> (keep-alive array, pointer or None)."""
+    if a is None:
+        return None, None
+    a = _f32(a, shape)
+    return a, a.ctypes.data_as(_f32p)
+
+
 def threads() -> int:
     return int(_lib.tno_oracle_threads())
 
@@ -60,25 +79,28 @@ def _geom(frames: np.ndarray, window, full_shape):
     return T, H, W, int(wx0), int(wy0), ww, wh
 
 
-def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=None
-          ) -> Tuple[float, float, float]:
-    """(snr, N, D) at start pixel (x, y) for one trajectory (vx, vy, ax, ay)."""
+def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=None,
+          times=None, jitter=None) -> Tuple[float, float, float]:
+    """(snr, N, D) at start pixel (x, y) for one trajectory (vx, vy, ax, ay).  times: frame times [T]
+    (default the frame index), jitter: pointing offsets [T, 2] in px added to the track (default 0)."""
     frames = _f32(frames)
     T, H, W, wx0, wy0, ww, wh = _geom(frames, window, full_shape)
     sigma_t = _f32(sigma_t, (T,))
     traj = _f32(traj, (4,))
     N, D, S = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
-    rc = _lib.tno_oracle_point(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
-                               sigma_t.ctypes.data_as(_f32p), traj.ctypes.data_as(_f32p),
-                               float(prf_sigma), float(t0), int(x), int(y),
-                               ctypes.byref(N), ctypes.byref(D), ctypes.byref(S))
+    _ta, tp = _opt(times, (T,))
+    _ja, jp = _opt(jitter, (T, 2))
+    rc = _lib.tno_oracle_point_ex(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
+                                  sigma_t.ctypes.data_as(_f32p), tp, jp, traj.ctypes.data_as(_f32p),
+                                  float(prf_sigma), float(t0), int(x), int(y),
+                                  ctypes.byref(N), ctypes.byref(D), ctypes.byref(S))
     if rc != 0:
         raise ValueError("oracle.point: tap outside the supplied window (rc=%d)" % rc)
     return S.value, N.value, D.value
 
 
 def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, full_shape=None,
-            return_ND: bool = False):
+            return_ND: bool = False, times=None, jitter=None):
     """float64 [K, h, w] SNR for start pixels x in [x_lo, x_hi), y in [y_lo, y_hi)
     (region = (x_lo, x_hi, y_lo, y_hi), default the whole frame)."""
     frames = _f32(frames)
@@ -91,8 +113,10 @@ def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, ful
     out = np.empty((K, y_hi - y_lo, x_hi - x_lo), dtype=np.float64)
     oN = np.empty_like(out) if return_ND else None
     oD = np.empty_like(out) if return_ND else None
-    rc = _lib.tno_oracle_map(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
-                             sigma_t.ctypes.data_as(_f32p), trajs.ctypes.data_as(_f32p), K,
+    _ta, tp = _opt(times, (T,))
+    _ja, jp = _opt(jitter, (T, 2))
+    rc = _lib.tno_oracle_map_ex(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
+                             sigma_t.ctypes.data_as(_f32p), tp, jp, trajs.ctypes.data_as(_f32p), K,
                              float(prf_sigma), float(t0), int(x_lo), int(x_hi), int(y_lo),
                              int(y_hi), out.ctypes.data_as(_f64p),
                              oN.ctypes.data_as(_f64p) if return_ND else None,
@@ -123,7 +147,7 @@ def topk(snr: np.ndarray, ktop: int, threshold: float, k_index: int = 0,
     return out
 
 
-def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0) -> None:
+def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0, times=None, jitter=None) -> None:
     """In place: add amp * g(p - c_t) for each source (full-frame float32 [T, H, W] buffer)."""
     assert frames.dtype == np.float32 and frames.flags.c_contiguous and frames.ndim == 3
     T, H, W = frames.shape
@@ -133,7 +157,9 @@ def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0) -> None:
     ys = np.ascontiguousarray(ys, dtype=np.int32)
     amps = _f32(amps, (n,))
     assert xs.shape == (n,) and ys.shape == (n,) and trajs.shape == (n, 4)
-    rc = _lib.tno_oracle_inject(frames.ctypes.data_as(_f32p), T, H, W,
+    _ta, tp = _opt(times, (T,))
+    _ja, jp = _opt(jitter, (T, 2))
+    rc = _lib.tno_oracle_inject_ex(frames.ctypes.data_as(_f32p), T, H, W, tp, jp,
                                 trajs.ctypes.data_as(_f32p), xs.ctypes.data_as(_i32p),
                                 ys.ctypes.data_as(_i32p), amps.ctypes.data_as(_f32p), n,
                                 float(prf_sigma), float(t0))

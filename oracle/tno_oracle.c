@@ -58,6 +58,18 @@ typedef struct {
 
 static inline double disp(double v, double a, double dt) { return v * dt + a * dt * dt; }
 
+/* Time of frame t and pointing jitter of frame t (readings f1-f3): the filter is "the line
+ * of the trajectory (including the pointing jitter)" and the frames are not equally
+ * spaced ("the time-jump that occurs when TESS is transmitting frames to Earth", L116).
+ *     c_t = (x, y) + v (tau_t - t0) + a (tau_t - t0)^2 + j_t
+ * times == NULL: tau_t = t;  jitter == NULL: j_t = 0;  jitter[2t], jitter[2t+1] = (jx_t, jy_t) in px. */
+static inline double frame_dt(const float *times, int t, double t0) {
+    return (times ? (double)times[t] : (double)t) - t0;
+}
+static inline double jit(const float *jitter, int t, int axis) {
+    return jitter ? (double)jitter[2 * t + axis] : 0.0;
+}
+
 /* round-half-up of a displacement: integer shift s and phase d - s in [-0.5, 0.5) */
 static inline void split(double d, int *s, double *ph) {
     double f = floor(d + 0.5);
@@ -74,19 +86,20 @@ int tno_oracle_threads(void) {
 }
 
 /* literal definition, one exp per tap */
-int tno_oracle_point(const float *frames, int T, int H, int W,
-                     int wx0, int wy0, int ww, int wh,
-                     const float *sigma_t, const float *traj4, float prf_sigma_f, float t0_f,
-                     int x, int y, double *N_out, double *D_out, double *snr_out)
+int tno_oracle_point_ex(const float *frames, int T, int H, int W,
+                        int wx0, int wy0, int ww, int wh,
+                        const float *sigma_t, const float *times, const float *jitter,
+                        const float *traj4, float prf_sigma_f, float t0_f,
+                        int x, int y, double *N_out, double *D_out, double *snr_out)
 {
     const double vx = traj4[0], vy = traj4[1], ax = traj4[2], ay = traj4[3];
     const double s = prf_sigma_f, t0 = t0_f;
     double N = 0.0, D = 0.0;
     for (int t = 0; t < T; ++t) {
-        const double dt = (double)t - t0;
+        const double dt = frame_dt(times, t, t0);
         int sx, sy; double phx, phy;
-        split(disp(vx, ax, dt), &sx, &phx);
-        split(disp(vy, ay, dt), &sy, &phy);
+        split(disp(vx, ax, dt) + jit(jitter, t, 0), &sx, &phx);
+        split(disp(vy, ay, dt) + jit(jitter, t, 1), &sy, &phy);
         const double sig = sigma_t[t];
         const double q = 1.0 / (sig * sig);
         for (int j = -2; j <= 2; ++j) {
@@ -108,15 +121,25 @@ int tno_oracle_point(const float *frames, int T, int H, int W,
     return 0;
 }
 
+int tno_oracle_point(const float *frames, int T, int H, int W,
+                     int wx0, int wy0, int ww, int wh,
+                     const float *sigma_t, const float *traj4, float prf_sigma_f, float t0_f,
+                     int x, int y, double *N_out, double *D_out, double *snr_out)
+{
+    return tno_oracle_point_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, traj4,
+                               prf_sigma_f, t0_f, x, y, N_out, D_out, snr_out);
+}
+
 /* same sums, per-(k,t) quantities hoisted out of the pixel loop.
  * Region of start pixels: x in [x_lo, x_hi), y in [y_lo, y_hi).
  * out_snr / out_N / out_D: double [K][y_hi-y_lo][x_hi-x_lo]; out_N, out_D may be NULL. */
-int tno_oracle_map(const float *frames, int T, int H, int W,
-                   int wx0, int wy0, int ww, int wh,
-                   const float *sigma_t, const float *traj, int K,
-                   float prf_sigma_f, float t0_f,
-                   int x_lo, int x_hi, int y_lo, int y_hi,
-                   double *out_snr, double *out_N, double *out_D)
+int tno_oracle_map_ex(const float *frames, int T, int H, int W,
+                      int wx0, int wy0, int ww, int wh,
+                      const float *sigma_t, const float *times, const float *jitter,
+                      const float *traj, int K,
+                      float prf_sigma_f, float t0_f,
+                      int x_lo, int x_hi, int y_lo, int y_hi,
+                      double *out_snr, double *out_N, double *out_D)
 {
     const double s = prf_sigma_f, t0 = t0_f;
     const int rw = x_hi - x_lo, rh = y_hi - y_lo;
@@ -129,10 +152,10 @@ int tno_oracle_map(const float *frames, int T, int H, int W,
         const double vx = traj[4 * k + 0], vy = traj[4 * k + 1];
         const double ax = traj[4 * k + 2], ay = traj[4 * k + 3];
         for (int t = 0; t < T; ++t) {
-            const double dt = (double)t - t0;
+            const double dt = frame_dt(times, t, t0);
             int sx, sy; double phx, phy;
-            split(disp(vx, ax, dt), &sx, &phx);
-            split(disp(vy, ay, dt), &sy, &phy);
+            split(disp(vx, ax, dt) + jit(jitter, t, 0), &sx, &phx);
+            split(disp(vy, ay, dt) + jit(jitter, t, 1), &sy, &phy);
             SX[2 * t] = sx; SX[2 * t + 1] = sy;
             for (int i = -2; i <= 2; ++i) {
                 const double ux = (double)i - phx, uy = (double)i - phy;
@@ -188,13 +211,24 @@ int tno_oracle_map(const float *frames, int T, int H, int W,
     return err;
 }
 
+int tno_oracle_map(const float *frames, int T, int H, int W,
+                   int wx0, int wy0, int ww, int wh,
+                   const float *sigma_t, const float *traj, int K,
+                   float prf_sigma_f, float t0_f,
+                   int x_lo, int x_hi, int y_lo, int y_hi,
+                   double *out_snr, double *out_N, double *out_D)
+{
+    return tno_oracle_map_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, traj, K,
+                             prf_sigma_f, t0_f, x_lo, x_hi, y_lo, y_hi, out_snr, out_N, out_D);
+}
+
 /* Injection: for each source, in order, add amp * g(p - c_t) on the 25 taps of
  * every frame, computed in double and rounded once to float32:
  *     R <- (float)((double)R + amp * g).
  * Works on a full-frame buffer [T][H][W].  traj: [n][4] per source. */
-int tno_oracle_inject(float *frames, int T, int H, int W,
-                      const float *traj, const int *xs, const int *ys, const float *amp, int n,
-                      float prf_sigma_f, float t0_f)
+int tno_oracle_inject_ex(float *frames, int T, int H, int W, const float *times, const float *jitter,
+                         const float *traj, const int *xs, const int *ys, const float *amp, int n,
+                         float prf_sigma_f, float t0_f)
 {
     const double s = prf_sigma_f, t0 = t0_f;
     for (int m = 0; m < n; ++m) {
@@ -202,10 +236,10 @@ int tno_oracle_inject(float *frames, int T, int H, int W,
         const double ax = traj[4 * m + 2], ay = traj[4 * m + 3];
         const double A = amp[m];
         for (int t = 0; t < T; ++t) {
-            const double dt = (double)t - t0;
+            const double dt = frame_dt(times, t, t0);
             int sx, sy; double phx, phy;
-            split(disp(vx, ax, dt), &sx, &phx);
-            split(disp(vy, ay, dt), &sy, &phy);
+            split(disp(vx, ax, dt) + jit(jitter, t, 0), &sx, &phx);
+            split(disp(vy, ay, dt) + jit(jitter, t, 1), &sy, &phy);
             for (int j = -2; j <= 2; ++j) {
                 for (int i = -2; i <= 2; ++i) {
                     const int px = xs[m] + sx + i, py = ys[m] + sy + j;
@@ -219,6 +253,13 @@ int tno_oracle_inject(float *frames, int T, int H, int W,
         }
     }
     return 0;
+}
+
+int tno_oracle_inject(float *frames, int T, int H, int W,
+                      const float *traj, const int *xs, const int *ys, const float *amp, int n,
+                      float prf_sigma_f, float t0_f)
+{
+    return tno_oracle_inject_ex(frames, T, H, W, NULL, NULL, traj, xs, ys, amp, n, prf_sigma_f, t0_f);
 }
 
 /* ------------------------------------------------------------------------------------------
