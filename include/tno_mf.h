@@ -101,6 +101,23 @@ int tno_mf_search(tno_mf_ctx *ctx,
                   float *out_snr,
                   tno_mf_cand *out_topk);
 
+/* The search with frame times and pointing jitter in the track -- the filter is "the line of the trajectory
+ * (including the pointing jitter)" and the frames of a sector are not equally spaced
+ * ("the time-jump that occurs when TESS is transmitting frames to Earth", L116):
+ *     c_t = (x, y) + v (tau_t - t0) + a (tau_t - t0)^2 + j_t
+ *   frame_times  HOST float32 [T], tau_t in the time unit of the velocities, or NULL (tau_t = t).
+ *   jitter_xy    HOST float32 [T][2], (jx_t, jy_t) in px, or NULL (no jitter).
+ * Everything else as tno_mf_search, which is this call with both NULL.  Rounding, window, PRF and the
+ * dropping of off-frame taps are unchanged (readings c1-c8, f1-f3); only the per-(trajectory,
+ * frame) table differs, so the cost is the same.  Additional error: EINVAL for non-finite entries. */
+int tno_mf_search_ex(tno_mf_ctx *ctx,
+                     const float *frames, int32_t T, int32_t H, int32_t W,
+                     const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                     const tno_mf_traj *trajectories, int32_t n_traj,
+                     float prf_sigma, float t0,
+                     float *out_snr,
+                     tno_mf_cand *out_topk);
+
 /* Signal injection ("signal injection corresponds to adding a filter times a flux
  * to the raw data"): for each source m in order and every frame t,
  *     R_t(p) <- (float)((double)R_t(p) + amplitude_m * g(p - c_t))  on the 25 window taps,

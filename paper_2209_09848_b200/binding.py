@@ -50,6 +50,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_create.argtypes = [ctypes.POINTER(tno_mf_config), ctypes.POINTER(vp)]
     lib.tno_mf_search.restype = ctypes.c_int
     lib.tno_mf_search.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_search_ex.restype = ctypes.c_int
+    lib.tno_mf_search_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_best.restype = ctypes.c_int
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
@@ -115,12 +117,29 @@ def tno_mf_search(ctx, frames, sigma_t, trajectories, prf_sigma: float, t0: floa
     """frames: CUDA float32 tensor [T, H, W] (contiguous); sigma_t: host float32 [T];
     trajectories: host [n, 4]; out_snr: CUDA float32 tensor [n, H, W] or None; out_topk: CUDA
     uint8/int32 tensor with n*topk*16 bytes or None.  Enqueues on the context's stream."""
+    tno_mf_search_ex(ctx, frames, sigma_t, None, None, trajectories, prf_sigma, t0, out_snr, out_topk,
+                     _plain=True)
+
+
+def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
+                     out_snr=None, out_topk=None, _plain: bool = False) -> None:
+    """tno_mf_search with frame times (host float32 [T] or None) and pointing jitter (host float32
+    [T, 2] px or None) in the track."""
     assert frames.is_cuda and frames.dtype.is_floating_point and frames.element_size() == 4
     assert frames.is_contiguous() and frames.dim() == 3
     T, H, W = frames.shape
     sig = np.ascontiguousarray(sigma_t, dtype=np.float32)
     if sig.shape != (T,):
         raise ValueError("sigma_t must have shape [T]")
+    tm = jt = None
+    if frame_times is not None:
+        tm = np.ascontiguousarray(frame_times, dtype=np.float32)
+        if tm.shape != (T,):
+            raise ValueError("frame_times must have shape [T]")
+    if jitter_xy is not None:
+        jt = np.ascontiguousarray(jitter_xy, dtype=np.float32)
+        if jt.shape != (T, 2):
+            raise ValueError("jitter_xy must have shape [T, 2]")
     tr = _traj_array(trajectories)
     n = tr.shape[0]
     p_snr = None
@@ -132,8 +151,15 @@ def tno_mf_search(ctx, frames, sigma_t, trajectories, prf_sigma: float, t0: floa
     if out_topk is not None:
         assert out_topk.is_cuda and out_topk.is_contiguous()
         p_top = out_topk.data_ptr()
-    _check(_lib.tno_mf_search(ctx, frames.data_ptr(), T, H, W, sig.ctypes.data, tr.ctypes.data, n,
-                              float(prf_sigma), float(t0), p_snr, p_top), ctx)
+    if _plain:
+        rc = _lib.tno_mf_search(ctx, frames.data_ptr(), T, H, W, sig.ctypes.data, tr.ctypes.data, n,
+                                float(prf_sigma), float(t0), p_snr, p_top)
+    else:
+        rc = _lib.tno_mf_search_ex(ctx, frames.data_ptr(), T, H, W, sig.ctypes.data,
+                                   tm.ctypes.data if tm is not None else None,
+                                   jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,
+                                   float(prf_sigma), float(t0), p_snr, p_top)
+    _check(rc, ctx)
 
 
 def tno_mf_best(ctx, snr, box: int, out_max, out_argk=None, out_z=None, out_topk=None) -> None:

@@ -230,7 +230,7 @@ int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, floa
             !finite_f(trajectories[k].ax) || !finite_f(trajectories[k].ay))
             return TNO_MF_EINVAL;
     Plan plan;
-    const int rc = build_classes(trajectories, n_traj, T, (double)t0, &plan);
+    const int rc = build_classes(trajectories, n_traj, T, (double)t0, nullptr, nullptr, &plan);
     if (rc != TNO_MF_OK) return rc;
     build_batches(&plan, max_entries, max_spread);
     for (size_t b = 0; b < plan.batches.size(); ++b)
@@ -321,6 +321,14 @@ int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
 int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
                   const float *sigma_t, const tno_mf_traj *trajectories, int32_t n_traj,
                   float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
+    return tno_mf_search_ex(ctx, frames, T, H, W, sigma_t, nullptr, nullptr, trajectories, n_traj, prf_sigma, t0,
+                            out_snr, out_topk);
+}
+
+int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
+                     const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                     const tno_mf_traj *trajectories, int32_t n_traj,
+                     float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
     ctx->ev_used = 0;
@@ -345,12 +353,18 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
         if (!finite_f(trajectories[k].vx) || !finite_f(trajectories[k].vy) ||
             !finite_f(trajectories[k].ax) || !finite_f(trajectories[k].ay))
             return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: trajectory %d has a non-finite value", k);
+    for (int32_t t = 0; t < T; ++t) {
+        if (frame_times && !finite_f(frame_times[t]))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: frame_times[%d] is not finite", t);
+        if (jitter_xy && (!finite_f(jitter_xy[2 * t]) || !finite_f(jitter_xy[2 * t + 1])))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: jitter_xy[%d] is not finite", t);
+    }
     CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t st = ctx->stream;
 
     // ------------------------------------------------------------------ planning (host)
     Plan plan;
-    if (build_classes(trajectories, n_traj, T, (double)t0, &plan) != TNO_MF_OK)
+    if (build_classes(trajectories, n_traj, T, (double)t0, frame_times, jitter_xy, &plan) != TNO_MF_OK)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: a trajectory displacement exceeds 1e9 px");
     const int32_t n_x = (int32_t)plan.xcls.size(), n_y = (int32_t)plan.ycls.size();
     const int32_t n_cls = n_x + n_y;
@@ -453,6 +467,8 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
     const size_t o_ti = blob.add(tinfo.data(), tinfo.size() * sizeof(TrajInfo));
     const size_t o_bx = blob.add(batch_xc.data(), batch_xc.size() * 4);
     const size_t o_by = blob.add(batch_yc.data(), batch_yc.size() * 4);
+    const size_t o_tm = blob.add(frame_times, frame_times ? (size_t)T * 4 : 0);
+    const size_t o_jt = blob.add(jitter_xy, jitter_xy ? (size_t)T * 8 : 0);
     const size_t o_bq = blob.add(batch_q.data(), batch_q.size() * 4);
     const size_t o_perm = blob.add(perm.data(), perm.size() * 4);
 
@@ -516,7 +532,9 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
 
     // ------------------------------------------------------------------ table kernels
     launch_class_tables(st, reinterpret_cast<const float *>(meta + o_v), reinterpret_cast<const float *>(meta + o_a),
-                        n_cls, T, (double)t0, (double)prf_sigma, static_cast<int32_t *>(ctx->shift.p),
+                        frame_times ? reinterpret_cast<const float *>(meta + o_tm) : nullptr,
+                        jitter_xy ? reinterpret_cast<const float *>(meta + o_jt) : nullptr,
+                        n_cls, n_x, T, (double)t0, (double)prf_sigma, static_cast<int32_t *>(ctx->shift.p),
                         static_cast<float *>(ctx->g.p), static_cast<double *>(ctx->gd.p));
     launch_border_tables(st, tab.shift, tab.gd, tab.qd, reinterpret_cast<const AxisBorder *>(meta + o_bd), d_off,
                          n_cls, n_x, max_n, T, W, H, static_cast<double *>(ctx->ab.p));

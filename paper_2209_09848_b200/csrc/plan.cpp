@@ -10,11 +10,12 @@
 
 namespace tno {
 
-bool axis_shift(double v, double a, double dt, int32_t *shift) {
-    volatile double p1 = v * dt;          // volatile: keep the products separately rounded
-    volatile double dt2 = dt * dt;
-    volatile double p2 = a * dt2;
-    const double d = p1 + p2;
+bool axis_shift(double v, double a, double dt, double j, int32_t *shift) {
+    volatile double p1 = v * dt;          // volatile: keep the operations separately rounded, in the
+    volatile double adt = a * dt;         // order the device (tables.cu) and the oracle use
+    volatile double p2 = adt * dt;
+    volatile double d0 = p1 + p2;
+    const double d = d0 + j;
     const double f = std::floor(d + 0.5);
     if (!(std::fabs(f) < 1.0e9)) return false;
     *shift = (int32_t)f;
@@ -30,7 +31,7 @@ static uint64_t key_of(float v, float a) {
 }
 
 static int class_of(std::map<uint64_t, int32_t> &index, std::vector<AxisClass> &cls, float v, float a,
-                    int32_t T, double t0, bool *ok) {
+                    int32_t T, double t0, const float *times, const float *jitter, int axis, bool *ok) {
     const uint64_t key = key_of(v, a);
     auto it = index.find(key);
     if (it != index.end()) return it->second;
@@ -40,7 +41,9 @@ static int class_of(std::map<uint64_t, int32_t> &index, std::vector<AxisClass> &
     c.smin = INT32_MAX; c.smax = INT32_MIN;
     for (int32_t t = 0; t < T; ++t) {
         int32_t s = 0;
-        if (!axis_shift((double)v, (double)a, (double)t - t0, &s)) { *ok = false; s = 0; }
+        const double dt = (times ? (double)times[t] : (double)t) - t0;
+        const double j = jitter ? (double)jitter[2 * t + axis] : 0.0;
+        if (!axis_shift((double)v, (double)a, dt, j, &s)) { *ok = false; s = 0; }
         c.shift[t] = s;
         c.smin = std::min(c.smin, s);
         c.smax = std::max(c.smax, s);
@@ -51,7 +54,8 @@ static int class_of(std::map<uint64_t, int32_t> &index, std::vector<AxisClass> &
     return id;
 }
 
-int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0, Plan *plan) {
+int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0, const float *frame_times,
+                  const float *jitter_xy, Plan *plan) {
     plan->T = T;
     plan->t0 = t0;
     plan->xcls.clear(); plan->ycls.clear();
@@ -60,8 +64,8 @@ int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0,
     std::map<uint64_t, int32_t> xi, yi;
     bool ok = true;
     for (int32_t k = 0; k < n_traj; ++k) {
-        plan->traj_xc[k] = class_of(xi, plan->xcls, traj[k].vx, traj[k].ax, T, t0, &ok);
-        plan->traj_yc[k] = class_of(yi, plan->ycls, traj[k].vy, traj[k].ay, T, t0, &ok);
+        plan->traj_xc[k] = class_of(xi, plan->xcls, traj[k].vx, traj[k].ax, T, t0, frame_times, jitter_xy, 0, &ok);
+        plan->traj_yc[k] = class_of(yi, plan->ycls, traj[k].vy, traj[k].ay, T, t0, frame_times, jitter_xy, 1, &ok);
     }
     return ok ? TNO_MF_OK : TNO_MF_EINVAL;
 }

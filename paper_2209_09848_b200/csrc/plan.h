@@ -13,10 +13,10 @@
 
 namespace tno {
 
-// floor(d + 1/2) of d = v*dt + a*dt*dt, all in IEEE double without contraction
+// floor(d + 1/2) of d = (v*dt + (a*dt)*dt) + j, all in IEEE double without contraction
 // (BASELINE.json:north_star "5x5 window at round(c_t)"; reading c1 in DESIGN.md: ties go up).
 // Returns false if the shift does not fit comfortably in 32 bits.
-bool axis_shift(double v, double a, double dt, int32_t *shift);
+bool axis_shift(double v, double a, double dt, double j, int32_t *shift);
 
 struct AxisClass {
     float v, a;                  // px/frame, px/frame^2 (exact float32 values of the ABI)
@@ -39,7 +39,10 @@ struct Plan {
 };
 
 // Group trajectories into axis classes.  Returns TNO_MF_OK or TNO_MF_EINVAL (shift overflow).
-int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0, Plan *plan);
+// frame_times (HOST [T], NULL = the frame index) and jitter_xy (HOST [T][2] px, NULL = none) enter the
+// displacement of every class: c_t = (x, y) + v (tau_t - t0) + a (tau_t - t0)^2 + j_t.
+int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0, const float *frame_times,
+                  const float *jitter_xy, Plan *plan);
 
 // Pack the trajectories of each x-class into batches of at most max_entries entries whose integer
 // y-shifts never differ by more than max_spread in any frame.  Entries are ordered by (vy, ay) so

@@ -10,16 +10,19 @@
 namespace tno {
 
 __global__ void k_class_tables(const float *__restrict__ cls_v, const float *__restrict__ cls_a,
-                               int32_t n_cls, int32_t T, double t0, double prf_sigma,
+                               const float *__restrict__ times, const float *__restrict__ jitter,
+                               int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma,
                                int32_t *__restrict__ shift, float *__restrict__ g,
                                double *__restrict__ gd) {
     const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (id >= (int64_t)n_cls * T) return;
     const int32_t c = (int32_t)(id / T), t = (int32_t)(id % T);
     const double v = (double)cls_v[c], a = (double)cls_a[c];
-    const double dt = (double)t - t0;
-    // d = v*dt + a*dt*dt evaluated left to right, every operation separately rounded
-    const double d = __dadd_rn(__dmul_rn(v, dt), __dmul_rn(__dmul_rn(a, dt), dt));
+    // tau_t (default t) and the pointing jitter of the class's axis (default 0): PAPER.md L106, L116
+    const double dt = __dsub_rn(times ? (double)times[t] : (double)t, t0);
+    const double j = jitter ? (double)jitter[2 * t + (c < n_x ? 0 : 1)] : 0.0;
+    // d = (v*dt + (a*dt)*dt) + j evaluated left to right, every operation separately rounded
+    const double d = __dadd_rn(__dadd_rn(__dmul_rn(v, dt), __dmul_rn(__dmul_rn(a, dt), dt)), j);
     const double f = floor(__dadd_rn(d, 0.5));
     const double ph = __dsub_rn(d, f);
     shift[id] = (int32_t)f;
@@ -70,12 +73,12 @@ __global__ void k_rsd_tables(const TrajInfo *__restrict__ traj, const double *__
     rsd[ti.rsd_off + id] = (D > 0.0) ? (float)(1.0 / sqrt(D)) : 0.0f;
 }
 
-void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a, int32_t n_cls,
-                         int32_t T, double t0, double prf_sigma, int32_t *shift, float *g,
-                         double *gd) {
+void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a, const float *times,
+                         const float *jitter, int32_t n_cls, int32_t n_x, int32_t T, double t0,
+                         double prf_sigma, int32_t *shift, float *g, double *gd) {
     const int64_t n = (int64_t)n_cls * T;
-    k_class_tables<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cls_v, cls_a, n_cls, T, t0,
-                                                                 prf_sigma, shift, g, gd);
+    k_class_tables<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cls_v, cls_a, times, jitter, n_cls, n_x, T,
+                                                                 t0, prf_sigma, shift, g, gd);
 }
 
 void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,

@@ -40,8 +40,9 @@ class MatchedFilter:
             pass
 
     def search(self, frames, sigma_t, trajectories, prf_sigma: float, t0: float,
-               want_maps: bool = True, out_snr=None, out_topk=None):
-        """Returns (snr maps tensor [n, H, W] or None, candidate tensor or None); asynchronous."""
+               want_maps: bool = True, out_snr=None, out_topk=None, frame_times=None, jitter_xy=None):
+        """Returns (snr maps tensor [n, H, W] or None, candidate tensor or None); asynchronous.
+        frame_times [T] / jitter_xy [T, 2] (host, optional) go through tno_mf_search_ex."""
         torch = self._torch
         n = np.asarray(trajectories).shape[0]
         T, H, W = frames.shape
@@ -49,8 +50,12 @@ class MatchedFilter:
             out_snr = torch.empty((n, H, W), dtype=torch.float32, device=frames.device)
         if self.topk > 0 and out_topk is None:
             out_topk = torch.empty((n, self.topk, 4), dtype=torch.int32, device=frames.device)
-        B.tno_mf_search(self.ctx, frames, sigma_t, trajectories, prf_sigma, t0,
-                        out_snr if want_maps else None, out_topk if self.topk > 0 else None)
+        if frame_times is None and jitter_xy is None:
+            B.tno_mf_search(self.ctx, frames, sigma_t, trajectories, prf_sigma, t0,
+                            out_snr if want_maps else None, out_topk if self.topk > 0 else None)
+        else:
+            B.tno_mf_search_ex(self.ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma, t0,
+                               out_snr if want_maps else None, out_topk if self.topk > 0 else None)
         return (out_snr if want_maps else None), (out_topk if self.topk > 0 else None)
 
     def best(self, snr, box: int = 255):
