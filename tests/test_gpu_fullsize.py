@@ -94,6 +94,21 @@ def _fullsize_with_maps(cfg, n_crop_traj, n_random):
     for i in range(len(p.src_k)):
         s = float(maps[int(p.src_k[i]), int(p.src_y[i]), int(p.src_x[i])])
         assert s > 0.5 * float(p.src_amp[i]) * np.sqrt(cfg.T * np.pi) / 1.2
+    # the paper's section 3.3 scoring at full size (max over the bank, units of the local sigma, box 255)
+    if cfg.idx == 3:
+        mx, ak, z, top = mf.best(maps, 255)
+        torch.cuda.synchronize()
+        g = maps.cpu().numpy()
+        om, oa = oracle.best(g)
+        assert np.array_equal(mx.cpu().numpy(), om) and np.array_equal(ak.cpu().numpy(), oa)
+        oz, _ = oracle.local_z(om, 255)
+        gz = z.cpu().numpy()
+        assert np.all(np.abs(gz.astype(np.float64) - oz) <= 2e-6 * np.maximum(1.0, np.abs(oz)))
+        ct = mf.candidates_to_numpy(top[None])[0]
+        ref = oracle.topk(gz.astype(np.float64), cfg.topk, cfg.threshold, 0)
+        assert np.array_equal(ct["x"], ref["x"]) and np.array_equal(ct["y"], ref["y"])
+        n = int(np.count_nonzero(ct["x"] >= 0))
+        assert np.array_equal(ct["k"][:n], oa[ct["y"][:n], ct["x"][:n]])
     mf.close()
 
 
