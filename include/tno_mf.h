@@ -147,6 +147,16 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
 int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, int32_t box,
                 float *out_max, int32_t *out_argk, float *out_z, tno_mf_cand *out_topk);
 
+/* Flux estimate (the score "is a direct estimate of the total flux due to that moving
+ * object, which allows to not only estimate the position and trajectory of a detection, but also the
+ * magnitude"): the maximum-likelihood amplitude of a source on trajectory k starting at (x, y),
+ *     A_k(x, y) = N / D = SNR_k(x, y) / sqrt(D_k(x, y)),        0 where D = 0,
+ * in the flux units of the frames, from the SNR maps and the D tables of the LAST tno_mf_search(_ex) on
+ * this context (same n_traj, H, W; the tables stay valid until the next search).
+ *   snr       DEVICE float32 [n_traj][H][W] as written by that search.   out_flux  DEVICE, same shape.
+ * Errors: EINVAL (NULL pointers, no matching preceding search), ECUDA. */
+int tno_mf_flux(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, float *out_flux);
+
 /* Host-only planning query (no device work; ctx may be NULL): how the search would group
  * `trajectories` into batches that share one x-motion (vx, ax) -- the unit of work of the
  * separable kernel.  Writes, for each trajectory, its batch index and slot

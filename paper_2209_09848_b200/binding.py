@@ -52,6 +52,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_search.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_search_ex.restype = ctypes.c_int
     lib.tno_mf_search_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_flux.restype = ctypes.c_int
+    lib.tno_mf_flux.argtypes = [vp, vp, i32, i32, i32, vp]
     lib.tno_mf_best.restype = ctypes.c_int
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
@@ -160,6 +162,14 @@ def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories,
                                    jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,
                                    float(prf_sigma), float(t0), p_snr, p_top)
     _check(rc, ctx)
+
+
+def tno_mf_flux(ctx, snr, out_flux) -> None:
+    """snr, out_flux: CUDA float32 tensors [n, H, W]; flux estimate N / D of the last search's maps."""
+    assert snr.is_cuda and snr.is_contiguous() and snr.dim() == 3 and snr.element_size() == 4
+    assert out_flux.is_cuda and out_flux.is_contiguous() and out_flux.shape == snr.shape
+    n, H, W = snr.shape
+    _check(_lib.tno_mf_flux(ctx, snr.data_ptr(), n, H, W, out_flux.data_ptr()), ctx)
 
 
 def tno_mf_best(ctx, snr, box: int, out_max, out_argk=None, out_z=None, out_topk=None) -> None:

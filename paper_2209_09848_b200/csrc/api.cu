@@ -30,6 +30,9 @@ struct tno_mf_ctx {
     void *encode_fn = nullptr;
     std::string err;
     int32_t last_launches = 0, last_kernel = 0;
+    // geometry and tables of the last successful search (for tno_mf_flux)
+    int32_t s_traj = 0, s_H = 0, s_W = 0;
+    const TrajInfo *s_ti = nullptr;
     double last_fma_x = 0.0, last_fma_y = 0.0;
     std::vector<cudaEvent_t> ev;      // pairs (before, after) around each main search kernel launch
     int32_t ev_used = 0;              // events recorded by the last search
@@ -325,12 +328,26 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
                             out_snr, out_topk);
 }
 
+int tno_mf_flux(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, float *out_flux) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (!snr || !out_flux) return fail(ctx, TNO_MF_EINVAL, "tno_mf_flux: NULL snr or out_flux");
+    if (!ctx->s_ti || n_traj != ctx->s_traj || H != ctx->s_H || W != ctx->s_W)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_flux: no preceding search with n_traj = %d, H = %d, W = %d on this "
+                    "context", n_traj, H, W);
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    launch_flux(ctx->stream, snr, ctx->s_ti, static_cast<const float *>(ctx->rsd.p), n_traj, H, W, out_flux);
+    ctx->last_launches = 1;
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
+}
+
 int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
                      const float *sigma_t, const float *frame_times, const float *jitter_xy,
                      const tno_mf_traj *trajectories, int32_t n_traj,
                      float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
+    ctx->s_ti = nullptr;
     ctx->ev_used = 0;
     // ------------------------------------------------------------------ validation
     if (!frames || !sigma_t || !trajectories)
@@ -622,6 +639,8 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
         ctx->last_launches += 1;
         CU_TRY(ctx, cudaGetLastError());
     }
+    ctx->s_traj = n_traj; ctx->s_H = H; ctx->s_W = W;
+    ctx->s_ti = d_ti;
     return TNO_MF_OK;
 }
 

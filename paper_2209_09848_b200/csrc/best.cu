@@ -136,6 +136,27 @@ __global__ void k_set_argk(tno_mf_cand *__restrict__ cand, int32_t n, const int3
     cand[i] = c;
 }
 
+// Flux estimate A = N / D = SNR * D^(-1/2) per trajectory and start pixel (the score "is a
+// direct estimate of the total flux due to that moving object ... but also the magnitude"), from the SNR
+// maps and the D^(-1/2) tables of the search that produced them.
+__global__ void __launch_bounds__(256)
+k_flux(const float *__restrict__ snr, const TrajInfo *__restrict__ traj, const float *__restrict__ rsd,
+       int32_t H, int32_t W, float *__restrict__ out) {
+    const int32_t x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
+    const int32_t k = blockIdx.z;
+    if (x >= W || y >= H) return;
+    const TrajInfo ti = traj[k];
+    const float r = __ldg(rsd + ti.rsd_off + (int64_t)border_class(y, ti.by, H) * ti.bx.n + border_class(x, ti.bx, W));
+    const int64_t i = ((int64_t)k * H + y) * W + x;
+    out[i] = snr[i] * r;
+}
+
+void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const float *rsd, int32_t K, int32_t H,
+                 int32_t W, float *out) {
+    dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)K);
+    k_flux<<<grid, 256, 0, st>>>(snr, traj, rsd, H, W, out);
+}
+
 void launch_max_map(cudaStream_t st, const float *snr, int32_t K, int32_t H, int32_t W, float *out_max,
                     int32_t *out_argk, int32_t n_sm) {
     k_max_map<<<(unsigned)(n_sm * 8), 256, 0, st>>>(snr, K, (int64_t)H * W, out_max, out_argk);

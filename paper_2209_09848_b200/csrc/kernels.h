@@ -39,6 +39,9 @@ void launch_max_map(cudaStream_t st, const float *snr, int32_t K, int32_t H, int
                     int32_t *out_argk /* may be NULL */, int32_t n_sm);
 // sat_ws: H*W*16 bytes of workspace (float64 summed-area tables of M and M^2)
 void launch_local_z(cudaStream_t st, const float *m, int32_t H, int32_t W, int32_t box, void *sat_ws, float *z);
+// out[k][y][x] = snr[k][y][x] * D_k(x, y)^(-1/2)  (flux estimate N / D)
+void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const float *rsd, int32_t K, int32_t H,
+                 int32_t W, float *out);
 void launch_set_argk(cudaStream_t st, tno_mf_cand *cand, int32_t n, const int32_t *argk, int32_t W);
 
 // ---- inject.cu ----

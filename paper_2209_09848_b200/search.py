@@ -58,6 +58,12 @@ class MatchedFilter:
                                out_snr if want_maps else None, out_topk if self.topk > 0 else None)
         return (out_snr if want_maps else None), (out_topk if self.topk > 0 else None)
 
+    def flux(self, snr):
+        """Flux estimate N / D of the maps of the last search on this context."""
+        out = self._torch.empty_like(snr)
+        B.tno_mf_flux(self.ctx, snr, out)
+        return out
+
     def best(self, snr, box: int = 255):
         """PAPER.md section 3.3 on SNR maps [n, H, W]: (max over trajectories, arg-max trajectory, Z =
         max / local sigma of the box, top-K records of Z or None); asynchronous."""

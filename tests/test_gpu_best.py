@@ -85,3 +85,34 @@ def test_best_on_a_search_result_and_errors():
         assert np.array_equal(c["x"], ref["x"]) and np.array_equal(c["y"], ref["y"])
         with pytest.raises(TnoMfError):
             tno_mf_best(mf.ctx, maps, 254, mx)                               # even box
+
+
+def test_flux_estimate_matches_oracle_n_over_d():
+    """tno_mf_flux: A = N / D, from the maps and D tables of the preceding search."""
+    torch = _torch()
+    from paper_2209_09848_b200 import MatchedFilter, TnoMfError, tno_mf_flux
+    T, H, W = 50, 96, 128
+    rng = np.random.default_rng(21)
+    f = rng.standard_normal((T, H, W)).astype(np.float32)
+    sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
+    traj = np.array([[0.2, -0.1, 0, 0], [0.2, 0.3, 0, 0.002], [-0.6, 0.0, 0, 0], [0.0, 0.0, 0, 0]], np.float32)
+    amp = 2.25
+    oracle.inject(f, traj[1:2], [70], [40], [amp], 1.0, 25.0)
+    _, oN, oD = oracle.snr_map(f, sigma, traj, 1.0, 25.0, return_ND=True)
+    ref = np.where(oD > 0, oN / np.where(oD > 0, oD, 1.0), 0.0)
+    with MatchedFilter(0, 0) as mf:
+        with pytest.raises(TnoMfError):                                   # no search yet on this context
+            tno_mf_flux(mf.ctx, torch.zeros((4, H, W), device="cuda"), torch.zeros((4, H, W), device="cuda"))
+        maps, _ = mf.search(torch.from_numpy(f).cuda(), sigma, traj, 1.0, 25.0)
+        fl = mf.flux(maps)
+        torch.cuda.synchronize()
+        g = fl.cpu().numpy().astype(np.float64)
+        with pytest.raises(TnoMfError):                                   # shape of another search
+            tno_mf_flux(mf.ctx, maps[:2].contiguous(), fl[:2].contiguous())
+    # |dSNR| <= 1e-3 scaled by D^(-1/2), plus float32 rounding of the product
+    tol = 1e-3 / np.sqrt(np.where(oD > 0, oD, 1.0)) + 4e-7 * np.abs(ref)
+    assert np.all(np.abs(g - ref) <= tol)
+    # the injected amplitude is recovered at the source (noise: sigma_A = D^(-1/2))
+    assert abs(g[1, 40, 70] - amp) <= 5.0 / np.sqrt(oD[1, 40, 70])
+    # corner pixels, where D is clipped: still N / D
+    assert g[2, 0, 0] == pytest.approx(ref[2, 0, 0], abs=float(tol[2, 0, 0]))
