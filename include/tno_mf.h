@@ -92,7 +92,11 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
  * trajectory or t0 values, both outputs absent, shapes whose shifts do not fit 32-bit pixel
  * arithmetic), ENOMEM, ECUDA.
  * Any H, W >= 1 is computed correctly; the TMA kernel needs W % 4 == 0 and 16-byte aligned
- * frames, other shapes take the generic kernel.  All element offsets are 64-bit. */
+ * frames (and y-shift ranges below 63 tile heights of 60 px), other inputs take the generic kernel.
+ * The TMA kernel accumulates into a context-owned partial-sum workspace of (1 + ceil(y-shift range /
+ * 60)) * n_traj * H * W floats, capped (cfg.workspace_limit_mb); a larger bank is searched in chunks
+ * of whole batches with identical results.  Results are bitwise reproducible, and the map of a
+ * trajectory does not depend on the other trajectories of the call.  All element offsets are 64-bit. */
 int tno_mf_search(tno_mf_ctx *ctx,
                   const float *frames, int32_t T, int32_t H, int32_t W,
                   const float *sigma_t,
@@ -162,7 +166,9 @@ int tno_mf_flux(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
  * separable kernel.  Writes, for each trajectory, its batch index and slot
  * within the batch to out_batch[n_traj] / out_slot[n_traj] (either may be NULL) and returns the
  * number of batches (>= 1), or a negative error.  max_entries: slots per batch (1..16);
- * max_spread: largest allowed difference of integer y-shifts inside a batch at any frame. */
+ * max_spread: largest allowed difference of integer y-shifts inside a batch at any frame; a value
+ * >= 2^30 means no limit and an even split of each x-motion into the fewest batches -- that is how
+ * tno_mf_search itself batches (with max_entries = 8 or 10, whichever costs less). */
 int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, float t0,
                 int32_t max_entries, int32_t max_spread,
                 int32_t *out_batch, int32_t *out_slot);
