@@ -63,6 +63,12 @@ static inline double disp(double v, double a, double dt) { return v * dt + a * d
  * spaced ("the time-jump that occurs when TESS is transmitting frames to Earth", L116).
  *     c_t = (x, y) + v (tau_t - t0) + a (tau_t - t0)^2 + j_t
  * times == NULL: tau_t = t;  jitter == NULL: j_t = 0;  jitter[2t], jitter[2t+1] = (jx_t, jy_t) in px. */
+/* Per-pixel validity / inverse-variance weights (readings h1-h3; "We set the
+ * value of bright pixels to 0 because the noise in those pixels will so high"): with valid != NULL
+ *     N = sum g F_t(p) / sigma_t^2          (the frames F as they are: the caller has zeroed or
+ *                                            down-weighted them, F = R * valid)
+ *     D = sum g^2 valid_t(p) / sigma_t^2    (a masked pixel carries no information)
+ * valid has the layout of the frames (same window); NULL = all ones. */
 static inline double frame_dt(const float *times, int t, double t0) {
     return (times ? (double)times[t] : (double)t) - t0;
 }
@@ -88,7 +94,7 @@ int tno_oracle_threads(void) {
 /* literal definition, one exp per tap */
 int tno_oracle_point_ex(const float *frames, int T, int H, int W,
                         int wx0, int wy0, int ww, int wh,
-                        const float *sigma_t, const float *times, const float *jitter,
+                        const float *sigma_t, const float *times, const float *jitter, const float *valid,
                         const float *traj4, float prf_sigma_f, float t0_f,
                         int x, int y, double *N_out, double *D_out, double *snr_out)
 {
@@ -109,9 +115,10 @@ int tno_oracle_point_ex(const float *frames, int T, int H, int W,
                 if (px < wx0 || px >= wx0 + ww || py < wy0 || py >= wy0 + wh) return -1;
                 const double ux = (double)i - phx, uy = (double)j - phy;
                 const double g = exp(-(ux * ux + uy * uy) / (2.0 * s * s));
-                const double R = frames[((size_t)t * wh + (size_t)(py - wy0)) * ww + (size_t)(px - wx0)];
+                const size_t idx = ((size_t)t * wh + (size_t)(py - wy0)) * ww + (size_t)(px - wx0);
+                const double R = frames[idx];
                 N += g * R * q;
-                D += g * g * q;
+                D += valid ? g * g * q * (double)valid[idx] : g * g * q;
             }
         }
     }
@@ -126,7 +133,7 @@ int tno_oracle_point(const float *frames, int T, int H, int W,
                      const float *sigma_t, const float *traj4, float prf_sigma_f, float t0_f,
                      int x, int y, double *N_out, double *D_out, double *snr_out)
 {
-    return tno_oracle_point_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, traj4,
+    return tno_oracle_point_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, NULL, traj4,
                                prf_sigma_f, t0_f, x, y, N_out, D_out, snr_out);
 }
 
@@ -135,7 +142,7 @@ int tno_oracle_point(const float *frames, int T, int H, int W,
  * out_snr / out_N / out_D: double [K][y_hi-y_lo][x_hi-x_lo]; out_N, out_D may be NULL. */
 int tno_oracle_map_ex(const float *frames, int T, int H, int W,
                       int wx0, int wy0, int ww, int wh,
-                      const float *sigma_t, const float *times, const float *jitter,
+                      const float *sigma_t, const float *times, const float *jitter, const float *valid,
                       const float *traj, int K,
                       float prf_sigma_f, float t0_f,
                       int x_lo, int x_hi, int y_lo, int y_hi,
@@ -181,6 +188,7 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
                     if (py < 0 || py >= H) continue;
                     if (py < wy0 || py >= wy0 + wh) { err = -1; continue; }
                     const float *row = frames + ((size_t)t * wh + (size_t)(py - wy0)) * ww;
+                    const float *vrow = valid ? valid + ((size_t)t * wh + (size_t)(py - wy0)) * ww : NULL;
                     for (int i = -2; i <= 2; ++i) {
                         const double g = gx[i + 2] * gy[j + 2];
                         const double wN = g * q, wD = g * g * q;
@@ -190,9 +198,10 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
                         if (xa >= xb) continue;
                         if (xa + sx + i < wx0 || xb + sx + i > wx0 + ww) { err = -1; continue; }
                         const float *src = row + (sx + i - wx0);
+                        const float *vsrc = vrow ? vrow + (sx + i - wx0) : NULL;
                         for (int x = xa; x < xb; ++x) {
                             Nr[x - x_lo] += wN * (double)src[x];
-                            Dr[x - x_lo] += wD;
+                            Dr[x - x_lo] += vsrc ? wD * (double)vsrc[x] : wD;
                         }
                     }
                 }
@@ -218,7 +227,7 @@ int tno_oracle_map(const float *frames, int T, int H, int W,
                    int x_lo, int x_hi, int y_lo, int y_hi,
                    double *out_snr, double *out_N, double *out_D)
 {
-    return tno_oracle_map_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, traj, K,
+    return tno_oracle_map_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, NULL, traj, K,
                              prf_sigma_f, t0_f, x_lo, x_hi, y_lo, y_hi, out_snr, out_N, out_D);
 }
 
