@@ -122,6 +122,26 @@ int tno_mf_search_ex(tno_mf_ctx *ctx,
                      float *out_snr,
                      tno_mf_cand *out_topk);
 
+/* The search with per-pixel validity weights.  The paper sets bright pixels to 0 before filtering
+ * ("the noise in those pixels will so high to make it impossible to detect a magnitude 20+ signal",
+ * PAPER.md:L106) and keeps the normalisation of the full filter; here a masked pixel also leaves the
+ * normalisation, which keeps the score in units of sigma next to masked stars:
+ *     N = sum_t sum_p g(p - c_t) F_t(p) / sigma_t^2          F = frames AS GIVEN: the caller has zeroed
+ *                                                            (or down-weighted) them, F = R * valid
+ *     D = sum_t sum_p g(p - c_t)^2 valid_t(p) / sigma_t^2    SNR = N / sqrt(D), 0 where D = 0
+ *   valid   DEVICE float32 [T][H][W], finite and >= 0: 1 = use, 0 = masked; other values act as relative
+ *           inverse variances of the pixels.  Read only.  NULL = tno_mf_search_ex.
+ * D is accumulated by a second pass of the same kernel over `valid` with squared taps: twice the time
+ * and twice the workspace of tno_mf_search.  tno_mf_flux does not apply to a masked search (EINVAL).
+ * Everything else as tno_mf_search_ex. */
+int tno_mf_search_masked(tno_mf_ctx *ctx,
+                         const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                         const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                         const tno_mf_traj *trajectories, int32_t n_traj,
+                         float prf_sigma, float t0,
+                         float *out_snr,
+                         tno_mf_cand *out_topk);
+
 /* Signal injection ("signal injection corresponds to adding a filter times a flux
  * to the raw data"): for each source m in order and every frame t,
  *     R_t(p) <- (float)((double)R_t(p) + amplitude_m * g(p - c_t))  on the 25 window taps,

@@ -52,6 +52,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_search.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_search_ex.restype = ctypes.c_int
     lib.tno_mf_search_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_search_masked.restype = ctypes.c_int
+    lib.tno_mf_search_masked.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_flux.restype = ctypes.c_int
     lib.tno_mf_flux.argtypes = [vp, vp, i32, i32, i32, vp]
     lib.tno_mf_best.restype = ctypes.c_int
@@ -123,8 +125,15 @@ def tno_mf_search(ctx, frames, sigma_t, trajectories, prf_sigma: float, t0: floa
                      _plain=True)
 
 
+def tno_mf_search_masked(ctx, frames, valid, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float,
+                         t0: float, out_snr=None, out_topk=None) -> None:
+    """tno_mf_search_ex with per-pixel validity weights (CUDA float32 tensor shaped like frames, or None)."""
+    tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma, t0, out_snr, out_topk,
+                     _valid=valid)
+
+
 def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
-                     out_snr=None, out_topk=None, _plain: bool = False) -> None:
+                     out_snr=None, out_topk=None, _plain: bool = False, _valid=None) -> None:
     """tno_mf_search with frame times (host float32 [T] or None) and pointing jitter (host float32
     [T, 2] px or None) in the track."""
     assert frames.is_cuda and frames.dtype.is_floating_point and frames.element_size() == 4
@@ -153,7 +162,14 @@ def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories,
     if out_topk is not None:
         assert out_topk.is_cuda and out_topk.is_contiguous()
         p_top = out_topk.data_ptr()
-    if _plain:
+    if _valid is not None:
+        assert _valid.is_cuda and _valid.is_contiguous() and _valid.shape == frames.shape
+        assert _valid.element_size() == 4 and _valid.dtype.is_floating_point
+        rc = _lib.tno_mf_search_masked(ctx, frames.data_ptr(), _valid.data_ptr(), T, H, W, sig.ctypes.data,
+                                       tm.ctypes.data if tm is not None else None,
+                                       jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,
+                                       float(prf_sigma), float(t0), p_snr, p_top)
+    elif _plain:
         rc = _lib.tno_mf_search(ctx, frames.data_ptr(), T, H, W, sig.ctypes.data, tr.ctypes.data, n,
                                 float(prf_sigma), float(t0), p_snr, p_top)
     else:

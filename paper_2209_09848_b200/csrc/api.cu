@@ -345,6 +345,14 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
                      const float *sigma_t, const float *frame_times, const float *jitter_xy,
                      const tno_mf_traj *trajectories, int32_t n_traj,
                      float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
+    return tno_mf_search_masked(ctx, frames, nullptr, T, H, W, sigma_t, frame_times, jitter_xy, trajectories, n_traj,
+                                prf_sigma, t0, out_snr, out_topk);
+}
+
+int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                         const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                         const tno_mf_traj *trajectories, int32_t n_traj,
+                         float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
     ctx->s_ti = nullptr;
@@ -390,8 +398,10 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
     // The separable kernel needs TMA-compatible frames (W % 4 == 0, 16-byte aligned) and a piece
     // count (1 + ceil(y-shift range / tile height)) that stays small.
     bool use_sep = !ctx->cfg.force_generic && (W % 4 == 0) &&
-                   ((reinterpret_cast<uintptr_t>(frames) & 15u) == 0) && W >= 4;
+                   ((reinterpret_cast<uintptr_t>(frames) & 15u) == 0) &&
+                   ((reinterpret_cast<uintptr_t>(valid) & 15u) == 0) && W >= 4;
     int32_t variant = -1, n_pieces = 1;
+    const int32_t n_pass = valid ? 2 : 1;             // masked search: a second pass accumulates D
     SepVariant sv = {0, 0};
     if (use_sep) {
         // variant = batch capacity; cost = x-pass per batch + y-pass per entry (FFMA per pixel), ties
@@ -509,8 +519,9 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
     const int64_t map_px = (int64_t)H * W;
     int64_t chunk_cap = n_traj;                            // entries per chunk
     if (use_sep) {
-        if ((rc = reserve(ctx, ctx->stage_tab, (size_t)n_batches * T * sep_table_words(variant) * 4))) return rc;
-        const size_t per_entry = (size_t)n_pieces * map_px * 4;
+        if ((rc = reserve(ctx, ctx->stage_tab, (size_t)n_pass * n_batches * T * sep_table_words(variant) * 4)))
+            return rc;
+        const size_t per_entry = (size_t)n_pass * n_pieces * map_px * 4;
         const size_t want = per_entry * n_traj;
         const size_t limit = ctx->cfg.workspace_limit_mb > 0 ? (size_t)ctx->cfg.workspace_limit_mb << 20
                                                              : (size_t)40 << 30;
@@ -568,10 +579,13 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
 
     // ------------------------------------------------------------------ search
     if (use_sep) {
-        launch_sep_tables(st, variant, tab, reinterpret_cast<const int32_t *>(meta + o_bx),
-                          reinterpret_cast<const int32_t *>(meta + o_by), n_batches,
-                          static_cast<float *>(ctx->stage_tab.p));
-        ctx->last_launches += 1;
+        const size_t tab_floats = (size_t)n_batches * T * sep_table_words(variant);
+        for (int32_t pass = 0; pass < n_pass; ++pass) {
+            launch_sep_tables(st, variant, tab, reinterpret_cast<const int32_t *>(meta + o_bx),
+                              reinterpret_cast<const int32_t *>(meta + o_by), n_batches, pass,
+                              static_cast<float *>(ctx->stage_tab.p) + pass * tab_floats);
+            ctx->last_launches += 1;
+        }
         CU_TRY(ctx, cudaGetLastError());
         const int32_t tabw = sep_table_words(variant);
         for (int32_t b0 = 0; b0 < n_batches;) {
@@ -588,17 +602,25 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
             a.piece_stride = (int64_t)qn * map_px;
             a.n_pieces = n_pieces;
             a.n_sm = ctx->n_sm;
-            CU_TRY(ctx, cudaMemsetAsync(a.pieces, 0, (size_t)n_pieces * a.piece_stride * 4, st));
-            int32_t grid = 0;
-            const char *err = "";
-            if ((rc = record_event(ctx))) return rc;
-            if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
-                return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
-            if ((rc = record_event(ctx))) return rc;
-            launch_finish(st, a.pieces, n_pieces, a.piece_stride, reinterpret_cast<const int32_t *>(meta + o_perm),
-                          q0, qn, d_ti, d_rsd, H, W, out_snr, slots);
+            const size_t pass_floats = (size_t)n_pieces * a.piece_stride;
+            CU_TRY(ctx, cudaMemsetAsync(a.pieces, 0, n_pass * pass_floats * 4, st));
+            for (int32_t pass = 0; pass < n_pass; ++pass) {
+                // pass 1 of a masked search: the same kernel over the validity weights with squared taps
+                a.frames = pass ? valid : frames;
+                a.stage_tab = static_cast<const float *>(ctx->stage_tab.p) + pass * tab_floats + (size_t)b0 * T * tabw;
+                a.pieces = static_cast<float *>(ctx->pieces.p) + pass * pass_floats;
+                int32_t grid = 0;
+                const char *err = "";
+                if ((rc = record_event(ctx))) return rc;
+                if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
+                    return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
+                if ((rc = record_event(ctx))) return rc;
+            }
+            const float *np_ = static_cast<const float *>(ctx->pieces.p);
+            launch_finish(st, np_, valid ? np_ + pass_floats : nullptr, n_pieces, a.piece_stride,
+                          reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W, out_snr, slots);
             CU_TRY(ctx, cudaGetLastError());
-            ctx->last_launches += 3;                       // memset, search, finish
+            ctx->last_launches += 2 + n_pass;              // memset, search(es), finish
             b0 = b1;
         }
         // work of the formulation: x-pass over the staged rows of every (tile, batch, frame),
@@ -606,8 +628,8 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
         double rows = 0.0;
         for (int32_t ty = 0; ty < sep_tile_rows(variant, H); ++ty)
             rows += (double)(std::min(sv.tile_h, H + 2 - (ty * sv.tile_h - 2)) + 4);
-        ctx->last_fma_x = 5.0 * rows * 64.0 * (double)((W + 63) / 64) * (double)n_batches * T;
-        ctx->last_fma_y = 5.0 * (double)n_traj * T * (double)H * W;
+        ctx->last_fma_x = n_pass * 5.0 * rows * 64.0 * (double)((W + 63) / 64) * (double)n_batches * T;
+        ctx->last_fma_y = n_pass * 5.0 * (double)n_traj * T * (double)H * W;
     } else {
         // generic path: maps are always materialised (caller's buffer, or a workspace chunk)
         int32_t chunk = n_traj;
@@ -619,12 +641,12 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
             maps = static_cast<float *>(ctx->tmp_maps.p);
         }
         ctx->last_fma_x = 0.0;
-        ctx->last_fma_y = 25.0 * (double)n_traj * T * (double)H * W;
+        ctx->last_fma_y = n_pass * 25.0 * (double)n_traj * T * (double)H * W;
         if ((rc = record_event(ctx))) return rc;
         for (int32_t k0 = 0; k0 < n_traj; k0 += chunk) {
             const int32_t kc = std::min(chunk, n_traj - k0);
             float *dst = out_snr ? out_snr + (int64_t)k0 * map_px : maps;
-            launch_search_generic(st, frames, T, H, W, tab, d_ti, d_rsd, k0, kc, dst);
+            launch_search_generic(st, frames, valid, T, H, W, tab, d_ti, d_rsd, k0, kc, dst);
             ctx->last_launches += 1;
             if (want_topk) {
                 launch_collect_from_map(st, dst, H, W, k0, kc, slots);
@@ -640,7 +662,7 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
         CU_TRY(ctx, cudaGetLastError());
     }
     ctx->s_traj = n_traj; ctx->s_H = H; ctx->s_W = W;
-    ctx->s_ti = d_ti;
+    ctx->s_ti = valid ? nullptr : d_ti;                // tno_mf_flux needs the analytic D tables
     return TNO_MF_OK;
 }
 

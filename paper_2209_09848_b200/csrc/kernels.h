@@ -20,7 +20,8 @@ void launch_rsd_tables(cudaStream_t st, const TrajInfo *traj, int32_t n_traj, in
 
 // ---- search_generic.cu ----
 // One thread per (trajectory, pixel); any H, W; maps only.
-void launch_search_generic(cudaStream_t st, const float *frames, int32_t T, int32_t H, int32_t W,
+// valid != NULL: D = sum g^2 valid / sigma^2 is accumulated next to N (masked search), rsd is not used
+void launch_search_generic(cudaStream_t st, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
                            const ClassTables &tab, const TrajInfo *traj, const float *rsd,
                            int32_t k_first, int32_t k_count, float *out_snr /* [k_count][H][W] */);
 
@@ -62,7 +63,7 @@ int32_t sep_table_words(int32_t v);
 int32_t sep_tile_rows(int32_t v, int32_t H);
 void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
                        const int32_t *batch_yc /* [n_batches][nb], -1 = empty */, int32_t n_batches,
-                       float *stage_tab);
+                       int32_t squared /* 1: taps g^2 (D pass of the masked search) */, float *stage_tab);
 struct SepArgs {
     const float *frames;
     int32_t T, H, W;
@@ -80,7 +81,8 @@ int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode
                       const char **err);
 // SNR = (sum of pieces) * D^(-1/2) for entries q0 .. q0 + q_count of the planned order (perm[q] =
 // trajectory); maps to out_snr (may be NULL), candidates to the 64 x 64 tile slots (keys may be NULL)
-void launch_finish(cudaStream_t st, const float *pieces, int32_t n_pieces, int64_t piece_stride,
+// dpieces != NULL (masked search): SNR = (sum of pieces) / sqrt(sum of dpieces), 0 where that is 0
+void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
                    int32_t H, int32_t W, float *out_snr, const TopkSlots &slots);
 

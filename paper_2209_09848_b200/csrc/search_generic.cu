@@ -9,7 +9,7 @@
 namespace tno {
 
 __global__ void __launch_bounds__(256)
-k_search_generic(const float *__restrict__ frames, int32_t T, int32_t H, int32_t W,
+k_search_generic(const float *__restrict__ frames, const float *__restrict__ valid, int32_t T, int32_t H, int32_t W,
                  ClassTables tab, const TrajInfo *__restrict__ traj, const float *__restrict__ rsd,
                  int32_t k_first, float *__restrict__ out_snr) {
     const int32_t x = blockIdx.x * 32 + threadIdx.x;
@@ -18,38 +18,49 @@ k_search_generic(const float *__restrict__ frames, int32_t T, int32_t H, int32_t
     if (x >= W || y >= H) return;
     const TrajInfo ti = traj[k];
     const int64_t cx0 = (int64_t)ti.xc * T, cy0 = (int64_t)(tab.n_x + ti.yc) * T;
-    double acc = 0.0;
+    double acc = 0.0, accd = 0.0;
     for (int32_t t = 0; t < T; ++t) {
         const int32_t px = x + tab.shift[cx0 + t] - 2, py = y + tab.shift[cy0 + t] - 2;
         const float *gx = tab.g + (cx0 + t) * 5, *gy = tab.g + (cy0 + t) * 5;
         const float *f = frames + (int64_t)t * H * W;
-        float p = 0.0f;
+        const float *vf = valid ? valid + (int64_t)t * H * W : nullptr;
+        float p = 0.0f, pd = 0.0f;
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
             const int32_t yy = py + j;
             if (yy < 0 || yy >= H) continue;
             const float *row = f + (int64_t)yy * W;
-            float r = 0.0f;
+            float r = 0.0f, rd = 0.0f;
 #pragma unroll
             for (int i = 0; i < 5; ++i) {
                 const int32_t xx = px + i;
-                if (xx >= 0 && xx < W) r = fmaf(gx[i], __ldg(row + xx), r);
+                if (xx >= 0 && xx < W) {
+                    r = fmaf(gx[i], __ldg(row + xx), r);
+                    if (vf) rd = fmaf(gx[i] * gx[i], __ldg(vf + (int64_t)yy * W + xx), rd);
+                }
             }
             p = fmaf(gy[j], r, p);
+            pd = fmaf(gy[j] * gy[j], rd, pd);
         }
         acc += (double)(p * tab.qf[t]);
+        accd += (double)(pd * tab.qf[t]);
     }
-    const int32_t cx = border_class(x, ti.bx, W), cy = border_class(y, ti.by, H);
-    const float s = (float)acc * rsd[ti.rsd_off + (int64_t)cy * ti.bx.n + cx];
+    float s;
+    if (valid) {
+        s = accd > 0.0 ? (float)(acc / sqrt(accd)) : 0.0f;
+    } else {
+        const int32_t cx = border_class(x, ti.bx, W), cy = border_class(y, ti.by, H);
+        s = (float)acc * rsd[ti.rsd_off + (int64_t)cy * ti.bx.n + cx];
+    }
     out_snr[((int64_t)kl * H + y) * W + x] = s;
 }
 
-void launch_search_generic(cudaStream_t st, const float *frames, int32_t T, int32_t H, int32_t W,
+void launch_search_generic(cudaStream_t st, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
                            const ClassTables &tab, const TrajInfo *traj, const float *rsd,
                            int32_t k_first, int32_t k_count, float *out_snr) {
     dim3 block(32, 8);
     dim3 grid((unsigned)((W + 31) / 32), (unsigned)((H + 7) / 8), (unsigned)k_count);
-    k_search_generic<<<grid, block, 0, st>>>(frames, T, H, W, tab, traj, rsd, k_first, out_snr);
+    k_search_generic<<<grid, block, 0, st>>>(frames, valid, T, H, W, tab, traj, rsd, k_first, out_snr);
 }
 
 }  // namespace tno

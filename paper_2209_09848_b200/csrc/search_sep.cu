@@ -136,7 +136,7 @@ __device__ __forceinline__ int32_t seg_phase(float v, float a) {
 // ------------------------------------------------------------------------------------ table kernel
 template <class C>
 __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_xc,
-                             const int32_t *__restrict__ batch_yc, int32_t n_batches,
+                             const int32_t *__restrict__ batch_yc, int32_t n_batches, int32_t squared,
                              float *__restrict__ stage_tab) {
     const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int32_t T = tab.T;
@@ -151,7 +151,11 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
     for (int i = 0; i < kHdr; ++i) outi[i] = 0;
     outi[0] = align4(sxm2);
     outi[1] = sxm2 - align4(sxm2);
-    for (int i = 0; i < 5; ++i) out[4 + i] = tab.g[((int64_t)xc * T + t) * 5 + i];
+    // squared = 1: the taps of the D pass over the validity weights, sum g^2 V / sigma^2
+    for (int i = 0; i < 5; ++i) {
+        const double gv = tab.gd[((int64_t)xc * T + t) * 5 + i];
+        out[4 + i] = squared ? (float)(gv * gv) : tab.g[((int64_t)xc * T + t) * 5 + i];
+    }
     int32_t n = 0, fmask = 0, fwait = 0;
     for (int e = 0; e < C::NB; ++e) {
         float *oe = out + kHdr + 8 * e;
@@ -161,7 +165,10 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
         n = e + 1;
         const int32_t c = tab.n_x + yc[e];
         const int64_t ci = (int64_t)c * T + t;
-        for (int j = 0; j < 5; ++j) oe[j] = (float)(tab.gd[ci * 5 + j] * tab.qd[t]);
+        for (int j = 0; j < 5; ++j) {
+            const double gv = tab.gd[ci * 5 + j];
+            oe[j] = (float)((squared ? gv * gv : gv) * tab.qd[t]);
+        }
         oi[5] = tab.shift[ci];
         // flush before the mapping position -> output row changes, once per kSeg frames, and after
         // the last frame
@@ -428,7 +435,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 // One block per (64 x 64 tile, entry q of the chunk): SNR = (sum of the pieces) * D^(-1/2), map
 // store, candidates >= threshold into the tile's slot (BASELINE.json:north_star a4, a5).
 __global__ void __launch_bounds__(256)
-k_finish(const float *__restrict__ pieces, int32_t n_pieces, int64_t piece_stride,
+k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, int32_t n_pieces, int64_t piece_stride,
          const int32_t *__restrict__ perm, int32_t q0, const TrajInfo *__restrict__ traj,
          const float *__restrict__ rsd, int32_t H, int32_t W, float *__restrict__ out_snr,
          TopkSlots slots) {
@@ -460,7 +467,19 @@ k_finish(const float *__restrict__ pieces, int32_t n_pieces, int64_t piece_strid
                 const float4 p = __ldcs(reinterpret_cast<const float4 *>(pin + c * piece_stride + off));
                 v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
             }
-            if (interior) {
+            if (dpieces) {
+                // masked search: D was accumulated like N, from the validity weights
+                float4 dsum = make_float4(0.f, 0.f, 0.f, 0.f);
+                const float *din = dpieces + (int64_t)ql * H * W;
+                for (int32_t c = 0; c < n_pieces; ++c) {
+                    const float4 p = __ldcs(reinterpret_cast<const float4 *>(din + c * piece_stride + off));
+                    dsum.x += p.x; dsum.y += p.y; dsum.z += p.z; dsum.w += p.w;
+                }
+                v.x = dsum.x > 0.f ? v.x / sqrtf(dsum.x) : 0.f;
+                v.y = dsum.y > 0.f ? v.y / sqrtf(dsum.y) : 0.f;
+                v.z = dsum.z > 0.f ? v.z / sqrtf(dsum.z) : 0.f;
+                v.w = dsum.w > 0.f ? v.w / sqrtf(dsum.w) : 0.f;
+            } else if (interior) {
                 v.x *= rs_in; v.y *= rs_in; v.z *= rs_in; v.w *= rs_in;
             } else {
                 const float *rr = rs + (int64_t)border_class(y, ti.by, H) * ti.bx.n;
@@ -502,11 +521,11 @@ int32_t sep_tile_rows(int32_t v, int32_t H) {
 }
 
 void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
-                       const int32_t *batch_yc, int32_t n_batches, float *stage_tab) {
+                       const int32_t *batch_yc, int32_t n_batches, int32_t squared, float *stage_tab) {
     const int64_t n = (int64_t)n_batches * tab.T;
     const unsigned grid = (unsigned)((n + 127) / 128);
-    if (v == 0) k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, batch_yc, n_batches, stage_tab);
-    else k_sep_tables<V1><<<grid, 128, 0, st>>>(tab, batch_xc, batch_yc, n_batches, stage_tab);
+    if (v == 0) k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, batch_yc, n_batches, squared, stage_tab);
+    else k_sep_tables<V1><<<grid, 128, 0, st>>>(tab, batch_xc, batch_yc, n_batches, squared, stage_tab);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
@@ -557,12 +576,12 @@ int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode
     return v == 0 ? launch_t<V0>(st, a, encode_fn, grid_out, err) : launch_t<V1>(st, a, encode_fn, grid_out, err);
 }
 
-void launch_finish(cudaStream_t st, const float *pieces, int32_t n_pieces, int64_t piece_stride,
+void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
                    int32_t H, int32_t W, float *out_snr, const TopkSlots &slots) {
     dim3 grid((unsigned)((W + kCollectTile - 1) / kCollectTile),
               (unsigned)((H + kCollectTile - 1) / kCollectTile), (unsigned)q_count);
-    k_finish<<<grid, 256, 0, st>>>(pieces, n_pieces, piece_stride, perm, q0, traj, rsd, H, W, out_snr, slots);
+    k_finish<<<grid, 256, 0, st>>>(pieces, dpieces, n_pieces, piece_stride, perm, q0, traj, rsd, H, W, out_snr, slots);
 }
 
 }  // namespace tno

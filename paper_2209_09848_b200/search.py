@@ -40,9 +40,11 @@ class MatchedFilter:
             pass
 
     def search(self, frames, sigma_t, trajectories, prf_sigma: float, t0: float,
-               want_maps: bool = True, out_snr=None, out_topk=None, frame_times=None, jitter_xy=None):
+               want_maps: bool = True, out_snr=None, out_topk=None, frame_times=None, jitter_xy=None,
+               valid=None):
         """Returns (snr maps tensor [n, H, W] or None, candidate tensor or None); asynchronous.
-        frame_times [T] / jitter_xy [T, 2] (host, optional) go through tno_mf_search_ex."""
+        frame_times [T] / jitter_xy [T, 2] (host, optional) go through tno_mf_search_ex; valid (CUDA
+        tensor shaped like frames, optional) through tno_mf_search_masked."""
         torch = self._torch
         n = np.asarray(trajectories).shape[0]
         T, H, W = frames.shape
@@ -50,7 +52,11 @@ class MatchedFilter:
             out_snr = torch.empty((n, H, W), dtype=torch.float32, device=frames.device)
         if self.topk > 0 and out_topk is None:
             out_topk = torch.empty((n, self.topk, 4), dtype=torch.int32, device=frames.device)
-        if frame_times is None and jitter_xy is None:
+        if valid is not None:
+            B.tno_mf_search_masked(self.ctx, frames, valid, sigma_t, frame_times, jitter_xy, trajectories,
+                                   prf_sigma, t0, out_snr if want_maps else None,
+                                   out_topk if self.topk > 0 else None)
+        elif frame_times is None and jitter_xy is None:
             B.tno_mf_search(self.ctx, frames, sigma_t, trajectories, prf_sigma, t0,
                             out_snr if want_maps else None, out_topk if self.topk > 0 else None)
         else:
