@@ -190,6 +190,17 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
 }
 
 // ------------------------------------------------------------------------------------ main kernel
+// Predicated red.global.add.v2.f32 (fire and forget: no read latency, no branch).
+__device__ __forceinline__ void red_add_v2_if(bool pred, float *addr, float2 v) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.u32 p, %0, 0;\n"
+        "@p red.global.add.v2.f32 [%1], {%2, %3};\n"
+        "}\n" ::"r"((uint32_t)pred),
+        "l"(addr), "f"(v.x), "f"(v.y)
+        : "memory");
+}
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -411,12 +422,12 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                             if (y_active) {
                                 const int32_t yb = yr0 - reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
                                 float *p = ebase + (int64_t)(s * H + yb) * W;
+                                asm volatile("" : "+l"(p));      // one address, then p += W per row
 #pragma unroll
                                 for (int r = 0; r < R; ++r, p += W) {
-                                    // red.global.add.v2.f32: no read latency; the piece address is
-                                    // owned by this CTA, and f_done orders the adds of successive flushes
-                                    if ((uint32_t)(yb + r) < (uint32_t)H)
-                                        atomicAdd(reinterpret_cast<float2 *>(p), acc[s][r]);
+                                    // the piece address is owned by this CTA, and f_done orders the adds
+                                    // of successive flushes; rows outside the frame are predicated off
+                                    red_add_v2_if((uint32_t)(yb + r) < (uint32_t)H, p, acc[s][r]);
                                     acc[s][r] = make_float2(0.f, 0.f);
                                 }
                             }
