@@ -47,15 +47,16 @@ namespace tno {
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return (uint32_t)__cvta_generic_to_shared(p);
 }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+// The mbarrier helpers take 32-bit shared-window addresses (smem base computed once per thread).
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar),
                  "r"(bytes)
                  : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t done;
     do {
         asm volatile(
@@ -65,23 +66,23 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
             "selp.u32 %0, 1, 0, p;\n"
             "}\n"
             : "=r"(done)
-            : "r"(smem_u32(bar)), "r"(parity)
+            : "r"(bar), "r"(parity)
             : "memory");
     } while (!done);
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int32_t c0, int32_t c1,
-                                            int32_t c2, uint64_t *bar) {
+                                            int32_t c2, uint32_t bar) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, "
         "%3, %4}], [%5];" ::"r"(smem_u32(dst)),
-        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
         : "memory");
 }
-__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint32_t bar) {
     asm volatile(
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
             smem_u32(dst)),
-        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        "l"(src), "r"(bytes), "r"(bar)
         : "memory");
 }
 
@@ -201,8 +202,8 @@ __device__ __forceinline__ void red_add_v2_if(bool pred, float *addr, float2 v) 
         "l"(addr), "f"(v.x), "f"(v.y)
         : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
 // Warp-specialised, persistent.  Per CTA-local frame counter n (frames of all its work items in
@@ -225,19 +226,19 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
     float *Rbuf = reinterpret_cast<float *>(smem_raw);
     float *Xbuf = Rbuf + SB * C::RBUF;
     float *Tab = Xbuf + XR * C::XBUF;
-    uint64_t *full_box = reinterpret_cast<uint64_t *>(Tab + TS * TABW);
-    uint64_t *x_full = full_box + SB;
-    uint64_t *x_empty = x_full + XR;
-    uint64_t *f_done = x_empty + XR;      // [NB] all consumer warps have finished their k-th flush of entry e
+    const uint32_t full_box = smem_u32(Tab + TS * TABW);   // mbarriers, 8 bytes each:
+    const uint32_t x_full = full_box + 8 * SB;             //   [SB] box + table landed, [XR] X produced,
+    const uint32_t x_empty = x_full + 8 * XR;              //   [XR] X consumed by all consumer warps,
+    const uint32_t f_done = x_empty + 8 * XR;              //   [NB] k-th flush of entry e finished by all of them
 
     const int32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int32_t T = a.T, H = a.H, W = a.W;
     const int32_t n_items = ntx * nty * a.n_batches;          // < 2^31 (checked by the host)
 
     if (tid == 0) {
-        for (int s = 0; s < SB; ++s) mbar_init(&full_box[s], 1);
-        for (int s = 0; s < XR; ++s) { mbar_init(&x_full[s], kPW); mbar_init(&x_empty[s], CW); }
-        for (int s = 0; s < NB; ++s) mbar_init(&f_done[s], CW);
+        for (int s = 0; s < SB; ++s) mbar_init(full_box + 8 * (s), 1);
+        for (int s = 0; s < XR; ++s) { mbar_init(x_full + 8 * (s), kPW); mbar_init(x_empty + 8 * (s), CW); }
+        for (int s = 0; s < NB; ++s) mbar_init(f_done + 8 * (s), CW);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -259,9 +260,9 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         };
         auto iss_one = [&]() {          // request frame iss_n into box stage iss_n % SB, table stage iss_ts
             const int32_t sb = iss_n & (SB - 1);
-            mbar_expect_tx(&full_box[sb], C::BOX_BYTES + TABW * 4);
-            tma_load_3d(Rbuf + sb * C::RBUF, &map, iss_x0 + xo_next, iss_y, iss_t, &full_box[sb]);
-            bulk_load(Tab + iss_ts * TABW, iss_ptr, TABW * 4, &full_box[sb]);
+            mbar_expect_tx(full_box + 8 * (sb), C::BOX_BYTES + TABW * 4);
+            tma_load_3d(Rbuf + sb * C::RBUF, &map, iss_x0 + xo_next, iss_y, iss_t, full_box + 8 * (sb));
+            bulk_load(Tab + iss_ts * TABW, iss_ptr, TABW * 4, full_box + 8 * (sb));
             ++iss_n;
             iss_ts = (iss_ts + 1) & (TS - 1);
             iss_ptr += TABW;
@@ -289,8 +290,8 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
             for (int32_t t = 0; t < T; ++t) {
                 const int32_t sb = n & (SB - 1), xr = n & (XR - 1);
-                mbar_wait(&full_box[sb], (n / SB) & 1);
-                if (n >= XR) mbar_wait(&x_empty[xr], ((n / XR) + 1) & 1);
+                mbar_wait(full_box + 8 * (sb), (n / SB) & 1);
+                if (n >= XR) mbar_wait(x_empty + 8 * (xr), ((n / XR) + 1) & 1);
                 const float *tb = Tab + (n & (TS - 1)) * TABW;
                 const int32_t o = reinterpret_cast<const int32_t *>(tb)[1];
                 const float g0 = tb[4], g1 = tb[5], g2 = tb[6], g3 = tb[7], g4 = tb[8];
@@ -316,7 +317,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                     *reinterpret_cast<float4 *>(dst) = v;
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&x_full[xr]);
+                if (lane == 0) mbar_arrive(x_full + 8 * (xr));
                 asm volatile("bar.sync 1, %0;" ::"n"(kPW * 32) : "memory");   // all producers are done with box sb
                 if (issuer && iss_item < n_items) iss_one();
                 ++n;
@@ -350,7 +351,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 
             for (int32_t t = 0; t < T; ++t) {
                 const int32_t xr = n & (XR - 1);
-                mbar_wait(&x_full[xr], (n / XR) & 1);
+                mbar_wait(x_full + 8 * (xr), (n / XR) & 1);
                 const float *th = Tab + (n & (TS - 1)) * TABW;
                 const float *tb = th + kHdr;
                 if (y_active) {
@@ -403,7 +404,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 const int32_t fmask = reinterpret_cast<const int32_t *>(th)[3];
                 const int32_t fwait = reinterpret_cast<const int32_t *>(th)[10];
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&x_empty[xr]);      // this warp no longer reads X[xr]
+                if (lane == 0) mbar_arrive(x_empty + 8 * (xr));      // this warp no longer reads X[xr]
                 if (fmask != 0) {
                     // ---------------- flush: piece[ty mod NP][entry][P - d][x] += acc, acc = 0
 #pragma unroll
@@ -417,7 +418,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                             // producers waited for every consumer to release frame n - XR, which each
                             // did after its flushes of the frames before); otherwise wait on f_done --
                             // also needed so that no warp arrives twice in one phase of f_done.
-                            if (fwait & (1 << s)) mbar_wait(&f_done[s], ((fpar >> s) & 1u) ^ 1u);
+                            if (fwait & (1 << s)) mbar_wait(f_done + 8 * (s), ((fpar >> s) & 1u) ^ 1u);
                             fpar ^= 1u << s;
                             if (y_active) {
                                 const int32_t yb = yr0 - reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
@@ -432,7 +433,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                                 }
                             }
                             __syncwarp();
-                            if (lane == 0) mbar_arrive(&f_done[s]);
+                            if (lane == 0) mbar_arrive(f_done + 8 * (s));
                         }
                     }
                 }
