@@ -91,7 +91,7 @@ constexpr int kTileW = 64;   // output tile width: 32 lanes x 2 columns
 constexpr int kBoxW = 76;    // staged columns: 64 + 4 halo + up to 3 of alignment (the TMA start
                              // coordinate must be 16-byte aligned) = 71, padded to a pitch = 12 mod 32
 constexpr int kXP = 68;      // pitch of the X rows (words), = 4 mod 32
-constexpr int kSeg = 64;     // an entry's accumulators are flushed at least every kSeg frames
+constexpr int kSeg = 128;    // an entry's accumulators are flushed at least every kSeg frames
 constexpr int kHdr = 16;     // header words of a stage table entry
 constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per warpgroup)
 // stage table entry (32-bit words), one per (batch, frame t):
