@@ -142,6 +142,23 @@ int tno_mf_search_masked(tno_mf_ctx *ctx,
                          float *out_snr,
                          tno_mf_cand *out_topk);
 
+/* The search on a stack in HOST memory, results to HOST memory.  The stack is uploaded in bands of frame
+ * rows on a second stream; the search of a band of tiles starts as soon as its rows (all T frames) are on the
+ * device, so the transfer (the longer of the two on PCIe) hides the computation.  Same results, bit for bit,
+ * as tno_mf_search_ex on the uploaded stack.
+ *   frames_host    HOST float32 [T][H][W]; page-locked memory is needed for the overlap (pageable works, slower).
+ *   out_snr_host   HOST float32 [n_traj][H][W] or NULL.     out_topk_host  HOST [n_traj][topk] or NULL.
+ * Unlike the device-pointer calls this one RETURNS AFTER THE RESULTS ARE IN THE HOST BUFFERS (it synchronises
+ * the context's stream).  The device copy of the stack and of the outputs lives in the context's workspace.
+ * Errors: as tno_mf_search_ex. */
+int tno_mf_search_host(tno_mf_ctx *ctx,
+                       const float *frames_host, int32_t T, int32_t H, int32_t W,
+                       const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                       const tno_mf_traj *trajectories, int32_t n_traj,
+                       float prf_sigma, float t0,
+                       float *out_snr_host,
+                       tno_mf_cand *out_topk_host);
+
 /* Signal injection ("signal injection corresponds to adding a filter times a flux
  * to the raw data"): for each source m in order and every frame t,
  *     R_t(p) <- (float)((double)R_t(p) + amplitude_m * g(p - c_t))  on the 25 window taps,

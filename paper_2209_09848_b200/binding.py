@@ -54,6 +54,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_search_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_search_masked.restype = ctypes.c_int
     lib.tno_mf_search_masked.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_search_host.restype = ctypes.c_int
+    lib.tno_mf_search_host.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_flux.restype = ctypes.c_int
     lib.tno_mf_flux.argtypes = [vp, vp, i32, i32, i32, vp]
     lib.tno_mf_best.restype = ctypes.c_int
@@ -178,6 +180,28 @@ def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories,
                                    jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,
                                    float(prf_sigma), float(t0), p_snr, p_top)
     _check(rc, ctx)
+
+
+def tno_mf_search_host(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
+                       out_snr=None, out_topk=None) -> None:
+    """frames: HOST float32 tensor or ndarray [T, H, W] (contiguous; pinned for overlap); out_snr: HOST float32
+    [n, H, W] or None; out_topk: HOST buffer of n*topk*16 bytes or None.  Returns when the results are in."""
+    def _ptr(a):
+        return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+    T, H, W = frames.shape
+    assert (frames.is_contiguous() if hasattr(frames, "is_contiguous") else frames.flags.c_contiguous)
+    assert (not hasattr(frames, "is_cuda")) or (not frames.is_cuda)
+    sig = np.ascontiguousarray(sigma_t, dtype=np.float32)
+    tm = None if frame_times is None else np.ascontiguousarray(frame_times, dtype=np.float32)
+    jt = None if jitter_xy is None else np.ascontiguousarray(jitter_xy, dtype=np.float32)
+    assert sig.shape == (T,) and (tm is None or tm.shape == (T,)) and (jt is None or jt.shape == (T, 2))
+    tr = _traj_array(trajectories)
+    _check(_lib.tno_mf_search_host(ctx, _ptr(frames), T, H, W, sig.ctypes.data,
+                                   tm.ctypes.data if tm is not None else None,
+                                   jt.ctypes.data if jt is not None else None, tr.ctypes.data, tr.shape[0],
+                                   float(prf_sigma), float(t0),
+                                   _ptr(out_snr) if out_snr is not None else None,
+                                   _ptr(out_topk) if out_topk is not None else None), ctx)
 
 
 def tno_mf_flux(ctx, snr, out_flux) -> None:

@@ -30,6 +30,13 @@ struct tno_mf_ctx {
     void *encode_fn = nullptr;
     std::string err;
     int32_t last_launches = 0, last_kernel = 0;
+    // host-fed search (tno_mf_search_host): rows [0, fed_rows) of every frame are on the device
+    const float *feed_host = nullptr;
+    float *feed_dev = nullptr;
+    int32_t fed_rows = 0, feed_T = 0, feed_H = 0, feed_W = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t copy_ev = nullptr, start_ev = nullptr;
+    DevBuf stack, hmaps, htopk;
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
     const TrajInfo *s_ti = nullptr;
@@ -131,6 +138,22 @@ int record_event(tno_mf_ctx *ctx) {
     return TNO_MF_OK;
 }
 
+// Host-fed search: upload the rows [fed_rows, r_end) of every frame (one strided 2-D copy on the copy
+// stream) and make the compute stream wait for them.  No-op for a device-resident stack.
+int feed_rows(tno_mf_ctx *ctx, int32_t r_end) {
+    if (!ctx->feed_host) return TNO_MF_OK;
+    r_end = std::min(r_end, ctx->feed_H);
+    if (r_end <= ctx->fed_rows) return TNO_MF_OK;
+    const size_t pitch = (size_t)ctx->feed_H * ctx->feed_W * 4, off = (size_t)ctx->fed_rows * ctx->feed_W;
+    CU_TRY(ctx, cudaMemcpy2DAsync(ctx->feed_dev + off, pitch, ctx->feed_host + off, pitch,
+                                  (size_t)(r_end - ctx->fed_rows) * ctx->feed_W * 4, (size_t)ctx->feed_T,
+                                  cudaMemcpyHostToDevice, ctx->copy_stream));
+    CU_TRY(ctx, cudaEventRecord(ctx->copy_ev, ctx->copy_stream));
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->copy_ev, 0));
+    ctx->fed_rows = r_end;
+    return TNO_MF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -208,10 +231,14 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     if (!ctx) return TNO_MF_OK;
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
-                      &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp};
+                      &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
+                      &ctx->stack, &ctx->hmaps, &ctx->htopk};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    if (ctx->copy_ev) cudaEventDestroy(ctx->copy_ev);
+    if (ctx->start_ev) cudaEventDestroy(ctx->start_ev);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     delete ctx;
     return TNO_MF_OK;
 }
@@ -609,12 +636,22 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
                 a.frames = pass ? valid : frames;
                 a.stage_tab = static_cast<const float *>(ctx->stage_tab.p) + pass * tab_floats + (size_t)b0 * T * tabw;
                 a.pieces = static_cast<float *>(ctx->pieces.p) + pass * pass_floats;
-                int32_t grid = 0;
-                const char *err = "";
-                if ((rc = record_event(ctx))) return rc;
-                if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
-                    return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
-                if ((rc = record_event(ctx))) return rc;
+                // a host-fed stack arrives in bands of tile rows: the search of a band starts as soon as
+                // its frame rows are on the device and overlaps the upload of the next bands
+                const int32_t nty = sep_tile_rows(variant, H);
+                const int32_t band = (ctx->feed_host && ctx->fed_rows < H) ? 4 : nty;
+                for (int32_t ty0 = 0; ty0 < nty; ty0 += band) {
+                    a.ty0 = ty0;
+                    a.ty1 = std::min(nty, ty0 + band);
+                    if ((rc = feed_rows(ctx, a.ty1 == nty ? H : a.ty1 * sv.tile_h))) return rc;
+                    int32_t grid = 0;
+                    const char *err = "";
+                    if ((rc = record_event(ctx))) return rc;
+                    if (launch_search_sep(st, variant, a, ctx->encode_fn, &grid, &err) != 0)
+                        return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
+                    if ((rc = record_event(ctx))) return rc;
+                    ctx->last_launches += (ty0 > 0);
+                }
             }
             const float *np_ = static_cast<const float *>(ctx->pieces.p);
             launch_finish(st, np_, valid ? np_ + pass_floats : nullptr, n_pieces, a.piece_stride,
@@ -632,6 +669,7 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
         ctx->last_fma_y = n_pass * 5.0 * (double)n_traj * T * (double)H * W;
     } else {
         // generic path: maps are always materialised (caller's buffer, or a workspace chunk)
+        if ((rc = feed_rows(ctx, H))) return rc;
         int32_t chunk = n_traj;
         float *maps = out_snr;
         if (!out_snr) {
@@ -663,6 +701,53 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
     }
     ctx->s_traj = n_traj; ctx->s_H = H; ctx->s_W = W;
     ctx->s_ti = valid ? nullptr : d_ti;                // tno_mf_flux needs the analytic D tables
+    return TNO_MF_OK;
+}
+
+int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int32_t H, int32_t W,
+                       const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                       const tno_mf_traj *trajectories, int32_t n_traj, float prf_sigma, float t0,
+                       float *out_snr_host, tno_mf_cand *out_topk_host) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (!frames_host) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host: NULL frames");
+    if (T < 1 || H < 1 || W < 1 || n_traj < 1)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host: T, H, W and n_traj must be >= 1");
+    const bool want_topk = out_topk_host != nullptr && ctx->cfg.topk > 0;
+    if (!out_snr_host && !want_topk)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host: no output requested");
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc;
+    const size_t px = (size_t)H * W;
+    if ((rc = reserve(ctx, ctx->stack, (size_t)T * px * 4))) return rc;
+    if (out_snr_host && (rc = reserve(ctx, ctx->hmaps, (size_t)n_traj * px * 4))) return rc;
+    if (want_topk && (rc = reserve(ctx, ctx->htopk, (size_t)n_traj * ctx->cfg.topk * sizeof(tno_mf_cand)))) return rc;
+    if (!ctx->copy_stream) {
+        CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->copy_ev, cudaEventDisableTiming));
+        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->start_ev, cudaEventDisableTiming));
+    }
+    // the upload must not overtake earlier work of the context that still reads the device stack
+    CU_TRY(ctx, cudaEventRecord(ctx->start_ev, ctx->stream));
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->start_ev, 0));
+    ctx->feed_host = frames_host;
+    ctx->feed_dev = static_cast<float *>(ctx->stack.p);
+    ctx->fed_rows = 0;
+    ctx->feed_T = T; ctx->feed_H = H; ctx->feed_W = W;
+    float *d_maps = out_snr_host ? static_cast<float *>(ctx->hmaps.p) : nullptr;
+    tno_mf_cand *d_topk = want_topk ? static_cast<tno_mf_cand *>(ctx->htopk.p) : nullptr;
+    rc = tno_mf_search_masked(ctx, ctx->feed_dev, nullptr, T, H, W, sigma_t, frame_times, jitter_xy, trajectories,
+                              n_traj, prf_sigma, t0, d_maps, d_topk);
+    ctx->feed_host = nullptr;
+    if (rc != TNO_MF_OK) {
+        cudaStreamSynchronize(ctx->copy_stream);           // nothing of the caller's buffer is in flight on return
+        return rc;
+    }
+    if (d_maps)
+        CU_TRY(ctx, cudaMemcpyAsync(out_snr_host, d_maps, (size_t)n_traj * px * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    if (d_topk)
+        CU_TRY(ctx, cudaMemcpyAsync(out_topk_host, d_topk, (size_t)n_traj * ctx->cfg.topk * sizeof(tno_mf_cand),
+                                    cudaMemcpyDeviceToHost, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
     return TNO_MF_OK;
 }
 

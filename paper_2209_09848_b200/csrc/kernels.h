@@ -75,6 +75,7 @@ struct SepArgs {
     int64_t piece_stride;         // floats between pieces = chunk entries * H * W
     int32_t n_pieces;
     int32_t n_sm;
+    int32_t ty0 = 0, ty1 = 0;     // tile rows [ty0, ty1) of the position space; ty1 = 0: up to the last one
 };
 // returns cudaError_t-like code (0 ok); *grid_out = number of CTAs used
 int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode_fn, int32_t *grid_out,

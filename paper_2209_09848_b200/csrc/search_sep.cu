@@ -36,6 +36,7 @@
 //   * y-pass: R rows x 2 columns x NB entries per thread in FP32 registers, packed FFMA2
 //     (fma.rn.f32x2: two columns per instruction), which halves the issue slots of the y-pass and
 //     leaves room for the producer warps on the same schedulers.
+#include <algorithm>
 #include <cstdio>
 
 #include "kernels.h"
@@ -219,7 +220,7 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 template <class C>
 __global__ void __launch_bounds__(C::NT, 1)
 k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int32_t ntx,
-             const int32_t nty) {
+             const int32_t nty) {      // nty tile rows starting at a.ty0
     constexpr int R = C::R, NB = C::NB, CW = C::CW, HT = C::HT;
     constexpr int SB = C::SB, XR = C::XR, TS = C::TS, TABW = C::TABW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -252,7 +253,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         int32_t iss_item = blockIdx.x, iss_t = 0, iss_n = 0, iss_ts = 0, iss_x0 = 0, iss_y = 0, xo_next = 0;
         const int32_t *iss_ptr = nullptr;
         auto iss_setup = [&]() {
-            const int32_t b = iss_item % a.n_batches, tile = iss_item / a.n_batches;
+            const int32_t b = iss_item % a.n_batches, tile = a.ty0 * ntx + iss_item / a.n_batches;
             iss_x0 = (tile % ntx) * kTileW;
             iss_y = (tile / ntx) * HT - 4;
             iss_ptr = reinterpret_cast<const int32_t *>(a.stage_tab + (int64_t)b * T * TABW);
@@ -285,7 +286,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         const int32_t row_in = lane & 7, quad = 4 * pw + (lane >> 3);
         int32_t n = 0;
         for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-            const int32_t Y0 = (item / a.n_batches / ntx) * HT - 2;
+            const int32_t Y0 = (a.ty0 + item / a.n_batches / ntx) * HT - 2;
             // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
             const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
             for (int32_t t = 0; t < T; ++t) {
@@ -333,7 +334,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             // flush coordinates of the item: entry s of the batch has planned index q_first + s, its
             // piece map starts at ebase + s*H*W (this lane's two columns), and the accumulator row r
             // of this warp holds output row yr0 + r - d
-            const int32_t b = item % a.n_batches, tile = item / a.n_batches;
+            const int32_t b = item % a.n_batches, tile = a.ty0 * ntx + item / a.n_batches;
             const int32_t ty = tile / ntx;
             const int32_t x = (tile % ntx) * kTileW + 2 * lane;
             float *ebase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride +
@@ -566,10 +567,15 @@ static int launch_t(cudaStream_t st, const SepArgs &a, void *encode_fn, int32_t 
         *err = cudaGetErrorString(e0);
         return (int)e0;
     }
-    const int32_t ntx = (a.W + kTileW - 1) / kTileW, nty = (a.H + 4 + C::HT - 1) / C::HT;
+    const int32_t ntx = (a.W + kTileW - 1) / kTileW, nty_all = (a.H + 4 + C::HT - 1) / C::HT;
+    const int32_t nty = (a.ty1 > 0 ? std::min(a.ty1, nty_all) : nty_all) - a.ty0;     // tile rows of this launch
+    if (a.ty0 < 0 || nty < 1) {
+        *err = "empty tile-row range";
+        return -1;
+    }
     const int64_t n_items = (int64_t)ntx * nty * a.n_batches;
-    if (n_items >= ((int64_t)1 << 31)) {
-        *err = "too many (tile, batch) work items";
+    if (n_items >= ((int64_t)1 << 31) || (n_items / a.n_sm + 1) * a.T >= ((int64_t)1 << 31)) {
+        *err = "too many (tile, batch, frame) steps";
         return -1;
     }
     const int32_t grid = (int32_t)(n_items < a.n_sm ? n_items : a.n_sm);

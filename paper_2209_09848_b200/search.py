@@ -64,6 +64,13 @@ class MatchedFilter:
                                out_snr if want_maps else None, out_topk if self.topk > 0 else None)
         return (out_snr if want_maps else None), (out_topk if self.topk > 0 else None)
 
+    def search_host(self, frames_host, sigma_t, trajectories, prf_sigma: float, t0: float, out_snr_host=None,
+                    out_topk_host=None, frame_times=None, jitter_xy=None) -> None:
+        """Stack and outputs in HOST memory (torch CPU tensors, pinned for overlap, or numpy arrays); the
+        upload is overlapped with the search.  Returns when the results are in the host buffers."""
+        B.tno_mf_search_host(self.ctx, frames_host, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma, t0,
+                             out_snr_host, out_topk_host)
+
     def flux(self, snr):
         """Flux estimate N / D of the maps of the last search on this context."""
         out = self._torch.empty_like(snr)
