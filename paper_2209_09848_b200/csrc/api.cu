@@ -34,8 +34,11 @@ struct tno_mf_ctx {
     const float *feed_host = nullptr;
     float *feed_dev = nullptr;
     int32_t fed_rows = 0, feed_T = 0, feed_H = 0, feed_W = 0;
-    cudaStream_t copy_stream = nullptr;
-    cudaEvent_t copy_ev = nullptr, start_ev = nullptr;
+    cudaStream_t copy_stream = nullptr, down_stream = nullptr;
+    cudaEvent_t copy_ev = nullptr, start_ev = nullptr, fin_ev = nullptr;
+    float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
+    const float *down_dev = nullptr;
+    int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
     DevBuf stack, hmaps, htopk;
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
@@ -154,6 +157,22 @@ int feed_rows(tno_mf_ctx *ctx, int32_t r_end) {
     return TNO_MF_OK;
 }
 
+// Host-fed search: once the rows [down_rows, r_end) of all maps are final on the compute stream, send them
+// to the host on the download stream (PCIe is full duplex: this overlaps the upload of later bands).
+int download_rows(tno_mf_ctx *ctx, int32_t r_end) {
+    if (!ctx->down_host) return TNO_MF_OK;
+    r_end = std::min(r_end, ctx->feed_H);
+    if (r_end <= ctx->down_rows) return TNO_MF_OK;
+    const size_t pitch = (size_t)ctx->feed_H * ctx->feed_W * 4, off = (size_t)ctx->down_rows * ctx->feed_W;
+    CU_TRY(ctx, cudaEventRecord(ctx->fin_ev, ctx->stream));
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->down_stream, ctx->fin_ev, 0));
+    CU_TRY(ctx, cudaMemcpy2DAsync(ctx->down_host + off, pitch, ctx->down_dev + off, pitch,
+                                  (size_t)(r_end - ctx->down_rows) * ctx->feed_W * 4, (size_t)ctx->down_K,
+                                  cudaMemcpyDeviceToHost, ctx->down_stream));
+    ctx->down_rows = r_end;
+    return TNO_MF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -238,7 +257,9 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     if (ctx->copy_ev) cudaEventDestroy(ctx->copy_ev);
     if (ctx->start_ev) cudaEventDestroy(ctx->start_ev);
+    if (ctx->fin_ev) cudaEventDestroy(ctx->fin_ev);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->down_stream) cudaStreamDestroy(ctx->down_stream);
     delete ctx;
     return TNO_MF_OK;
 }
@@ -631,6 +652,11 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
             a.n_sm = ctx->n_sm;
             const size_t pass_floats = (size_t)n_pieces * a.piece_stride;
             CU_TRY(ctx, cudaMemsetAsync(a.pieces, 0, n_pass * pass_floats * 4, st));
+            const int32_t nfy = (H + kCollectTile - 1) / kCollectTile;   // rows of 64 x 64 output tiles
+            int32_t fin_tiles = 0;                                        // ... already finished (banded)
+            const bool banded_finish = ctx->feed_host && ctx->fed_rows < H && n_pass == 1 && qn == n_traj;
+            int64_t y_smax = INT32_MIN;                                   // largest y-shift of the bank
+            for (const AxisClass &c : plan.ycls) y_smax = std::max<int64_t>(y_smax, c.smax);
             for (int32_t pass = 0; pass < n_pass; ++pass) {
                 // pass 1 of a masked search: the same kernel over the validity weights with squared taps
                 a.frames = pass ? valid : frames;
@@ -651,11 +677,26 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
                         return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
                     if ((rc = record_event(ctx))) return rc;
                     ctx->last_launches += (ty0 > 0);
+                    // host-fed, one chunk, one pass: the output rows that no later tile row can touch are
+                    // finished and sent to the host while the next bands are still being uploaded
+                    if (banded_finish && a.ty1 < nty) {
+                        const int32_t fy1 = std::min<int64_t>(nfy, std::max<int64_t>(
+                            fin_tiles, ((int64_t)a.ty1 * sv.tile_h - y_smax - 2) / kCollectTile));
+                        if (fy1 > fin_tiles) {
+                            launch_finish(st, static_cast<const float *>(ctx->pieces.p), nullptr, n_pieces, a.piece_stride,
+                                          reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W,
+                                          fin_tiles, fy1, out_snr, slots);
+                            ctx->last_launches += 1;
+                            fin_tiles = fy1;
+                            if ((rc = download_rows(ctx, fy1 * kCollectTile))) return rc;
+                        }
+                    }
                 }
             }
             const float *np_ = static_cast<const float *>(ctx->pieces.p);
             launch_finish(st, np_, valid ? np_ + pass_floats : nullptr, n_pieces, a.piece_stride,
-                          reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W, out_snr, slots);
+                          reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W, fin_tiles, nfy,
+                          out_snr, slots);
             CU_TRY(ctx, cudaGetLastError());
             ctx->last_launches += 2 + n_pass;              // memset, search(es), finish
             b0 = b1;
@@ -725,6 +766,8 @@ int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int
         CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
         CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->copy_ev, cudaEventDisableTiming));
         CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->start_ev, cudaEventDisableTiming));
+        CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->down_stream, cudaStreamNonBlocking));
+        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->fin_ev, cudaEventDisableTiming));
     }
     // the upload must not overtake earlier work of the context that still reads the device stack
     CU_TRY(ctx, cudaEventRecord(ctx->start_ev, ctx->stream));
@@ -734,20 +777,26 @@ int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int
     ctx->fed_rows = 0;
     ctx->feed_T = T; ctx->feed_H = H; ctx->feed_W = W;
     float *d_maps = out_snr_host ? static_cast<float *>(ctx->hmaps.p) : nullptr;
+    ctx->down_host = out_snr_host;
+    ctx->down_dev = d_maps;
+    ctx->down_rows = 0;
+    ctx->down_K = n_traj;
     tno_mf_cand *d_topk = want_topk ? static_cast<tno_mf_cand *>(ctx->htopk.p) : nullptr;
     rc = tno_mf_search_masked(ctx, ctx->feed_dev, nullptr, T, H, W, sigma_t, frame_times, jitter_xy, trajectories,
                               n_traj, prf_sigma, t0, d_maps, d_topk);
     ctx->feed_host = nullptr;
+    if (rc == TNO_MF_OK) rc = download_rows(ctx, H);       // the rows no band could finish early
+    ctx->down_host = nullptr;
     if (rc != TNO_MF_OK) {
-        cudaStreamSynchronize(ctx->copy_stream);           // nothing of the caller's buffer is in flight on return
+        cudaStreamSynchronize(ctx->copy_stream);           // nothing of the caller's buffers is in flight on return
+        cudaStreamSynchronize(ctx->down_stream);
         return rc;
     }
-    if (d_maps)
-        CU_TRY(ctx, cudaMemcpyAsync(out_snr_host, d_maps, (size_t)n_traj * px * 4, cudaMemcpyDeviceToHost, ctx->stream));
     if (d_topk)
         CU_TRY(ctx, cudaMemcpyAsync(out_topk_host, d_topk, (size_t)n_traj * ctx->cfg.topk * sizeof(tno_mf_cand),
                                     cudaMemcpyDeviceToHost, ctx->stream));
     CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->down_stream));
     return TNO_MF_OK;
 }
 

@@ -85,6 +85,7 @@ int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode
 // dpieces != NULL (masked search): SNR = (sum of pieces) / sqrt(sum of dpieces), 0 where that is 0
 void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
-                   int32_t H, int32_t W, float *out_snr, const TopkSlots &slots);
+                   int32_t H, int32_t W, int32_t fy0, int32_t fy1 /* rows of 64 x 64 tiles [fy0, fy1) */,
+                   float *out_snr, const TopkSlots &slots);
 
 }  // namespace tno

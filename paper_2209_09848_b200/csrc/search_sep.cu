@@ -450,13 +450,13 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 __global__ void __launch_bounds__(256)
 k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, int32_t n_pieces, int64_t piece_stride,
          const int32_t *__restrict__ perm, int32_t q0, const TrajInfo *__restrict__ traj,
-         const float *__restrict__ rsd, int32_t H, int32_t W, float *__restrict__ out_snr,
+         const float *__restrict__ rsd, int32_t H, int32_t W, int32_t fy0, float *__restrict__ out_snr,
          TopkSlots slots) {
     __shared__ uint64_t list[kCollectTile * kCollectTile];
     __shared__ int32_t count;
     const int32_t tid = threadIdx.x, lane = tid & 31;
     const int32_t ql = blockIdx.z, k = perm[q0 + ql];
-    const int32_t x0 = blockIdx.x * kCollectTile, y0 = blockIdx.y * kCollectTile;
+    const int32_t x0 = blockIdx.x * kCollectTile, y0 = (fy0 + blockIdx.y) * kCollectTile;
     const bool want_topk = slots.keys != nullptr;
     if (tid == 0) count = 0;
     __syncthreads();
@@ -514,7 +514,7 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
     }
     if (want_topk) {
         __syncthreads();
-        const int64_t tile = (int64_t)blockIdx.y * gridDim.x + blockIdx.x;
+        const int64_t tile = (int64_t)(fy0 + blockIdx.y) * gridDim.x + blockIdx.x;
         tile_flush<256>(list, count, slots, tile, k, tid);
     }
 }
@@ -596,10 +596,10 @@ int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode
 
 void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
-                   int32_t H, int32_t W, float *out_snr, const TopkSlots &slots) {
-    dim3 grid((unsigned)((W + kCollectTile - 1) / kCollectTile),
-              (unsigned)((H + kCollectTile - 1) / kCollectTile), (unsigned)q_count);
-    k_finish<<<grid, 256, 0, st>>>(pieces, dpieces, n_pieces, piece_stride, perm, q0, traj, rsd, H, W, out_snr, slots);
+                   int32_t H, int32_t W, int32_t fy0, int32_t fy1, float *out_snr, const TopkSlots &slots) {
+    dim3 grid((unsigned)((W + kCollectTile - 1) / kCollectTile), (unsigned)(fy1 - fy0), (unsigned)q_count);
+    k_finish<<<grid, 256, 0, st>>>(pieces, dpieces, n_pieces, piece_stride, perm, q0, traj, rsd, H, W, fy0, out_snr,
+                                   slots);
 }
 
 }  // namespace tno

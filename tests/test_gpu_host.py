@@ -27,8 +27,8 @@ def test_host_search_equals_device_search(shape, pinned):
         f = f.pin_memory()
     sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
     traj = np.array([[0.3, -0.2, 0, 0], [0.3, 0.45, 0, 0], [0.3, 0.0, 0, 0.01], [-1.25, 0.5, 0, 0],
-                     [0.0, 0.0, 0, 0]], np.float32)
-    n, topk = traj.shape[0], 6
+                     [0.0, 0.0, 0, 0], [0.3, 7.0, 0, 0], [0.3, -5.5, 0, 0.2]], np.float32)   # large y-shifts too:
+    n, topk = traj.shape[0], 6                   # the early finish of output rows must wait for them
     ref_m, ref_c, _ = run_gpu(f.cuda(), sigma, traj, 1.0, T / 2.0, topk, 3.0)
     ctx = P.tno_mf_create(0, None, topk, 3.0)
     out = torch.empty((n, H, W), dtype=torch.float32)
