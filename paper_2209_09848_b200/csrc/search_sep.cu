@@ -355,13 +355,15 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 mbar_wait(x_full + 8 * (xr), (n / XR) & 1);
                 const float *th = Tab + (n & (TS - 1)) * TABW;
                 const float *tb = th + kHdr;
+                // number of entries and flush mask of the frame, read together ahead of the FFMAs
+                const int2 hdr23 = *reinterpret_cast<const int2 *>(th + 2);
                 if (y_active) {
                     // ---------------- y-pass: one register window of X for all entries of the batch
                     const float2 *xp = reinterpret_cast<const float2 *>(Xbuf + xr * C::XBUF + r0 * kXP) + lane;
                     float2 win[R + 4];
 #pragma unroll
                     for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
-                    const int32_t nfill = reinterpret_cast<const int32_t *>(th)[2];
+                    const int32_t nfill = hdr23.x;
 #define TNO_FMAS(s)                                                                                   \
     {                                                                                                 \
         const float2 w0 = make_float2(wa.x, wa.x), w1 = make_float2(wa.y, wa.y),                      \
@@ -402,11 +404,11 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                     }
 #undef TNO_FMAS
                 }
-                const int32_t fmask = reinterpret_cast<const int32_t *>(th)[3];
-                const int32_t fwait = reinterpret_cast<const int32_t *>(th)[10];
+                const int32_t fmask = hdr23.y;
                 __syncwarp();
                 if (lane == 0) mbar_arrive(x_empty + 8 * (xr));      // this warp no longer reads X[xr]
                 if (fmask != 0) {
+                    const int32_t fwait = reinterpret_cast<const int32_t *>(th)[10];
                     // ---------------- flush: piece[ty mod NP][entry][P - d][x] += acc, acc = 0
 #pragma unroll
                     for (int s = 0; s < NB; ++s) {
