@@ -40,10 +40,10 @@ CAND_DTYPE = np.dtype([("snr", np.float64), ("x", np.int32), ("y", np.int32), ("
 
 
 _lib.tno_oracle_point_ex.restype = ctypes.c_int
-_lib.tno_oracle_point_ex.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, _f32p, _f32p, _f32p, ctypes.c_float,
+_lib.tno_oracle_point_ex.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, _f32p, _f32p, ctypes.c_int, _f32p, ctypes.c_float,
                                      ctypes.c_float, ctypes.c_int, ctypes.c_int, _f64p, _f64p, _f64p]
 _lib.tno_oracle_map_ex.restype = ctypes.c_int
-_lib.tno_oracle_map_ex.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, _f32p, _f32p, _f32p, ctypes.c_int,
+_lib.tno_oracle_map_ex.argtypes = [_f32p] + [ctypes.c_int] * 7 + [_f32p, _f32p, _f32p, _f32p, ctypes.c_int, _f32p, ctypes.c_int,
                                    ctypes.c_float, ctypes.c_float] + [ctypes.c_int] * 4 + [_f64p] * 3
 _lib.tno_oracle_inject_ex.restype = ctypes.c_int
 _lib.tno_oracle_inject_ex.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f32p, _f32p, _f32p,
@@ -88,7 +88,7 @@ def _geom(frames: np.ndarray, window, full_shape):
 
 
 def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=None,
-          times=None, jitter=None, valid=None) -> Tuple[float, float, float]:
+          times=None, jitter=None, valid=None, shift_stack: bool = False) -> Tuple[float, float, float]:
     """(snr, N, D) at start pixel (x, y) for one trajectory (vx, vy, ax, ay).  times: frame times [T]
     (default the frame index), jitter: pointing offsets [T, 2] in px added to the track (default 0),
     valid: per-pixel weights of D with the layout of frames (default 1; N uses the frames as they are)."""
@@ -101,7 +101,8 @@ def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=No
     _ja, jp = _opt(jitter, (T, 2))
     rc = _lib.tno_oracle_point_ex(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
                                   sigma_t.ctypes.data_as(_f32p), tp, jp, _valid_ptr(valid, frames),
-                                  traj.ctypes.data_as(_f32p), float(prf_sigma), float(t0), int(x), int(y),
+                                  int(bool(shift_stack)), traj.ctypes.data_as(_f32p), float(prf_sigma), float(t0),
+                                  int(x), int(y),
                                   ctypes.byref(N), ctypes.byref(D), ctypes.byref(S))
     if rc != 0:
         raise ValueError("oracle.point: tap outside the supplied window (rc=%d)" % rc)
@@ -109,7 +110,7 @@ def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=No
 
 
 def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, full_shape=None,
-            return_ND: bool = False, times=None, jitter=None, valid=None):
+            return_ND: bool = False, times=None, jitter=None, valid=None, shift_stack: bool = False):
     """float64 [K, h, w] SNR for start pixels x in [x_lo, x_hi), y in [y_lo, y_hi)
     (region = (x_lo, x_hi, y_lo, y_hi), default the whole frame)."""
     frames = _f32(frames)
@@ -126,7 +127,7 @@ def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, ful
     _ja, jp = _opt(jitter, (T, 2))
     rc = _lib.tno_oracle_map_ex(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
                              sigma_t.ctypes.data_as(_f32p), tp, jp, _valid_ptr(valid, frames),
-                             trajs.ctypes.data_as(_f32p), K,
+                             int(bool(shift_stack)), trajs.ctypes.data_as(_f32p), K,
                              float(prf_sigma), float(t0), int(x_lo), int(x_hi), int(y_lo),
                              int(y_hi), out.ctypes.data_as(_f64p),
                              oN.ctypes.data_as(_f64p) if return_ND else None,

@@ -69,6 +69,14 @@ static inline double disp(double v, double a, double dt) { return v * dt + a * d
  *                                            down-weighted them, F = R * valid)
  *     D = sum g^2 valid_t(p) / sigma_t^2    (a masked pixel carries no information)
  * valid has the layout of the frames (same window); NULL = all ones. */
+/* Filter of one axis at tap offset u = i - phase (reading g2): mode 0 = the Gaussian PRF
+ * matched filter exp(-u^2 / (2 s^2)); mode 1 = shift-stack (after Rice & Laughlin 2020:
+ * "a single non-zero value, set to 1, for each time-slice"): 1 at the rounded position (i = 0), else 0. */
+static inline double tap1(int mode, int i, double ph, double s) {
+    if (mode == 1) return i == 0 ? 1.0 : 0.0;
+    const double u = (double)i - ph;
+    return exp(-(u * u) / (2.0 * s * s));
+}
 static inline double frame_dt(const float *times, int t, double t0) {
     return (times ? (double)times[t] : (double)t) - t0;
 }
@@ -95,7 +103,7 @@ int tno_oracle_threads(void) {
 int tno_oracle_point_ex(const float *frames, int T, int H, int W,
                         int wx0, int wy0, int ww, int wh,
                         const float *sigma_t, const float *times, const float *jitter, const float *valid,
-                        const float *traj4, float prf_sigma_f, float t0_f,
+                        int mode, const float *traj4, float prf_sigma_f, float t0_f,
                         int x, int y, double *N_out, double *D_out, double *snr_out)
 {
     const double vx = traj4[0], vy = traj4[1], ax = traj4[2], ay = traj4[3];
@@ -114,7 +122,8 @@ int tno_oracle_point_ex(const float *frames, int T, int H, int W,
                 if (px < 0 || px >= W || py < 0 || py >= H) continue;
                 if (px < wx0 || px >= wx0 + ww || py < wy0 || py >= wy0 + wh) return -1;
                 const double ux = (double)i - phx, uy = (double)j - phy;
-                const double g = exp(-(ux * ux + uy * uy) / (2.0 * s * s));
+                const double g = mode == 1 ? tap1(1, i, phx, s) * tap1(1, j, phy, s)
+                                           : exp(-(ux * ux + uy * uy) / (2.0 * s * s));
                 const size_t idx = ((size_t)t * wh + (size_t)(py - wy0)) * ww + (size_t)(px - wx0);
                 const double R = frames[idx];
                 N += g * R * q;
@@ -133,7 +142,7 @@ int tno_oracle_point(const float *frames, int T, int H, int W,
                      const float *sigma_t, const float *traj4, float prf_sigma_f, float t0_f,
                      int x, int y, double *N_out, double *D_out, double *snr_out)
 {
-    return tno_oracle_point_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, NULL, traj4,
+    return tno_oracle_point_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, NULL, 0, traj4,
                                prf_sigma_f, t0_f, x, y, N_out, D_out, snr_out);
 }
 
@@ -143,7 +152,7 @@ int tno_oracle_point(const float *frames, int T, int H, int W,
 int tno_oracle_map_ex(const float *frames, int T, int H, int W,
                       int wx0, int wy0, int ww, int wh,
                       const float *sigma_t, const float *times, const float *jitter, const float *valid,
-                      const float *traj, int K,
+                      int mode, const float *traj, int K,
                       float prf_sigma_f, float t0_f,
                       int x_lo, int x_hi, int y_lo, int y_hi,
                       double *out_snr, double *out_N, double *out_D)
@@ -165,9 +174,8 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
             split(disp(vy, ay, dt) + jit(jitter, t, 1), &sy, &phy);
             SX[2 * t] = sx; SX[2 * t + 1] = sy;
             for (int i = -2; i <= 2; ++i) {
-                const double ux = (double)i - phx, uy = (double)i - phy;
-                G[11 * t + (i + 2)] = exp(-(ux * ux) / (2.0 * s * s));
-                G[11 * t + 5 + (i + 2)] = exp(-(uy * uy) / (2.0 * s * s));
+                G[11 * t + (i + 2)] = tap1(mode, i, phx, s);
+                G[11 * t + 5 + (i + 2)] = tap1(mode, i, phy, s);
             }
             const double sig = sigma_t[t];
             G[11 * t + 10] = 1.0 / (sig * sig);
@@ -227,7 +235,7 @@ int tno_oracle_map(const float *frames, int T, int H, int W,
                    int x_lo, int x_hi, int y_lo, int y_hi,
                    double *out_snr, double *out_N, double *out_D)
 {
-    return tno_oracle_map_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, NULL, traj, K,
+    return tno_oracle_map_ex(frames, T, H, W, wx0, wy0, ww, wh, sigma_t, NULL, NULL, NULL, 0, traj, K,
                              prf_sigma_f, t0_f, x_lo, x_hi, y_lo, y_hi, out_snr, out_N, out_D);
 }
 
