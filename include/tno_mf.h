@@ -74,11 +74,15 @@ typedef struct {
                                 > 0: cap, in MiB, of the partial-sum workspace of the separable
                                 kernel -- a bank that needs more is searched in chunks of whole
                                 batches (same results) */
-    int32_t reserved;        /* must be 0 */
+    int32_t filter;          /* 0 = the Gaussian-PRF matched filter (the method); 1 = shift-stack, the comparison
+                                method of PAPER.md:L118 (Rice & Laughlin 2020 "use a single non-zero value, set to 1,
+                                for each time-slice"): the filter is 1 at round(c_t) and 0 elsewhere,
+                                N = sum R_t(round(c_t))/sigma_t^2, D = sum [in frame]/sigma_t^2; prf_sigma is ignored
+                                by the search (tno_mf_inject still renders with the PRF) */
 } tno_mf_config;
 
 /* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
- * workspace_limit_mb < 0, reserved != 0), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
+ * workspace_limit_mb < 0, filter not 0 or 1), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
 int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
 
 /* The search (formula above).

@@ -190,8 +190,8 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
     if (std::isnan(cfg->snr_threshold))
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
-    if (cfg->reserved || cfg->workspace_limit_mb < 0)
-        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: reserved must be 0 and workspace_limit_mb >= 0");
+    if (cfg->filter < 0 || cfg->filter > 1 || cfg->workspace_limit_mb < 0)
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 or 1 and workspace_limit_mb >= 0");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess || n_dev == 0) {
@@ -610,7 +610,7 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
     launch_class_tables(st, reinterpret_cast<const float *>(meta + o_v), reinterpret_cast<const float *>(meta + o_a),
                         frame_times ? reinterpret_cast<const float *>(meta + o_tm) : nullptr,
                         jitter_xy ? reinterpret_cast<const float *>(meta + o_jt) : nullptr,
-                        n_cls, n_x, T, (double)t0, (double)prf_sigma, static_cast<int32_t *>(ctx->shift.p),
+                        n_cls, n_x, T, (double)t0, (double)prf_sigma, ctx->cfg.filter, static_cast<int32_t *>(ctx->shift.p),
                         static_cast<float *>(ctx->g.p), static_cast<double *>(ctx->gd.p));
     launch_border_tables(st, tab.shift, tab.gd, tab.qd, reinterpret_cast<const AxisBorder *>(meta + o_bd), d_off,
                          n_cls, n_x, max_n, T, W, H, static_cast<double *>(ctx->ab.p));

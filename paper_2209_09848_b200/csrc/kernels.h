@@ -10,7 +10,8 @@ namespace tno {
 // ---- tables.cu ----
 void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a,
                          const float *times /* DEVICE [T] or NULL */, const float *jitter /* DEVICE [T][2] or NULL */,
-                         int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma, int32_t *shift,
+                         int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma,
+                         int32_t filter /* 0 = Gaussian PRF taps, 1 = shift-stack single tap */, int32_t *shift,
                          float *g, double *gd);
 void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,
                           const AxisBorder *border, const int64_t *off, int32_t n_cls, int32_t n_x,

@@ -11,7 +11,7 @@ namespace tno {
 
 __global__ void k_class_tables(const float *__restrict__ cls_v, const float *__restrict__ cls_a,
                                const float *__restrict__ times, const float *__restrict__ jitter,
-                               int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma,
+                               int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma, int32_t filter,
                                int32_t *__restrict__ shift, float *__restrict__ g,
                                double *__restrict__ gd) {
     const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -30,7 +30,8 @@ __global__ void k_class_tables(const float *__restrict__ cls_v, const float *__r
 #pragma unroll
     for (int i = 0; i < 5; ++i) {
         const double u = (double)(i - 2) - ph;
-        const double w = exp(-(u * u) * inv);
+        // filter 1 = shift-stack: a single tap of weight 1 at the rounded position
+        const double w = filter == 1 ? (i == 2 ? 1.0 : 0.0) : exp(-(u * u) * inv);
         g[id * 5 + i] = (float)w;
         gd[id * 5 + i] = w;
     }
@@ -75,10 +76,10 @@ __global__ void k_rsd_tables(const TrajInfo *__restrict__ traj, const double *__
 
 void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a, const float *times,
                          const float *jitter, int32_t n_cls, int32_t n_x, int32_t T, double t0,
-                         double prf_sigma, int32_t *shift, float *g, double *gd) {
+                         double prf_sigma, int32_t filter, int32_t *shift, float *g, double *gd) {
     const int64_t n = (int64_t)n_cls * T;
     k_class_tables<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cls_v, cls_a, times, jitter, n_cls, n_x, T,
-                                                                 t0, prf_sigma, shift, g, gd);
+                                                                 t0, prf_sigma, filter, shift, g, gd);
 }
 
 void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,

@@ -12,14 +12,15 @@ class MatchedFilter:
     """One library context bound to the current torch CUDA stream of `device`."""
 
     def __init__(self, device: int = 0, topk: int = 0, snr_threshold: float = float("-inf"),
-                 force_generic: bool = False, record_events: bool = False, workspace_limit_mb: int = 0):
+                 force_generic: bool = False, record_events: bool = False, workspace_limit_mb: int = 0,
+                 shift_stack: bool = False):
         import torch
         self._torch = torch
         self.device = torch.device("cuda", device)
         self.topk = int(topk)
         stream = torch.cuda.current_stream(self.device).cuda_stream
         self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events,
-                                   workspace_limit_mb)
+                                   workspace_limit_mb, shift_stack)
 
     def close(self) -> None:
         if self.ctx is not None:
