@@ -212,3 +212,33 @@ def local_z(m, box: int = 255, literal: bool = False):
     if rc != 0:
         raise ValueError("tno_oracle_local_z failed (%d)" % rc)
     return z, s
+
+
+# ---- high-resolution background model (PAPER.md section 3.1, L66-100) ---------------------------
+def background_basis(jitter) -> np.ndarray:
+    """[T, 6] float64 basis (1, x, y, x^2, y^2, x y) of the per-pixel model of PAPER.md Eq. 1: the background
+    B plus its 2nd-order Taylor expansion B_theta in the pointing jitter theta_t = (x_t, y_t) (L66)."""
+    j = np.asarray(jitter, dtype=np.float32).astype(np.float64)
+    x, y = j[:, 0], j[:, 1]
+    return np.stack([np.ones_like(x), x, y, x * x, y * y, x * y], axis=1)
+
+
+def background(frames, jitter, delta: float, n_iter: int):
+    """Per-pixel robust fit of the background model with the scattered light already removed:
+        y_t(p) = B(p) + B_theta(p) . theta_t^k + eps,   minimise sum_t L_delta(residual)   (Eq. 2-4)
+    by "repeated least squares solves, alternated with clipping the residuals (Huber 1977)", every pixel
+    regressed "against the same input data", so one pseudo-inverse serves all (L98-100):
+        beta_0 = pinv(Phi) y ;   beta_{i+1} = beta_i + pinv(Phi) clip(y - Phi beta_i, -delta, +delta).
+    Returns (coefficients float64 [6, H, W], residual stack float64 [T, H, W])."""
+    y = np.asarray(frames, dtype=np.float32).astype(np.float64)
+    T, H, W = y.shape
+    phi = background_basis(jitter)
+    pinv = np.linalg.pinv(phi)                       # [6, T]
+    Y = y.reshape(T, H * W)
+    beta = pinv @ Y
+    d = float(np.float32(delta))
+    for _ in range(int(n_iter)):
+        r = Y - phi @ beta
+        beta = beta + pinv @ np.clip(r, -d, d)
+    r = Y - phi @ beta
+    return beta.reshape(6, H, W), r.reshape(T, H, W)
