@@ -202,6 +202,27 @@ int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
  * Errors: EINVAL (NULL pointers, no matching preceding search), ECUDA. */
 int tno_mf_flux(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, float *out_flux);
 
+/* High-resolution background model (section 3.1, Eq. 1-4): the step that produces the residual
+ * stack the search runs on.  With the scattered light U(S_t) already removed, every pixel p is regressed on
+ * the pointing jitter theta_t = (x_t, y_t),
+ *     y_t(p) = B(p) + B_theta(p) . (x_t, y_t, x_t^2, y_t^2, x_t y_t) + eps,
+ * with the Huber loss L_delta (Eq. 4) "through repeated least squares solves, alternated with clipping the
+ * residuals (Huber 1977)" (L100):  beta_0 = least squares;  beta_{i+1} = beta_i + pinv(Phi) clip(y - Phi beta_i,
+ * -delta, +delta), i = 0 .. n_iter-1;  all pixels share Phi (orthonormalised once on the host in float64).
+ *   frames     DEVICE float32 [T][H][W]: data minus scattered light.     jitter_xy  HOST float32 [T][2], px.
+ *   delta      Huber threshold in flux units, > 0 (INFINITY: plain least squares).    n_iter >= 0.
+ *   out_coef   DEVICE float32 [6][H][W]: B, then the coefficients of x, y, x^2, y^2, xy; or NULL.  Columns of
+ *              the basis that are linearly dependent on earlier ones (e.g. no jitter at all) get 0.
+ *   out_resid  DEVICE float32 [T][H][W]: y - Phi beta, the input of tno_mf_search; may be `frames` itself
+ *              (in place); or NULL.
+ * Traffic: (n_iter + 3) * T*H*W*4 bytes (one read per pass, the last pass also writes), HBM-bound; the fast
+ * kernel needs H*W % 4 == 0 and 16-byte aligned pointers, other stacks take a slower plain kernel with the
+ * same results.  T >= 6 distinct jitter values are needed for all six coefficients to be identifiable.
+ * Enqueues on the context's stream after a short synchronisation for the basis upload.
+ * Errors: EINVAL, ENOMEM, ECUDA. */
+int tno_mf_background(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
+                      const float *jitter_xy, float delta, int32_t n_iter, float *out_coef, float *out_resid);
+
 /* Host-only planning query (no device work; ctx may be NULL): how the search would group
  * `trajectories` into batches that share one x-motion (vx, ax) -- the unit of work of the
  * separable kernel.  Writes, for each trajectory, its batch index and slot

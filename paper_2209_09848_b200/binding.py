@@ -56,6 +56,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_search_masked.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_search_host.restype = ctypes.c_int
     lib.tno_mf_search_host.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_background.restype = ctypes.c_int
+    lib.tno_mf_background.argtypes = [vp, vp, i32, i32, i32, vp, f32, i32, vp, vp]
     lib.tno_mf_flux.restype = ctypes.c_int
     lib.tno_mf_flux.argtypes = [vp, vp, i32, i32, i32, vp]
     lib.tno_mf_best.restype = ctypes.c_int
@@ -203,6 +205,20 @@ def tno_mf_search_host(ctx, frames, sigma_t, frame_times, jitter_xy, trajectorie
                                    float(prf_sigma), float(t0),
                                    _ptr(out_snr) if out_snr is not None else None,
                                    _ptr(out_topk) if out_topk is not None else None), ctx)
+
+
+def tno_mf_background(ctx, frames, jitter_xy, delta: float, n_iter: int, out_coef=None, out_resid=None) -> None:
+    """frames: CUDA float32 [T, H, W]; jitter_xy: host [T, 2]; out_coef: CUDA float32 [6, H, W] or None;
+    out_resid: CUDA float32 [T, H, W] (may be `frames`) or None.  PAPER.md section 3.1."""
+    assert frames.is_cuda and frames.is_contiguous() and frames.dim() == 3 and frames.element_size() == 4
+    T, H, W = frames.shape
+    jt = np.ascontiguousarray(jitter_xy, dtype=np.float32)
+    assert jt.shape == (T, 2)
+    for t, shp in ((out_coef, (6, H, W)), (out_resid, (T, H, W))):
+        assert t is None or (t.is_cuda and t.is_contiguous() and tuple(t.shape) == shp and t.element_size() == 4)
+    _check(_lib.tno_mf_background(ctx, frames.data_ptr(), T, H, W, jt.ctypes.data, float(delta), int(n_iter),
+                                  out_coef.data_ptr() if out_coef is not None else None,
+                                  out_resid.data_ptr() if out_resid is not None else None), ctx)
 
 
 def tno_mf_flux(ctx, snr, out_flux) -> None:

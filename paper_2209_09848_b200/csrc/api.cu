@@ -39,7 +39,7 @@ struct tno_mf_ctx {
     float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
     const float *down_dev = nullptr;
     int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
-    DevBuf stack, hmaps, htopk;
+    DevBuf stack, hmaps, htopk, bgq;
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
     const TrajInfo *s_ti = nullptr;
@@ -251,7 +251,7 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
                       &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
-                      &ctx->stack, &ctx->hmaps, &ctx->htopk};
+                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -374,6 +374,78 @@ int tno_mf_search(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, in
                   float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
     return tno_mf_search_ex(ctx, frames, T, H, W, sigma_t, nullptr, nullptr, trajectories, n_traj, prf_sigma, t0,
                             out_snr, out_topk);
+}
+
+int tno_mf_background(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
+                      const float *jitter_xy, float delta, int32_t n_iter, float *out_coef, float *out_resid) {
+    if (!ctx) return TNO_MF_EINVAL;
+    ctx->last_launches = 0;
+    ctx->ev_used = 0;
+    if (!frames || !jitter_xy) return fail(ctx, TNO_MF_EINVAL, "tno_mf_background: NULL frames or jitter_xy");
+    if (T < 1 || H < 1 || W < 1) return fail(ctx, TNO_MF_EINVAL, "tno_mf_background: T, H, W must be >= 1");
+    if (!(delta > 0.f) || std::isnan(delta)) return fail(ctx, TNO_MF_EINVAL, "tno_mf_background: delta must be > 0");
+    if (n_iter < 0) return fail(ctx, TNO_MF_EINVAL, "tno_mf_background: n_iter must be >= 0");
+    if (!out_coef && !out_resid) return fail(ctx, TNO_MF_EINVAL, "tno_mf_background: no output requested");
+    for (int32_t t = 0; t < T; ++t)
+        if (!finite_f(jitter_xy[2 * t]) || !finite_f(jitter_xy[2 * t + 1]))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_background: jitter_xy[%d] is not finite", t);
+    // basis (1, x, y, x^2, y^2, x y), orthonormalised column by column in float64 (modified Gram-Schmidt,
+    // two passes); a column that is (numerically) in the span of the earlier ones is dropped
+    std::vector<double> q((size_t)T * 6), r(36, 0.0);
+    for (int32_t t = 0; t < T; ++t) {
+        const double x = jitter_xy[2 * t], y = jitter_xy[2 * t + 1];
+        double *row = &q[(size_t)t * 6];
+        row[0] = 1.0; row[1] = x; row[2] = y; row[3] = x * x; row[4] = y * y; row[5] = x * y;
+    }
+    bool kept[6];
+    for (int k = 0; k < 6; ++k) {
+        double norm0 = 0.0;
+        for (int32_t t = 0; t < T; ++t) norm0 += q[(size_t)t * 6 + k] * q[(size_t)t * 6 + k];
+        for (int pass = 0; pass < 2; ++pass)
+            for (int m = 0; m < k; ++m) {
+                if (!kept[m]) continue;
+                double dot = 0.0;
+                for (int32_t t = 0; t < T; ++t) dot += q[(size_t)t * 6 + m] * q[(size_t)t * 6 + k];
+                r[m * 6 + k] += dot;
+                for (int32_t t = 0; t < T; ++t) q[(size_t)t * 6 + k] -= dot * q[(size_t)t * 6 + m];
+            }
+        double norm = 0.0;
+        for (int32_t t = 0; t < T; ++t) norm += q[(size_t)t * 6 + k] * q[(size_t)t * 6 + k];
+        kept[k] = norm > 1e-20 * std::max(norm0, 1e-300) && norm > 0.0;
+        const double inv = kept[k] ? 1.0 / std::sqrt(norm) : 0.0;
+        r[k * 6 + k] = kept[k] ? std::sqrt(norm) : 0.0;
+        for (int32_t t = 0; t < T; ++t) q[(size_t)t * 6 + k] *= inv;
+        if (!kept[k]) for (int m = 0; m < k; ++m) r[m * 6 + k] = 0.0;
+    }
+    // R^{-1} by back substitution on the kept columns
+    BgRinv rinv;
+    double ri[36] = {0.0};
+    for (int col = 0; col < 6; ++col) {
+        if (!kept[col]) continue;
+        for (int k = col; k >= 0; --k) {
+            if (!kept[k]) continue;
+            double v = (k == col) ? 1.0 : 0.0;
+            for (int m = k + 1; m <= col; ++m) v -= r[k * 6 + m] * ri[m * 6 + col];
+            ri[k * 6 + col] = v / r[k * 6 + k];
+        }
+    }
+    for (int i = 0; i < 36; ++i) rinv.v[i] = (float)ri[i];
+    std::vector<float> qf((size_t)T * 16, 0.f);         // row t: (q0,q0, q1,q1, ..., q5,q5, 0,0,0,0)
+    for (int32_t t = 0; t < T; ++t)
+        for (int k = 0; k < 6; ++k)
+            qf[(size_t)t * 16 + 2 * k] = qf[(size_t)t * 16 + 2 * k + 1] = (float)q[(size_t)t * 6 + k];
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc;
+    if ((rc = reserve(ctx, ctx->bgq, qf.size() * 4))) return rc;
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->bgq.p, qf.data(), qf.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));      // qf is a local buffer
+    if ((rc = record_event(ctx))) return rc;
+    launch_background(ctx->stream, frames, T, (int64_t)H * W, static_cast<const float *>(ctx->bgq.p), rinv, delta,
+                      n_iter, out_coef, out_resid);
+    if ((rc = record_event(ctx))) return rc;
+    ctx->last_launches = 1;
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
 }
 
 int tno_mf_flux(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, float *out_flux) {

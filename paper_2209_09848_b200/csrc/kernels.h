@@ -46,6 +46,12 @@ void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const 
                  int32_t W, float *out);
 void launch_set_argk(cudaStream_t st, tno_mf_cand *cand, int32_t n, const int32_t *argk, int32_t W);
 
+// ---- background.cu ---- (section 3.1: per-pixel Huber fit on the jitter basis)
+struct BgRinv { float v[36]; };      // R^{-1} of the orthonormalised basis, row major
+// Q: DEVICE [T][16] orthonormal basis, every coefficient twice + padding (see background.cu); out_resid may alias frames (in place)
+void launch_background(cudaStream_t st, const float *frames, int32_t T, int64_t n_px, const float *Q,
+                       const BgRinv &rinv, float delta, int32_t n_iter, float *out_coef, float *out_resid);
+
 // ---- inject.cu ----
 struct SourceDev { float vx, vy, ax, ay; int32_t x, y; float amp; };
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,

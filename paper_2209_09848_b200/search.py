@@ -72,6 +72,14 @@ class MatchedFilter:
         B.tno_mf_search_host(self.ctx, frames_host, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma, t0,
                              out_snr_host, out_topk_host)
 
+    def background(self, frames, jitter_xy, delta: float, n_iter: int, in_place: bool = False):
+        """PAPER.md section 3.1 on a stack with the scattered light removed: (coefficients [6, H, W], residual
+        stack [T, H, W] -- `frames` itself if in_place)."""
+        coef = self._torch.empty((6,) + tuple(frames.shape[1:]), dtype=self._torch.float32, device=frames.device)
+        res = frames if in_place else self._torch.empty_like(frames)
+        B.tno_mf_background(self.ctx, frames, jitter_xy, delta, n_iter, coef, res)
+        return coef, res
+
     def flux(self, snr):
         """Flux estimate N / D of the maps of the last search on this context."""
         out = self._torch.empty_like(snr)
