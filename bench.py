@@ -300,6 +300,37 @@ def run_ours(args, cfg):
                          "benchmarked stack" % (trajs.shape[0], cfg.T, block, block),
                "full_search_extrapolated_s": cfg.evals / rate}
 
+    # ---- optional: the calls around the search (DESIGN 8b, 8d, 8f) on the same stack, device-timed; run last
+    # because the background fit overwrites the stack with its residuals
+    extras = None
+    if args.extras:
+        def timed(fn, reps=3):
+            fn()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(reps):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / reps
+        extras = {}
+        hbm = peaks.get("hbm_gbs")
+        if cfg.want_maps:
+            step()                              # the context's D tables must be those of out_snr
+            ms = timed(lambda: mf.best(out_snr))
+            extras["best"] = {"ms": ms, "bytes": out_snr.numel() * 4, "what": "max over trajectories, local-sigma Z "
+                              "(255 box), top-K of Z"}
+            ms = timed(lambda: mf.flux(out_snr))
+            gb = 2.0 * out_snr.numel() * 4 / 1e9
+            extras["flux"] = {"ms": ms, "achieved_gbs": gb / ms * 1e3, "peak_gbs": hbm}
+        jit = (0.4 * np.random.default_rng(cfg.idx).standard_normal((cfg.T, 2))).astype(np.float32)
+        for n_iter in (0, 10):
+            ms = timed(lambda: mf.background(frames, jit, 1.0, n_iter, in_place=True), reps=2)
+            gb = (n_iter + 3.0) * frames.numel() * 4 / 1e9
+            extras["background_n_iter_%d" % n_iter] = {"ms": ms, "algorithmic_gb": gb, "achieved_gbs": gb / ms * 1e3,
+                                                       "peak_gbs": hbm, "frac": gb / ms * 1e3 / hbm if hbm else None}
+
     mf.close()
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -309,7 +340,7 @@ def run_ours(args, cfg):
                           "l2": "inputs (%.1f GB stack) larger than L2" % (frames.numel() * 4 / 1e9),
                           "search_wall_time_s": ms_per_step * 1e-3},
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-               "roofline": roofline, "cpu_baseline": cpu,
+               "roofline": roofline, "cpu_baseline": cpu, "extras": extras,
                "context": {"paper_a100_evals_per_s": 1.4e9,
                            "paper_claim": "100 trajectories x 1000 frames x 2048^2 in ~5 min on one A100 (PAPER.md:L9)"}}
         print(json.dumps(out), flush=True)
@@ -325,6 +356,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index 1..5 (3 = headline)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", action="store_true",
+                    help="also time tno_mf_best / tno_mf_flux / tno_mf_background on the same stack (after the timed region)")
     ap.add_argument("--frames", type=int, default=0,
                     help="profiling only: shorten the stack to this many frames (same recipe)")
     args = ap.parse_args()
