@@ -50,6 +50,13 @@ _lib.tno_oracle_inject_ex.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.
                                       _i32p, _i32p, _f32p, ctypes.c_int, ctypes.c_float, ctypes.c_float]
 
 
+_lib.tno_oracle_inject_mode.restype = ctypes.c_int
+_lib.tno_oracle_inject_mode.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f32p, _f32p, ctypes.c_int,
+                                        _f32p, _i32p, _i32p, _f32p, ctypes.c_int, ctypes.c_float, ctypes.c_float]
+_lib.tno_oracle_set_prf_table.restype = ctypes.c_int
+_lib.tno_oracle_set_prf_table.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+
+
 def _opt(a, shape):
     """Optional float32 array -> (keep-alive array, pointer or None)."""
     if a is None:
@@ -64,6 +71,22 @@ def _valid_ptr(valid, frames):
         return None
     assert valid.dtype == np.float32 and valid.flags.c_contiguous and valid.shape == frames.shape
     return valid.ctypes.data_as(_f32p)
+
+
+_f64c = ctypes.POINTER(ctypes.c_double)
+
+
+def _mode(shift_stack, filter, prf_table) -> int:
+    """Filter mode of tap1 in tno_oracle.c (0 point-sampled Gaussian, 1 shift-stack, 2 pixel-integrated
+    Gaussian, 3 tabulated); mode 3 installs `prf_table` ([n_phase, 5] fractions) first."""
+    mode = int(filter) if filter else int(bool(shift_stack))
+    assert mode in (0, 1, 2, 3)
+    if mode == 3:
+        tab = np.ascontiguousarray(prf_table, dtype=np.float64)
+        assert tab.ndim == 2 and tab.shape[1] == 5 and tab.shape[0] >= 1
+        rc = _lib.tno_oracle_set_prf_table(tab.ctypes.data_as(_f64c), int(tab.shape[0]))
+        assert rc == 0
+    return mode
 
 
 def threads() -> int:
@@ -88,7 +111,8 @@ def _geom(frames: np.ndarray, window, full_shape):
 
 
 def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=None,
-          times=None, jitter=None, valid=None, shift_stack: bool = False) -> Tuple[float, float, float]:
+          times=None, jitter=None, valid=None, shift_stack: bool = False, filter: int = 0,
+          prf_table=None) -> Tuple[float, float, float]:
     """(snr, N, D) at start pixel (x, y) for one trajectory (vx, vy, ax, ay).  times: frame times [T]
     (default the frame index), jitter: pointing offsets [T, 2] in px added to the track (default 0),
     valid: per-pixel weights of D with the layout of frames (default 1; N uses the frames as they are)."""
@@ -101,7 +125,8 @@ def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=No
     _ja, jp = _opt(jitter, (T, 2))
     rc = _lib.tno_oracle_point_ex(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
                                   sigma_t.ctypes.data_as(_f32p), tp, jp, _valid_ptr(valid, frames),
-                                  int(bool(shift_stack)), traj.ctypes.data_as(_f32p), float(prf_sigma), float(t0),
+                                  _mode(shift_stack, filter, prf_table), traj.ctypes.data_as(_f32p), float(prf_sigma),
+                                  float(t0),
                                   int(x), int(y),
                                   ctypes.byref(N), ctypes.byref(D), ctypes.byref(S))
     if rc != 0:
@@ -110,7 +135,8 @@ def point(frames, sigma_t, traj, prf_sigma, t0, x, y, window=None, full_shape=No
 
 
 def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, full_shape=None,
-            return_ND: bool = False, times=None, jitter=None, valid=None, shift_stack: bool = False):
+            return_ND: bool = False, times=None, jitter=None, valid=None, shift_stack: bool = False,
+            filter: int = 0, prf_table=None):
     """float64 [K, h, w] SNR for start pixels x in [x_lo, x_hi), y in [y_lo, y_hi)
     (region = (x_lo, x_hi, y_lo, y_hi), default the whole frame)."""
     frames = _f32(frames)
@@ -127,7 +153,7 @@ def snr_map(frames, sigma_t, trajs, prf_sigma, t0, region=None, window=None, ful
     _ja, jp = _opt(jitter, (T, 2))
     rc = _lib.tno_oracle_map_ex(frames.ctypes.data_as(_f32p), T, H, W, wx0, wy0, ww, wh,
                              sigma_t.ctypes.data_as(_f32p), tp, jp, _valid_ptr(valid, frames),
-                             int(bool(shift_stack)), trajs.ctypes.data_as(_f32p), K,
+                             _mode(shift_stack, filter, prf_table), trajs.ctypes.data_as(_f32p), K,
                              float(prf_sigma), float(t0), int(x_lo), int(x_hi), int(y_lo),
                              int(y_hi), out.ctypes.data_as(_f64p),
                              oN.ctypes.data_as(_f64p) if return_ND else None,
@@ -158,8 +184,10 @@ def topk(snr: np.ndarray, ktop: int, threshold: float, k_index: int = 0,
     return out
 
 
-def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0, times=None, jitter=None) -> None:
-    """In place: add amp * g(p - c_t) for each source (full-frame float32 [T, H, W] buffer)."""
+def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0, times=None, jitter=None, filter: int = 0,
+           prf_table=None) -> None:
+    """In place: add amp * g(p - c_t) for each source (full-frame float32 [T, H, W] buffer); g is the filter
+    of mode `filter` (0: the point-sampled Gaussian)."""
     assert frames.dtype == np.float32 and frames.flags.c_contiguous and frames.ndim == 3
     T, H, W = frames.shape
     trajs = _f32(trajs)
@@ -170,10 +198,17 @@ def inject(frames: np.ndarray, trajs, xs, ys, amps, prf_sigma, t0, times=None, j
     assert xs.shape == (n,) and ys.shape == (n,) and trajs.shape == (n, 4)
     _ta, tp = _opt(times, (T,))
     _ja, jp = _opt(jitter, (T, 2))
-    rc = _lib.tno_oracle_inject_ex(frames.ctypes.data_as(_f32p), T, H, W, tp, jp,
-                                trajs.ctypes.data_as(_f32p), xs.ctypes.data_as(_i32p),
-                                ys.ctypes.data_as(_i32p), amps.ctypes.data_as(_f32p), n,
-                                float(prf_sigma), float(t0))
+    if filter:
+        rc = _lib.tno_oracle_inject_mode(frames.ctypes.data_as(_f32p), T, H, W, tp, jp,
+                                         ctypes.c_int(_mode(False, filter, prf_table)),
+                                         trajs.ctypes.data_as(_f32p), xs.ctypes.data_as(_i32p),
+                                         ys.ctypes.data_as(_i32p), amps.ctypes.data_as(_f32p), n,
+                                         ctypes.c_float(prf_sigma), ctypes.c_float(t0))
+    else:
+        rc = _lib.tno_oracle_inject_ex(frames.ctypes.data_as(_f32p), T, H, W, tp, jp,
+                                       trajs.ctypes.data_as(_f32p), xs.ctypes.data_as(_i32p),
+                                       ys.ctypes.data_as(_i32p), amps.ctypes.data_as(_f32p), n,
+                                       float(prf_sigma), float(t0))
     assert rc == 0
 
 

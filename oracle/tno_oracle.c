@@ -69,12 +69,43 @@ static inline double disp(double v, double a, double dt) { return v * dt + a * d
  *                                            down-weighted them, F = R * valid)
  *     D = sum g^2 valid_t(p) / sigma_t^2    (a masked pixel carries no information)
  * valid has the layout of the frames (same window); NULL = all ones. */
-/* Filter of one axis at tap offset u = i - phase (reading g2): mode 0 = the Gaussian PRF
- * matched filter exp(-u^2 / (2 s^2)); mode 1 = shift-stack (after Rice & Laughlin 2020:
- * "a single non-zero value, set to 1, for each time-slice"): 1 at the rounded position (i = 0), else 0. */
+/* Filter of one axis at tap offset u = i - phase (readings g2, g3): the PRF as seen by the pixel grid.
+ *   mode 0  the point-sampled Gaussian of BASELINE.json:north_star, exp(-u^2 / (2 s^2));
+ *   mode 1  shift-stack (after Rice & Laughlin 2020: "a single non-zero value, set to 1, for
+ *           each time-slice"): 1 at the rounded position (i = 0), else 0;
+ *   mode 2  the pixel-integrated Gaussian: the flux of a unit source at sub-pixel phase `ph` that falls into
+ *           pixel i, the integral of the normalised Gaussian density over [i - 1/2, i + 1/2]
+ *           = Phi((u + 1/2) / s) - Phi((u - 1/2) / s)   (the PRF is the fraction of the flux
+ *           per pixel, "50 % in the peak pixel, 90 % in 2 x 2");
+ *   mode 3  a tabulated separable PRF: row floor((ph + 1/2) * n_phase) (clamped) of the table installed with
+ *           tno_oracle_set_prf_table, [n_phase][5] fractions for taps i = -2 .. 2, phases uniform over
+ *           [-1/2, 1/2).  The table is the ONE piece of global state of this file (test infrastructure). */
+static double *g_prf_table = NULL;
+static int g_prf_phases = 0;
+int tno_oracle_set_prf_table(const double *table, int n_phase) {
+    free(g_prf_table);
+    g_prf_table = NULL;
+    g_prf_phases = 0;
+    if (!table || n_phase <= 0) return 0;
+    g_prf_table = (double *)malloc(sizeof(double) * 5 * (size_t)n_phase);
+    if (!g_prf_table) return -2;
+    memcpy(g_prf_table, table, sizeof(double) * 5 * (size_t)n_phase);
+    g_prf_phases = n_phase;
+    return 0;
+}
 static inline double tap1(int mode, int i, double ph, double s) {
     if (mode == 1) return i == 0 ? 1.0 : 0.0;
     const double u = (double)i - ph;
+    if (mode == 2) {
+        const double r = 1.0 / (s * sqrt(2.0));
+        return 0.5 * (erf((u + 0.5) * r) - erf((u - 0.5) * r));
+    }
+    if (mode == 3) {
+        int row = (int)floor((ph + 0.5) * (double)g_prf_phases);
+        if (row < 0) row = 0;
+        if (row > g_prf_phases - 1) row = g_prf_phases - 1;
+        return g_prf_table[5 * row + (i + 2)];
+    }
     return exp(-(u * u) / (2.0 * s * s));
 }
 static inline double frame_dt(const float *times, int t, double t0) {
@@ -122,7 +153,7 @@ int tno_oracle_point_ex(const float *frames, int T, int H, int W,
                 if (px < 0 || px >= W || py < 0 || py >= H) continue;
                 if (px < wx0 || px >= wx0 + ww || py < wy0 || py >= wy0 + wh) return -1;
                 const double ux = (double)i - phx, uy = (double)j - phy;
-                const double g = mode == 1 ? tap1(1, i, phx, s) * tap1(1, j, phy, s)
+                const double g = mode != 0 ? tap1(mode, i, phx, s) * tap1(mode, j, phy, s)
                                            : exp(-(ux * ux + uy * uy) / (2.0 * s * s));
                 const size_t idx = ((size_t)t * wh + (size_t)(py - wy0)) * ww + (size_t)(px - wx0);
                 const double R = frames[idx];
@@ -263,6 +294,35 @@ int tno_oracle_inject_ex(float *frames, int T, int H, int W, const float *times,
                     if (px < 0 || px >= W || py < 0 || py >= H) continue;
                     const double ux = (double)i - phx, uy = (double)j - phy;
                     const double g = exp(-(ux * ux + uy * uy) / (2.0 * s * s));
+                    float *p = frames + ((size_t)t * H + (size_t)py) * W + (size_t)px;
+                    *p = (float)((double)*p + A * g);
+                }
+            }
+        }
+    }
+    return 0;
+}
+
+/* The same with the per-axis filter of `mode` (tap1): the source as modes 1-3 see it. */
+int tno_oracle_inject_mode(float *frames, int T, int H, int W, const float *times, const float *jitter, int mode,
+                         const float *traj, const int *xs, const int *ys, const float *amp, int n,
+                         float prf_sigma_f, float t0_f)
+{
+    const double s = prf_sigma_f, t0 = t0_f;
+    for (int m = 0; m < n; ++m) {
+        const double vx = traj[4 * m + 0], vy = traj[4 * m + 1];
+        const double ax = traj[4 * m + 2], ay = traj[4 * m + 3];
+        const double A = amp[m];
+        for (int t = 0; t < T; ++t) {
+            const double dt = frame_dt(times, t, t0);
+            int sx, sy; double phx, phy;
+            split(disp(vx, ax, dt) + jit(jitter, t, 0), &sx, &phx);
+            split(disp(vy, ay, dt) + jit(jitter, t, 1), &sy, &phy);
+            for (int j = -2; j <= 2; ++j) {
+                for (int i = -2; i <= 2; ++i) {
+                    const int px = xs[m] + sx + i, py = ys[m] + sy + j;
+                    if (px < 0 || px >= W || py < 0 || py >= H) continue;
+                    const double g = tap1(mode, i, phx, s) * tap1(mode, j, phy, s);
                     float *p = frames + ((size_t)t * H + (size_t)py) * W + (size_t)px;
                     *p = (float)((double)*p + A * g);
                 }
