@@ -78,11 +78,16 @@ typedef struct {
                                 method of PAPER.md:L118 (Rice & Laughlin 2020 "use a single non-zero value, set to 1,
                                 for each time-slice"): the filter is 1 at round(c_t) and 0 elsewhere,
                                 N = sum R_t(round(c_t))/sigma_t^2, D = sum [in frame]/sigma_t^2; prf_sigma is ignored
-                                by the search (tno_mf_inject still renders with the PRF) */
+                                by the search (tno_mf_inject still renders with the PRF);
+                                2 = pixel-integrated Gaussian PRF: the tap of pixel i is the flux fraction a source
+                                at sub-pixel phase ph puts into it, Phi((i-ph+1/2)/prf_sigma) - Phi((i-ph-1/2)/prf_sigma)
+                                per axis (PAPER.md:L41 describes the PRF by such fractions: ~50 % in the peak pixel);
+                                3 = tabulated separable PRF, see tno_mf_set_prf_table; prf_sigma is ignored.
+                                In modes 2 and 3 tno_mf_inject renders sources with the same taps. */
 } tno_mf_config;
 
 /* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
- * workspace_limit_mb < 0, filter not 0 or 1), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
+ * workspace_limit_mb < 0, filter not 0 .. 3), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
 int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
 
 /* The search (formula above).
@@ -162,6 +167,15 @@ int tno_mf_search_host(tno_mf_ctx *ctx,
                        float prf_sigma, float t0,
                        float *out_snr_host,
                        tno_mf_cand *out_topk_host);
+
+/* Tabulated separable PRF for filter 3: `table` is HOST float32
+ * [n_phase][5], row r = the fractions of the flux that fall into the pixels -2 .. +2 around the rounded
+ * position for a source whose sub-pixel phase ph = c - round(c) lies in [-1/2 + r/n_phase, -1/2 + (r+1)/n_phase);
+ * the search and tno_mf_inject use row floor((ph + 1/2) * n_phase) for x and for y (nearest tabulated phase, no
+ * interpolation), the 2-D filter is the outer product.  Values must be finite and >= 0.  The table is copied;
+ * n_phase = 0 removes it.  A context with filter 3 and no table fails its searches with EINVAL.
+ * Errors: EINVAL, ENOMEM, ECUDA. */
+int tno_mf_set_prf_table(tno_mf_ctx *ctx, const float *table, int32_t n_phase);
 
 /* Signal injection ("signal injection corresponds to adding a filter times a flux
  * to the raw data"): for each source m in order and every frame t,

@@ -64,6 +64,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
+    lib.tno_mf_set_prf_table.restype = i32
+    lib.tno_mf_set_prf_table.argtypes = [vp, vp, i32]
     lib.tno_mf_plan.restype = ctypes.c_int
     lib.tno_mf_plan.argtypes = [vp, i32, i32, f32, i32, i32, vp, vp]
     lib.tno_mf_last_stats.restype = ctypes.c_int
@@ -99,12 +101,13 @@ def tno_mf_last_error(ctx=None) -> str:
 
 def tno_mf_create(device: int = 0, stream: Optional[int] = None, topk: int = 0,
                   snr_threshold: float = float("-inf"), force_generic: bool = False,
-                  record_events: bool = False, workspace_limit_mb: int = 0, shift_stack: bool = False):
+                  record_events: bool = False, workspace_limit_mb: int = 0, shift_stack: bool = False,
+                  filter: int = 0):
     """Returns an opaque context handle.  `stream` is a raw cudaStream_t (int) or None."""
     cfg = tno_mf_config(device=int(device), stream=ctypes.c_void_p(stream or 0), topk=int(topk),
                         snr_threshold=float(snr_threshold), force_generic=int(bool(force_generic)),
                         record_events=int(bool(record_events)), workspace_limit_mb=int(workspace_limit_mb),
-                        filter=int(bool(shift_stack)))
+                        filter=int(filter) if filter else int(bool(shift_stack)))
     ctx = ctypes.c_void_p()
     _check(_lib.tno_mf_create(ctypes.byref(cfg), ctypes.byref(ctx)), None)
     return ctx
@@ -255,6 +258,17 @@ def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float)
     src = np.ascontiguousarray(sources, dtype=SOURCE_DTYPE)
     _check(_lib.tno_mf_inject(ctx, frames.data_ptr(), T, H, W, src.ctypes.data, src.shape[0],
                               float(prf_sigma), float(t0)), ctx)
+
+
+def tno_mf_set_prf_table(ctx, table) -> None:
+    """table: [n_phase, 5] flux fractions (host array) for filter 3; None or an empty table removes it."""
+    if table is None or len(table) == 0:
+        _check(_lib.tno_mf_set_prf_table(ctx, None, 0), ctx)
+        return
+    tab = np.ascontiguousarray(table, dtype=np.float32)
+    if tab.ndim != 2 or tab.shape[1] != 5:
+        raise ValueError("prf table must have shape [n_phase, 5]")
+    _check(_lib.tno_mf_set_prf_table(ctx, tab.ctypes.data, tab.shape[0]), ctx)
 
 
 def tno_mf_plan(trajectories, T: int, t0: float, max_entries: int, max_spread: int

@@ -39,7 +39,8 @@ struct tno_mf_ctx {
     float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
     const float *down_dev = nullptr;
     int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
-    DevBuf stack, hmaps, htopk, bgq;
+    DevBuf stack, hmaps, htopk, bgq, prf_tab;
+    int32_t prf_phases = 0;          // rows of prf_tab (tno_mf_set_prf_table), 0 = none
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
     const TrajInfo *s_ti = nullptr;
@@ -190,8 +191,8 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
     if (std::isnan(cfg->snr_threshold))
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
-    if (cfg->filter < 0 || cfg->filter > 1 || cfg->workspace_limit_mb < 0)
-        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 or 1 and workspace_limit_mb >= 0");
+    if (cfg->filter < 0 || cfg->filter > 3 || cfg->workspace_limit_mb < 0)
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 .. 3 and workspace_limit_mb >= 0");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess || n_dev == 0) {
@@ -251,7 +252,7 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
                       &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
-                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq};
+                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq, &ctx->prf_tab};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -292,6 +293,26 @@ int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, floa
     return (int)plan.batches.size();
 }
 
+int tno_mf_set_prf_table(tno_mf_ctx *ctx, const float *table, int32_t n_phase) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (n_phase < 0 || n_phase > (1 << 20) || (n_phase > 0 && !table))
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_set_prf_table: n_phase must be in [0, 2^20] and table non-NULL");
+    for (int64_t i = 0; i < (int64_t)n_phase * 5; ++i)
+        if (!finite_f(table[i]) || table[i] < 0.f)
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_set_prf_table: table[%lld] is negative or not finite", (long long)i);
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    ctx->prf_phases = 0;
+    if (n_phase == 0) return TNO_MF_OK;
+    int rc = reserve(ctx, ctx->prf_tab, (size_t)n_phase * 5 * sizeof(float));
+    if (rc) return rc;
+    // the caller's buffer may go away after the call
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->prf_tab.p, table, (size_t)n_phase * 5 * sizeof(float), cudaMemcpyHostToDevice,
+                                ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->prf_phases = n_phase;
+    return TNO_MF_OK;
+}
+
 int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W,
                   const tno_mf_source *sources, int32_t n_sources, float prf_sigma, float t0) {
     if (!ctx) return TNO_MF_EINVAL;
@@ -299,6 +320,8 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: NULL pointer or non-positive size");
     if (!(prf_sigma > 0.f) || !finite_f(prf_sigma) || !finite_f(t0))
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: prf_sigma must be finite and > 0, t0 finite");
+    if (ctx->cfg.filter == 3 && ctx->prf_phases == 0)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: filter 3 needs a table (tno_mf_set_prf_table)");
     if (n_sources == 0) return TNO_MF_OK;
     std::vector<SourceDev> host(n_sources);
     for (int32_t m = 0; m < n_sources; ++m) {
@@ -314,7 +337,8 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
     CU_TRY(ctx, cudaMemcpyAsync(ctx->src.p, host.data(), host.size() * sizeof(SourceDev),
                                 cudaMemcpyHostToDevice, ctx->stream));
     launch_inject(ctx->stream, frames, T, H, W, static_cast<const SourceDev *>(ctx->src.p), n_sources,
-                  (double)prf_sigma, (double)t0);
+                  (double)prf_sigma, (double)t0, ctx->cfg.filter, static_cast<const float *>(ctx->prf_tab.p),
+                  ctx->prf_phases);
     CU_TRY(ctx, cudaGetLastError());
     return TNO_MF_OK;
 }
@@ -487,6 +511,8 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: H*W must not exceed 2^31 pixels");
     if (!(prf_sigma > 0.f) || !finite_f(prf_sigma))
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: prf_sigma must be finite and > 0");
+    if (ctx->cfg.filter == 3 && ctx->prf_phases == 0)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: filter 3 needs a table (tno_mf_set_prf_table)");
     if (!finite_f(t0)) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: t0 must be finite");
     const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
     if (!out_snr && !want_topk)
@@ -682,7 +708,8 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
     launch_class_tables(st, reinterpret_cast<const float *>(meta + o_v), reinterpret_cast<const float *>(meta + o_a),
                         frame_times ? reinterpret_cast<const float *>(meta + o_tm) : nullptr,
                         jitter_xy ? reinterpret_cast<const float *>(meta + o_jt) : nullptr,
-                        n_cls, n_x, T, (double)t0, (double)prf_sigma, ctx->cfg.filter, static_cast<int32_t *>(ctx->shift.p),
+                        n_cls, n_x, T, (double)t0, (double)prf_sigma, ctx->cfg.filter,
+                        static_cast<const float *>(ctx->prf_tab.p), ctx->prf_phases, static_cast<int32_t *>(ctx->shift.p),
                         static_cast<float *>(ctx->g.p), static_cast<double *>(ctx->gd.p));
     launch_border_tables(st, tab.shift, tab.gd, tab.qd, reinterpret_cast<const AxisBorder *>(meta + o_bd), d_off,
                          n_cls, n_x, max_n, T, W, H, static_cast<double *>(ctx->ab.p));

@@ -77,4 +77,23 @@ struct TopkSlots {
     float threshold;
 };
 
+// Filter of one axis at tap i (0 .. 4, offset i - 2 from the rounded position) for sub-pixel phase ph in
+// [-1/2, 1/2): tno_mf_config::filter (include/tno_mf.h) -- 0 point-sampled Gaussian, 1 shift-stack single tap,
+// 2 pixel-integrated Gaussian (the flux fraction per pixel), 3 tabulated (row of the phase).
+__device__ __forceinline__ double prf_tap(int32_t filter, int i, double ph, double prf_sigma,
+                                          const float *__restrict__ prf_tab, int32_t n_phase) {
+    if (filter == 1) return i == 2 ? 1.0 : 0.0;
+    const double u = (double)(i - 2) - ph;
+    if (filter == 2) {
+        const double r = 1.0 / (prf_sigma * sqrt(2.0));
+        return 0.5 * (erf((u + 0.5) * r) - erf((u - 0.5) * r));
+    }
+    if (filter == 3) {
+        int32_t row = (int32_t)floor((ph + 0.5) * (double)n_phase);
+        row = row < 0 ? 0 : (row > n_phase - 1 ? n_phase - 1 : row);
+        return (double)prf_tab[5 * row + i];
+    }
+    return exp(-(u * u) / (2.0 * prf_sigma * prf_sigma));
+}
+
 }  // namespace tno

@@ -14,7 +14,7 @@ __device__ __forceinline__ void axis_pos(double v, double a, double dt, int32_t 
 
 __global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32_t W,
                          const SourceDev *__restrict__ src, int32_t n_src, double prf_sigma,
-                         double t0) {
+                         double t0, int32_t filter, const float *__restrict__ prf_tab, int32_t n_phase) {
     const int32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= T) return;
     const double dt = (double)t - t0;
@@ -33,7 +33,11 @@ __global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32
                 const int32_t px = s.x + sx + i;
                 if (px < 0 || px >= W) continue;
                 const double ux = (double)i - phx, uy = (double)j - phy;
-                const double g = exp(-(ux * ux + uy * uy) * inv);
+                // filters 2 and 3 render the source with their own (separable) PRF; 0 and 1 with the
+                // point-sampled Gaussian (shift-stack is a way to search, not a PRF)
+                const double g = filter >= 2 ? prf_tap(filter, i + 2, phx, prf_sigma, prf_tab, n_phase) *
+                                                   prf_tap(filter, j + 2, phy, prf_sigma, prf_tab, n_phase)
+                                             : exp(-(ux * ux + uy * uy) * inv);
                 float *p = f + (int64_t)py * W + px;
                 *p = (float)((double)*p + (double)s.amp * g);
             }
@@ -42,8 +46,10 @@ __global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32
 }
 
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,
-                   const SourceDev *src, int32_t n_src, double prf_sigma, double t0) {
-    k_inject<<<(unsigned)((T + 63) / 64), 64, 0, st>>>(frames, T, H, W, src, n_src, prf_sigma, t0);
+                   const SourceDev *src, int32_t n_src, double prf_sigma, double t0, int32_t filter,
+                   const float *prf_tab, int32_t n_phase) {
+    k_inject<<<(unsigned)((T + 63) / 64), 64, 0, st>>>(frames, T, H, W, src, n_src, prf_sigma, t0, filter, prf_tab,
+                                                       n_phase);
 }
 
 }  // namespace tno

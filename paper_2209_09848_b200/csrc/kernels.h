@@ -11,8 +11,8 @@ namespace tno {
 void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a,
                          const float *times /* DEVICE [T] or NULL */, const float *jitter /* DEVICE [T][2] or NULL */,
                          int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma,
-                         int32_t filter /* 0 = Gaussian PRF taps, 1 = shift-stack single tap */, int32_t *shift,
-                         float *g, double *gd);
+                         int32_t filter /* tno_mf_config::filter */, const float *prf_tab /* DEVICE [n_phase][5] */,
+                         int32_t n_phase, int32_t *shift, float *g, double *gd);
 void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,
                           const AxisBorder *border, const int64_t *off, int32_t n_cls, int32_t n_x,
                           int32_t max_n, int32_t T, int32_t W, int32_t H, double *out);
@@ -55,7 +55,8 @@ void launch_background(cudaStream_t st, const float *frames, int32_t T, int64_t 
 // ---- inject.cu ----
 struct SourceDev { float vx, vy, ax, ay; int32_t x, y; float amp; };
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,
-                   const SourceDev *src, int32_t n_src, double prf_sigma, double t0);
+                   const SourceDev *src, int32_t n_src, double prf_sigma, double t0, int32_t filter,
+                   const float *prf_tab, int32_t n_phase);
 
 // ---- search_sep.cu ----
 struct SepVariant {

@@ -12,6 +12,7 @@ namespace tno {
 __global__ void k_class_tables(const float *__restrict__ cls_v, const float *__restrict__ cls_a,
                                const float *__restrict__ times, const float *__restrict__ jitter,
                                int32_t n_cls, int32_t n_x, int32_t T, double t0, double prf_sigma, int32_t filter,
+                               const float *__restrict__ prf_tab, int32_t n_phase,
                                int32_t *__restrict__ shift, float *__restrict__ g,
                                double *__restrict__ gd) {
     const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -30,8 +31,9 @@ __global__ void k_class_tables(const float *__restrict__ cls_v, const float *__r
 #pragma unroll
     for (int i = 0; i < 5; ++i) {
         const double u = (double)(i - 2) - ph;
-        // filter 1 = shift-stack: a single tap of weight 1 at the rounded position
-        const double w = filter == 1 ? (i == 2 ? 1.0 : 0.0) : exp(-(u * u) * inv);
+        // filter 0: the expression the first version of this kernel had (bit-compatible tables);
+        // 1 shift-stack, 2 pixel-integrated Gaussian, 3 tabulated: prf_tap (common.cuh)
+        const double w = filter == 0 ? exp(-(u * u) * inv) : prf_tap(filter, i, ph, prf_sigma, prf_tab, n_phase);
         g[id * 5 + i] = (float)w;
         gd[id * 5 + i] = w;
     }
@@ -76,10 +78,11 @@ __global__ void k_rsd_tables(const TrajInfo *__restrict__ traj, const double *__
 
 void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a, const float *times,
                          const float *jitter, int32_t n_cls, int32_t n_x, int32_t T, double t0,
-                         double prf_sigma, int32_t filter, int32_t *shift, float *g, double *gd) {
+                         double prf_sigma, int32_t filter, const float *prf_tab, int32_t n_phase, int32_t *shift,
+                         float *g, double *gd) {
     const int64_t n = (int64_t)n_cls * T;
     k_class_tables<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cls_v, cls_a, times, jitter, n_cls, n_x, T,
-                                                                 t0, prf_sigma, filter, shift, g, gd);
+                                                                 t0, prf_sigma, filter, prf_tab, n_phase, shift, g, gd);
 }
 
 void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,

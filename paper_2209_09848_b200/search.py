@@ -13,14 +13,18 @@ class MatchedFilter:
 
     def __init__(self, device: int = 0, topk: int = 0, snr_threshold: float = float("-inf"),
                  force_generic: bool = False, record_events: bool = False, workspace_limit_mb: int = 0,
-                 shift_stack: bool = False):
+                 shift_stack: bool = False, filter: int = 0, prf_table=None):
+        """filter: tno_mf_config::filter (0 Gaussian PRF, 1 shift-stack, 2 pixel-integrated Gaussian, 3 tabulated:
+        prf_table [n_phase, 5])."""
         import torch
         self._torch = torch
         self.device = torch.device("cuda", device)
         self.topk = int(topk)
         stream = torch.cuda.current_stream(self.device).cuda_stream
         self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events,
-                                   workspace_limit_mb, shift_stack)
+                                   workspace_limit_mb, shift_stack, filter)
+        if prf_table is not None:
+            B.tno_mf_set_prf_table(self.ctx, prf_table)
 
     def close(self) -> None:
         if self.ctx is not None:
