@@ -249,6 +249,28 @@ def local_z(m, box: int = 255, literal: bool = False):
     return z, s
 
 
+def peaks(score, radius: int, threshold: float = -np.inf):
+    """Non-maximum suppression of a score map [H, W] (SURVEY 8(f) rank 1: "so one object yields one candidate";
+    DESIGN.md reading e4): pixel p is a peak iff score(p) >= threshold and, for every other pixel q of the frame
+    with |qx - px| <= radius and |qy - py| <= radius, score(p) > score(q), or score(p) == score(q) and p comes
+    first in row-major order.  Returns the boolean peak mask.  Written as the definition, one window offset at
+    a time (numpy float64)."""
+    z = np.asarray(score, dtype=np.float64)
+    H, W = z.shape
+    r = int(radius)
+    keep = z >= threshold
+    pad = np.full((H + 2 * r, W + 2 * r), -np.inf)
+    pad[r:r + H, r:r + W] = z
+    for dy in range(-r, r + 1):
+        for dx in range(-r, r + 1):
+            if dy == 0 and dx == 0:
+                continue
+            q = pad[r + dy:r + dy + H, r + dx:r + dx + W]          # score of the neighbour at offset (dx, dy)
+            q_is_later = dy > 0 or (dy == 0 and dx > 0)
+            keep &= (z > q) | ((z == q) & q_is_later)
+    return keep
+
+
 # ---- high-resolution background model (PAPER.md section 3.1, L66-100) ---------------------------
 def background_basis(jitter) -> np.ndarray:
     """[T, 6] float64 basis (1, x, y, x^2, y^2, x y) of the per-pixel model of PAPER.md Eq. 1: the background
