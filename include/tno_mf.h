@@ -206,6 +206,21 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
 int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, int32_t box,
                 float *out_max, int32_t *out_argk, float *out_z, tno_mf_cand *out_topk);
 
+/* Non-maximum suppression of a score map, "so one object yields one candidate" (the paper
+ * lists every score above 3 sigma as a candidate, L124, and one object lights up a neighbourhood):
+ * pixel p is a peak iff score(p) >= cfg.snr_threshold and for every other pixel q of the frame with
+ * |qx - px| <= radius and |qy - py| <= radius: score(p) > score(q), or score(p) == score(q) and p precedes q
+ * in row-major order (of equal neighbours the first one survives).
+ *   score      DEVICE float32 [H][W], e.g. out_z or out_max of tno_mf_best.  Read only.
+ *   argk       DEVICE int32 [H][W] (out_argk of tno_mf_best) or NULL: fills record.k (else 0).
+ *   radius     0 .. 1024 px (0: every pixel above the threshold is a peak).
+ *   out_peaks  DEVICE float32 [H][W]: score at the peaks, -INFINITY elsewhere; or NULL.  Must not alias score.
+ *   out_topk   DEVICE [topk] records of the highest peaks, ordered (score descending, y, x ascending), unused
+ *              tail {-INFINITY, -1, -1, -1}; or NULL (or topk == 0).
+ * Errors: EINVAL, ENOMEM, ECUDA. */
+int tno_mf_peaks(tno_mf_ctx *ctx, const float *score, const int32_t *argk, int32_t H, int32_t W, int32_t radius,
+                 float *out_peaks, tno_mf_cand *out_topk);
+
 /* Flux estimate (the score "is a direct estimate of the total flux due to that moving
  * object, which allows to not only estimate the position and trajectory of a detection, but also the
  * magnitude"): the maximum-likelihood amplitude of a source on trajectory k starting at (x, y),

@@ -251,7 +251,7 @@ def local_z(m, box: int = 255, literal: bool = False):
 
 def peaks(score, radius: int, threshold: float = -np.inf):
     """Non-maximum suppression of a score map [H, W] (SURVEY 8(f) rank 1: "so one object yields one candidate";
-    DESIGN.md reading e4): pixel p is a peak iff score(p) >= threshold and, for every other pixel q of the frame
+    DESIGN.md reading e6): pixel p is a peak iff score(p) >= threshold and, for every other pixel q of the frame
     with |qx - px| <= radius and |qy - py| <= radius, score(p) > score(q), or score(p) == score(q) and p comes
     first in row-major order.  Returns the boolean peak mask.  Written as the definition, one window offset at
     a time (numpy float64)."""

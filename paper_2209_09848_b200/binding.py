@@ -64,6 +64,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
+    lib.tno_mf_peaks.restype = i32
+    lib.tno_mf_peaks.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     lib.tno_mf_set_prf_table.restype = i32
     lib.tno_mf_set_prf_table.argtypes = [vp, vp, i32]
     lib.tno_mf_plan.restype = ctypes.c_int
@@ -258,6 +260,19 @@ def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float)
     src = np.ascontiguousarray(sources, dtype=SOURCE_DTYPE)
     _check(_lib.tno_mf_inject(ctx, frames.data_ptr(), T, H, W, src.ctypes.data, src.shape[0],
                               float(prf_sigma), float(t0)), ctx)
+
+
+def tno_mf_peaks(ctx, score, argk, radius: int, out_peaks, out_topk) -> None:
+    """score: CUDA float32 [H, W]; argk: CUDA int32 [H, W] or None; out_peaks: CUDA float32 [H, W] or None;
+    out_topk: CUDA int32 [topk, 4] or None."""
+    assert score.is_cuda and score.is_contiguous() and score.dim() == 2 and score.element_size() == 4
+    H, W = score.shape
+    for t in (argk, out_peaks):
+        assert t is None or (t.is_cuda and t.is_contiguous() and tuple(t.shape) == (H, W) and t.element_size() == 4)
+    assert out_topk is None or (out_topk.is_cuda and out_topk.is_contiguous())
+    _check(_lib.tno_mf_peaks(ctx, score.data_ptr(), argk.data_ptr() if argk is not None else None, H, W, int(radius),
+                             out_peaks.data_ptr() if out_peaks is not None else None,
+                             out_topk.data_ptr() if out_topk is not None else None), ctx)
 
 
 def tno_mf_set_prf_table(ctx, table) -> None:

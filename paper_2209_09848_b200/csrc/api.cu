@@ -1,4 +1,5 @@
 // C ABI of libtno_mf.so (include/tno_mf.h): context, validation, planning, launches.
+#include <cfloat>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -387,6 +388,51 @@ int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
             launch_topk_merge(st, slots, (int32_t)n_tiles, W, out_topk);
             launch_set_argk(st, out_topk, ctx->cfg.topk, argk, W);
             ctx->last_launches += 3;
+        }
+    }
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
+}
+
+int tno_mf_peaks(tno_mf_ctx *ctx, const float *score, const int32_t *argk, int32_t H, int32_t W, int32_t radius,
+                 float *out_peaks, tno_mf_cand *out_topk) {
+    if (!ctx) return TNO_MF_EINVAL;
+    ctx->last_launches = 0;
+    if (!score) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: NULL score map");
+    if (H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 31)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: H, W must be >= 1 and H*W <= 2^31");
+    if (radius < 0 || radius > 1024) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: radius must be in [0, 1024]");
+    const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
+    if (!out_peaks && !want_topk) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: no output requested");
+    if (out_peaks == score) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: out_peaks must not alias score");
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = ctx->stream;
+    int rc;
+    float *pk = out_peaks;
+    if (!pk) {
+        if ((rc = reserve(ctx, ctx->ztmp, (size_t)H * W * 4))) return rc;
+        pk = static_cast<float *>(ctx->ztmp.p);
+        if (pk == score) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: score is the context's scratch map");
+    }
+    launch_nms(st, score, H, W, radius, ctx->cfg.snr_threshold, pk);
+    ctx->last_launches += 1;
+    if (want_topk) {
+        const int32_t ntx = (W + kCollectTile - 1) / kCollectTile, nty = (H + kCollectTile - 1) / kCollectTile;
+        const int64_t n_tiles = (int64_t)ntx * nty;
+        if ((rc = reserve(ctx, ctx->keys, (size_t)n_tiles * ctx->cfg.topk * 8))) return rc;
+        if ((rc = reserve(ctx, ctx->counts, (size_t)n_tiles * 4))) return rc;
+        TopkSlots slots;
+        slots.keys = static_cast<uint64_t *>(ctx->keys.p);
+        slots.counts = static_cast<int32_t *>(ctx->counts.p);
+        slots.ktop = ctx->cfg.topk;
+        slots.K = 1;
+        slots.threshold = std::max(ctx->cfg.snr_threshold, -FLT_MAX);      // never the -inf of a suppressed pixel
+        launch_collect_from_map(st, pk, H, W, 0, 1, slots);
+        launch_topk_merge(st, slots, (int32_t)n_tiles, W, out_topk);
+        ctx->last_launches += 2;
+        if (argk) {
+            launch_set_argk(st, out_topk, ctx->cfg.topk, argk, W);
+            ctx->last_launches += 1;
         }
     }
     CU_TRY(ctx, cudaGetLastError());

@@ -151,6 +151,34 @@ k_flux(const float *__restrict__ snr, const TrajInfo *__restrict__ traj, const f
     out[i] = snr[i] * r;
 }
 
+// Non-maximum suppression (reading e6): out = score where the pixel is >= thr and
+// beats every other pixel of its (2r+1)^2 window (larger score, or equal score and earlier in row-major order),
+// -inf elsewhere.  Only pixels above the threshold scan their window, and they stop at the first loss.
+__global__ void __launch_bounds__(256)
+k_nms(const float *__restrict__ score, int32_t H, int32_t W, int32_t r, float thr, float *__restrict__ out) {
+    const int32_t x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
+    if (x >= W || y >= H) return;
+    const float s = score[(int64_t)y * W + x];
+    bool keep = s >= thr;
+    if (keep) {
+        const int32_t x0 = max(0, x - r), x1 = min(W - 1, x + r), y0 = max(0, y - r), y1 = min(H - 1, y + r);
+        for (int32_t yy = y0; yy <= y1 && keep; ++yy) {
+            const float *row = score + (int64_t)yy * W;
+            for (int32_t xx = x0; xx <= x1; ++xx) {
+                const float q = __ldg(row + xx);
+                const bool earlier = yy < y || (yy == y && xx < x);
+                if (q > s || (q == s && earlier)) { keep = false; break; }
+            }
+        }
+    }
+    out[(int64_t)y * W + x] = keep ? s : -INFINITY;
+}
+
+void launch_nms(cudaStream_t st, const float *score, int32_t H, int32_t W, int32_t radius, float thr, float *out) {
+    dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4));
+    k_nms<<<grid, 256, 0, st>>>(score, H, W, radius, thr, out);
+}
+
 void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const float *rsd, int32_t K, int32_t H,
                  int32_t W, float *out) {
     dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)K);

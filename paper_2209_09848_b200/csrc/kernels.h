@@ -44,6 +44,7 @@ void launch_local_z(cudaStream_t st, const float *m, int32_t H, int32_t W, int32
 // out[k][y][x] = snr[k][y][x] * D_k(x, y)^(-1/2)  (flux estimate N / D)
 void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const float *rsd, int32_t K, int32_t H,
                  int32_t W, float *out);
+void launch_nms(cudaStream_t st, const float *score, int32_t H, int32_t W, int32_t radius, float thr, float *out);
 void launch_set_argk(cudaStream_t st, tno_mf_cand *cand, int32_t n, const int32_t *argk, int32_t W);
 
 // ---- background.cu ---- (section 3.1: per-pixel Huber fit on the jitter basis)

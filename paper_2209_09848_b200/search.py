@@ -102,6 +102,15 @@ class MatchedFilter:
         B.tno_mf_best(self.ctx, snr, box, mx, ak, z, top)
         return mx, ak, z, top
 
+    def peaks(self, score, radius: int, argk=None):
+        """Non-maximum suppression of a score map [H, W] (e.g. Z of best()): (map with the score at the peaks and
+        -inf elsewhere, top-K records of the peaks or None); asynchronous."""
+        torch = self._torch
+        out = torch.empty_like(score)
+        top = torch.empty((self.topk, 4), dtype=torch.int32, device=score.device) if self.topk > 0 else None
+        B.tno_mf_peaks(self.ctx, score, argk, radius, out, top)
+        return out, top
+
     def inject(self, frames, trajs, xs, ys, amps, prf_sigma: float, t0: float) -> None:
         B.tno_mf_inject(self.ctx, frames, B.make_sources(trajs, xs, ys, amps), prf_sigma, t0)
 
