@@ -321,6 +321,16 @@ def run_ours(args, cfg):
             ms = timed(lambda: mf.best(out_snr))
             extras["best"] = {"ms": ms, "bytes": out_snr.numel() * 4, "what": "max over trajectories, local-sigma Z "
                               "(255 box), top-K of Z"}
+            mx, ak, z, _ = mf.best(out_snr)
+            ms = timed(lambda: mf.peaks(z, 5, ak))
+            extras["peaks"] = {"ms": ms, "what": "non-maximum suppression of Z, radius 5, threshold %g, top-K" % cfg.threshold}
+            mxf = torch.empty_like(mx)
+            akf = torch.empty_like(ak)
+            from paper_2209_09848_b200 import tno_mf_search_max
+            ms = timed(lambda: tno_mf_search_max(mf.ctx, frames, None, p.sigma_t, None, None, p.traj, cfg.prf_sigma,
+                                                 cfg.t0, mxf, akf, out_snr, out_topk), reps=2)
+            extras["search_max"] = {"ms": ms, "what": "the timed search with the max over the bank fused in",
+                                    "equals_best": bool(torch.equal(mxf, mx) and torch.equal(akf, ak))}
             ms = timed(lambda: mf.flux(out_snr))
             gb = 2.0 * out_snr.numel() * 4 / 1e9
             extras["flux"] = {"ms": ms, "achieved_gbs": gb / ms * 1e3, "peak_gbs": hbm}

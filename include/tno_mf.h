@@ -206,6 +206,21 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
 int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, int32_t box,
                 float *out_max, int32_t *out_argk, float *out_z, tno_mf_cand *out_topk);
 
+/* The search with the max over the filter bank fused into its epilogue ("We take
+ * the maximum score across the filter bank, which then tells us the most likely trajectory, along with the score
+ * of that trajectory"): everything tno_mf_search_masked does, plus
+ *   out_max    DEVICE float32 [H][W]   M(x, y) = max_k SNR_k(x, y)               (required)
+ *   out_argk   DEVICE int32   [H][W]   the smallest k that attains it, or NULL
+ * -- bit for bit what tno_mf_best computes from out_snr, without the maps having to exist: out_snr and out_topk
+ * may both be NULL (a bank of 1024 trajectories on 2048^2 then needs no 17 GB of maps).  valid, frame_times and
+ * jitter_xy may be NULL as in the other searches.  Z and the peaks follow with tno_mf_best(out_max as a bank of
+ * one map) and tno_mf_peaks(Z, out_argk).  The running maximum lives in a 64-bit key per pixel (8 * H * W bytes of
+ * workspace), updated with atomicMax: order independent, hence reproducible.  Errors as tno_mf_search_masked. */
+int tno_mf_search_max(tno_mf_ctx *ctx, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                      const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                      const tno_mf_traj *trajectories, int32_t n_traj, float prf_sigma, float t0,
+                      float *out_max, int32_t *out_argk, float *out_snr, tno_mf_cand *out_topk);
+
 /* Non-maximum suppression of a score map, "so one object yields one candidate" (the paper
  * lists every score above 3 sigma as a candidate, L124, and one object lights up a neighbourhood):
  * pixel p is a peak iff score(p) >= cfg.snr_threshold and for every other pixel q of the frame with

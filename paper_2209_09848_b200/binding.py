@@ -55,6 +55,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_search_masked.restype = ctypes.c_int
     lib.tno_mf_search_masked.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_search_host.restype = ctypes.c_int
+    lib.tno_mf_search_max.restype = i32
+    lib.tno_mf_search_max.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp, vp, vp]
     lib.tno_mf_search_host.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
     lib.tno_mf_background.restype = ctypes.c_int
     lib.tno_mf_background.argtypes = [vp, vp, i32, i32, i32, vp, f32, i32, vp, vp]
@@ -142,8 +144,20 @@ def tno_mf_search_masked(ctx, frames, valid, sigma_t, frame_times, jitter_xy, tr
                      _valid=valid)
 
 
+def tno_mf_search_max(ctx, frames, valid, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
+                      out_max, out_argk=None, out_snr=None, out_topk=None) -> None:
+    """The search with the max over the bank fused in: out_max CUDA float32 [H, W] (required), out_argk CUDA int32
+    [H, W] or None; valid, out_snr, out_topk optional."""
+    T, H, W = frames.shape
+    assert out_max.is_cuda and out_max.is_contiguous() and tuple(out_max.shape) == (H, W) and out_max.element_size() == 4
+    assert out_argk is None or (out_argk.is_cuda and out_argk.is_contiguous() and tuple(out_argk.shape) == (H, W)
+                                and out_argk.element_size() == 4)
+    tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma, t0, out_snr, out_topk,
+                     _valid=valid, _max=(out_max, out_argk))
+
+
 def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
-                     out_snr=None, out_topk=None, _plain: bool = False, _valid=None) -> None:
+                     out_snr=None, out_topk=None, _plain: bool = False, _valid=None, _max=None) -> None:
     """tno_mf_search with frame times (host float32 [T] or None) and pointing jitter (host float32
     [T, 2] px or None) in the track."""
     assert frames.is_cuda and frames.dtype.is_floating_point and frames.element_size() == 4
@@ -175,6 +189,13 @@ def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories,
     if _valid is not None:
         assert _valid.is_cuda and _valid.is_contiguous() and _valid.shape == frames.shape
         assert _valid.element_size() == 4 and _valid.dtype.is_floating_point
+    if _max is not None:
+        rc = _lib.tno_mf_search_max(ctx, frames.data_ptr(), _valid.data_ptr() if _valid is not None else None, T, H, W,
+                                    sig.ctypes.data, tm.ctypes.data if tm is not None else None,
+                                    jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,
+                                    float(prf_sigma), float(t0), _max[0].data_ptr(),
+                                    _max[1].data_ptr() if _max[1] is not None else None, p_snr, p_top)
+    elif _valid is not None:
         rc = _lib.tno_mf_search_masked(ctx, frames.data_ptr(), _valid.data_ptr(), T, H, W, sig.ctypes.data,
                                        tm.ctypes.data if tm is not None else None,
                                        jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,

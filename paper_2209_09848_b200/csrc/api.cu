@@ -40,7 +40,7 @@ struct tno_mf_ctx {
     float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
     const float *down_dev = nullptr;
     int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
-    DevBuf stack, hmaps, htopk, bgq, prf_tab;
+    DevBuf stack, hmaps, htopk, bgq, prf_tab, maxkeys;
     int32_t prf_phases = 0;          // rows of prf_tab (tno_mf_set_prf_table), 0 = none
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
@@ -253,7 +253,7 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
                       &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
-                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq, &ctx->prf_tab};
+                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq, &ctx->prf_tab, &ctx->maxkeys};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -539,10 +539,12 @@ int tno_mf_search_ex(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H,
                                 prf_sigma, t0, out_snr, out_topk);
 }
 
-int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
-                         const float *sigma_t, const float *frame_times, const float *jitter_xy,
-                         const tno_mf_traj *trajectories, int32_t n_traj,
-                         float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
+// The search proper; out_max / out_argk (tno_mf_search_max) may be NULL.
+static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                       const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                       const tno_mf_traj *trajectories, int32_t n_traj,
+                       float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk, float *out_max,
+                       int32_t *out_argk) {
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
     ctx->s_ti = nullptr;
@@ -561,8 +563,9 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: filter 3 needs a table (tno_mf_set_prf_table)");
     if (!finite_f(t0)) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: t0 must be finite");
     const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
-    if (!out_snr && !want_topk)
+    if (!out_snr && !want_topk && !out_max)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: no output requested (out_snr NULL and no top-K)");
+    if (out_argk && !out_max) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_max: out_argk needs out_max");
     for (int32_t t = 0; t < T; ++t)
         if (!(sigma_t[t] > 0.f) || !finite_f(sigma_t[t]))
             return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: sigma_t[%d] must be finite and > 0", t);
@@ -770,6 +773,13 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
     slots.K = n_traj;
     slots.threshold = ctx->cfg.snr_threshold;
 
+    uint64_t *mk = nullptr;                  // running (score, ~k) maximum per pixel, 0 = below every score
+    if (out_max) {
+        if ((rc = reserve(ctx, ctx->maxkeys, (size_t)map_px * 8))) return rc;
+        mk = static_cast<uint64_t *>(ctx->maxkeys.p);
+        CU_TRY(ctx, cudaMemsetAsync(mk, 0, (size_t)map_px * 8, st));
+    }
+
     // ------------------------------------------------------------------ search
     if (use_sep) {
         const size_t tab_floats = (size_t)n_batches * T * sep_table_words(variant);
@@ -830,7 +840,7 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
                         if (fy1 > fin_tiles) {
                             launch_finish(st, static_cast<const float *>(ctx->pieces.p), nullptr, n_pieces, a.piece_stride,
                                           reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W,
-                                          fin_tiles, fy1, out_snr, slots);
+                                          fin_tiles, fy1, out_snr, mk, slots);
                             ctx->last_launches += 1;
                             fin_tiles = fy1;
                             if ((rc = download_rows(ctx, fy1 * kCollectTile))) return rc;
@@ -841,7 +851,7 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
             const float *np_ = static_cast<const float *>(ctx->pieces.p);
             launch_finish(st, np_, valid ? np_ + pass_floats : nullptr, n_pieces, a.piece_stride,
                           reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W, fin_tiles, nfy,
-                          out_snr, slots);
+                          out_snr, mk, slots);
             CU_TRY(ctx, cudaGetLastError());
             ctx->last_launches += 2 + n_pass;              // memset, search(es), finish
             b0 = b1;
@@ -876,6 +886,10 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
                 launch_collect_from_map(st, dst, H, W, k0, kc, slots);
                 ctx->last_launches += 1;
             }
+            if (mk) {
+                launch_max_keys_from_maps(st, dst, k0, kc, map_px, mk);
+                ctx->last_launches += 1;
+            }
         }
         if ((rc = record_event(ctx))) return rc;
         CU_TRY(ctx, cudaGetLastError());
@@ -885,9 +899,32 @@ int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *vali
         ctx->last_launches += 1;
         CU_TRY(ctx, cudaGetLastError());
     }
+    if (mk) {
+        launch_max_decode(st, mk, map_px, out_max, out_argk);
+        ctx->last_launches += 1;
+        CU_TRY(ctx, cudaGetLastError());
+    }
     ctx->s_traj = n_traj; ctx->s_H = H; ctx->s_W = W;
     ctx->s_ti = valid ? nullptr : d_ti;                // tno_mf_flux needs the analytic D tables
     return TNO_MF_OK;
+}
+
+int tno_mf_search_masked(tno_mf_ctx *ctx, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                         const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                         const tno_mf_traj *trajectories, int32_t n_traj,
+                         float prf_sigma, float t0, float *out_snr, tno_mf_cand *out_topk) {
+    return search_core(ctx, frames, valid, T, H, W, sigma_t, frame_times, jitter_xy, trajectories, n_traj, prf_sigma, t0,
+                       out_snr, out_topk, nullptr, nullptr);
+}
+
+int tno_mf_search_max(tno_mf_ctx *ctx, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                      const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                      const tno_mf_traj *trajectories, int32_t n_traj, float prf_sigma, float t0,
+                      float *out_max, int32_t *out_argk, float *out_snr, tno_mf_cand *out_topk) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (!out_max) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_max: NULL out_max");
+    return search_core(ctx, frames, valid, T, H, W, sigma_t, frame_times, jitter_xy, trajectories, n_traj, prf_sigma, t0,
+                       out_snr, out_topk, out_max, out_argk);
 }
 
 int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int32_t H, int32_t W,

@@ -151,6 +151,41 @@ k_flux(const float *__restrict__ snr, const TrajInfo *__restrict__ traj, const f
     out[i] = snr[i] * r;
 }
 
+// Max over the bank fused into the search (tno_mf_search_max): the search keeps, per pixel, the maximum of the keys
+// (score order << 32 | ~k) -- k_finish with atomicMax, the generic path with this kernel on its map chunks.
+__global__ void __launch_bounds__(256)
+k_max_keys_from_maps(const float *__restrict__ maps, int32_t k0, int32_t kc, int64_t n_px,
+                     unsigned long long *__restrict__ keys) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_px) return;
+    unsigned long long best = keys[i];
+    for (int32_t k = 0; k < kc; ++k) {
+        const unsigned long long key = make_key(maps[(int64_t)k * n_px + i], (uint32_t)(k0 + k));
+        best = key > best ? key : best;
+    }
+    keys[i] = best;
+}
+
+__global__ void __launch_bounds__(256)
+k_max_decode(const unsigned long long *__restrict__ keys, int64_t n_px, float *__restrict__ out_max,
+             int32_t *__restrict__ out_argk) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_px) return;
+    const unsigned long long key = keys[i];
+    out_max[i] = ord_to_snr((uint32_t)(key >> 32));
+    if (out_argk) out_argk[i] = (int32_t)(~(uint32_t)key);
+}
+
+void launch_max_keys_from_maps(cudaStream_t st, const float *maps, int32_t k0, int32_t kc, int64_t n_px, uint64_t *keys) {
+    k_max_keys_from_maps<<<(unsigned)((n_px + 255) / 256), 256, 0, st>>>(maps, k0, kc, n_px,
+                                                                        reinterpret_cast<unsigned long long *>(keys));
+}
+
+void launch_max_decode(cudaStream_t st, const uint64_t *keys, int64_t n_px, float *out_max, int32_t *out_argk) {
+    k_max_decode<<<(unsigned)((n_px + 255) / 256), 256, 0, st>>>(reinterpret_cast<const unsigned long long *>(keys),
+                                                                n_px, out_max, out_argk);
+}
+
 // Non-maximum suppression (reading e6): out = score where the pixel is >= thr and
 // beats every other pixel of its (2r+1)^2 window (larger score, or equal score and earlier in row-major order),
 // -inf elsewhere.  Only pixels above the threshold scan their window, and they stop at the first loss.

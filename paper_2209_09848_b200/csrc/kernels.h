@@ -44,6 +44,9 @@ void launch_local_z(cudaStream_t st, const float *m, int32_t H, int32_t W, int32
 // out[k][y][x] = snr[k][y][x] * D_k(x, y)^(-1/2)  (flux estimate N / D)
 void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const float *rsd, int32_t K, int32_t H,
                  int32_t W, float *out);
+// running maximum over the bank as 64-bit keys (score order << 32 | ~k): update from materialised maps, decode
+void launch_max_keys_from_maps(cudaStream_t st, const float *maps, int32_t k0, int32_t kc, int64_t n_px, uint64_t *keys);
+void launch_max_decode(cudaStream_t st, const uint64_t *keys, int64_t n_px, float *out_max, int32_t *out_argk);
 void launch_nms(cudaStream_t st, const float *score, int32_t H, int32_t W, int32_t radius, float thr, float *out);
 void launch_set_argk(cudaStream_t st, tno_mf_cand *cand, int32_t n, const int32_t *argk, int32_t W);
 
@@ -95,6 +98,7 @@ int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode
 void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
                    int32_t H, int32_t W, int32_t fy0, int32_t fy1 /* rows of 64 x 64 tiles [fy0, fy1) */,
-                   float *out_snr, const TopkSlots &slots);
+                   float *out_snr, uint64_t *maxkeys /* DEVICE [H][W] running (score, ~k) maximum, or NULL */,
+                   const TopkSlots &slots);
 
 }  // namespace tno

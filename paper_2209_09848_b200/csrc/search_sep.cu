@@ -453,7 +453,7 @@ __global__ void __launch_bounds__(256)
 k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, int32_t n_pieces, int64_t piece_stride,
          const int32_t *__restrict__ perm, int32_t q0, const TrajInfo *__restrict__ traj,
          const float *__restrict__ rsd, int32_t H, int32_t W, int32_t fy0, float *__restrict__ out_snr,
-         TopkSlots slots) {
+         unsigned long long *__restrict__ maxkeys, TopkSlots slots) {
     __shared__ uint64_t list[kCollectTile * kCollectTile];
     __shared__ int32_t count;
     const int32_t tid = threadIdx.x, lane = tid & 31;
@@ -504,6 +504,14 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
                 v.w *= __ldg(rr + border_class(x + 3, ti.bx, W));
             }
             if (om) *reinterpret_cast<float4 *>(om + off) = v;
+            if (maxkeys) {
+                // fused max over the bank: key = (score, ~k), so the maximum of the keys is
+                // the largest score and, of equal scores, the smallest k -- order independent, hence exact
+                atomicMax(maxkeys + off, make_key(v.x, (uint32_t)k));
+                atomicMax(maxkeys + off + 1, make_key(v.y, (uint32_t)k));
+                atomicMax(maxkeys + off + 2, make_key(v.z, (uint32_t)k));
+                atomicMax(maxkeys + off + 3, make_key(v.w, (uint32_t)k));
+            }
         }
         if (want_topk) {
             const uint32_t pix = (uint32_t)(y * W + x);
@@ -598,10 +606,11 @@ int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode
 
 void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
-                   int32_t H, int32_t W, int32_t fy0, int32_t fy1, float *out_snr, const TopkSlots &slots) {
+                   int32_t H, int32_t W, int32_t fy0, int32_t fy1, float *out_snr, uint64_t *maxkeys,
+                   const TopkSlots &slots) {
     dim3 grid((unsigned)((W + kCollectTile - 1) / kCollectTile), (unsigned)(fy1 - fy0), (unsigned)q_count);
     k_finish<<<grid, 256, 0, st>>>(pieces, dpieces, n_pieces, piece_stride, perm, q0, traj, rsd, H, W, fy0, out_snr,
-                                   slots);
+                                   reinterpret_cast<unsigned long long *>(maxkeys), slots);
 }
 
 }  // namespace tno

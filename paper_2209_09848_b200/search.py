@@ -69,6 +69,21 @@ class MatchedFilter:
                                out_snr if want_maps else None, out_topk if self.topk > 0 else None)
         return (out_snr if want_maps else None), (out_topk if self.topk > 0 else None)
 
+    def search_max(self, frames, sigma_t, trajectories, prf_sigma: float, t0: float, want_maps: bool = False,
+                   frame_times=None, jitter_xy=None, valid=None):
+        """The search with the max over the bank fused in: (max map [H, W], arg-max trajectory
+        [H, W], snr maps or None, candidate tensor or None); asynchronous."""
+        torch = self._torch
+        n = np.asarray(trajectories).shape[0]
+        T, H, W = frames.shape
+        mx = torch.empty((H, W), dtype=torch.float32, device=frames.device)
+        ak = torch.empty((H, W), dtype=torch.int32, device=frames.device)
+        snr = torch.empty((n, H, W), dtype=torch.float32, device=frames.device) if want_maps else None
+        top = torch.empty((n, self.topk, 4), dtype=torch.int32, device=frames.device) if self.topk > 0 else None
+        B.tno_mf_search_max(self.ctx, frames, valid, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma, t0,
+                            mx, ak, snr, top)
+        return mx, ak, snr, top
+
     def search_host(self, frames_host, sigma_t, trajectories, prf_sigma: float, t0: float, out_snr_host=None,
                     out_topk_host=None, frame_times=None, jitter_xy=None) -> None:
         """Stack and outputs in HOST memory (torch CPU tensors, pinned for overlap, or numpy arrays); the
