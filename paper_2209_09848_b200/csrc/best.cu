@@ -139,16 +139,28 @@ __global__ void k_set_argk(tno_mf_cand *__restrict__ cand, int32_t n, const int3
 // Flux estimate A = N / D = SNR * D^(-1/2) per trajectory and start pixel (the score "is a
 // direct estimate of the total flux due to that moving object ... but also the magnitude"), from the SNR
 // maps and the D^(-1/2) tables of the search that produced them.
+// VEC: four neighbouring pixels per thread (16-byte loads and stores; needs W % 4 == 0 and aligned pointers)
+template <bool VEC>
 __global__ void __launch_bounds__(256)
 k_flux(const float *__restrict__ snr, const TrajInfo *__restrict__ traj, const float *__restrict__ rsd,
        int32_t H, int32_t W, float *__restrict__ out) {
-    const int32_t x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
+    constexpr int PX = VEC ? 4 : 1;
+    const int32_t x = (blockIdx.x * 64 + (threadIdx.x & 63)) * PX, y = blockIdx.y * 4 + (threadIdx.x >> 6);
     const int32_t k = blockIdx.z;
     if (x >= W || y >= H) return;
     const TrajInfo ti = traj[k];
-    const float r = __ldg(rsd + ti.rsd_off + (int64_t)border_class(y, ti.by, H) * ti.bx.n + border_class(x, ti.bx, W));
+    const float *rr = rsd + ti.rsd_off + (int64_t)border_class(y, ti.by, H) * ti.bx.n;
     const int64_t i = ((int64_t)k * H + y) * W + x;
-    out[i] = snr[i] * r;
+    if (VEC) {
+        float4 v = __ldcs(reinterpret_cast<const float4 *>(snr + i));
+        v.x *= __ldg(rr + border_class(x, ti.bx, W));
+        v.y *= __ldg(rr + border_class(x + 1, ti.bx, W));
+        v.z *= __ldg(rr + border_class(x + 2, ti.bx, W));
+        v.w *= __ldg(rr + border_class(x + 3, ti.bx, W));
+        __stcs(reinterpret_cast<float4 *>(out + i), v);
+    } else {
+        out[i] = snr[i] * __ldg(rr + border_class(x, ti.bx, W));
+    }
 }
 
 // Max over the bank fused into the search (tno_mf_search_max): the search keeps, per pixel, the maximum of the keys
@@ -216,8 +228,14 @@ void launch_nms(cudaStream_t st, const float *score, int32_t H, int32_t W, int32
 
 void launch_flux(cudaStream_t st, const float *snr, const TrajInfo *traj, const float *rsd, int32_t K, int32_t H,
                  int32_t W, float *out) {
-    dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)K);
-    k_flux<<<grid, 256, 0, st>>>(snr, traj, rsd, H, W, out);
+    const bool vec = W % 4 == 0 && ((reinterpret_cast<uintptr_t>(snr) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0;
+    if (vec) {
+        dim3 grid((unsigned)((W / 4 + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)K);
+        k_flux<true><<<grid, 256, 0, st>>>(snr, traj, rsd, H, W, out);
+    } else {
+        dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)K);
+        k_flux<false><<<grid, 256, 0, st>>>(snr, traj, rsd, H, W, out);
+    }
 }
 
 void launch_max_map(cudaStream_t st, const float *snr, int32_t K, int32_t H, int32_t W, float *out_max,
