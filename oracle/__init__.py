@@ -299,3 +299,80 @@ def background(frames, jitter, delta: float, n_iter: int):
         beta = beta + pinv @ np.clip(r, -d, d)
     r = Y - phi @ beta
     return beta.reshape(6, H, W), r.reshape(T, H, W)
+
+
+# ---- low-resolution scattered-light model (PAPER.md section 3.1, Eq. 1-4, L66-96) ------------------------------
+def bilinear_matrix(n_out: int, n_in: int) -> np.ndarray:
+    """[n_out, n_in] matrix of 1-D bilinear upsampling (reading s2): output pixel i has its centre at
+    u = (i + 1/2) n_in / n_out - 1/2 in input pixel units, clamped to [0, n_in - 1]; it is the weighted
+    combination of the two nearest input pixels, floor(u) with weight 1 - frac(u) and floor(u) + 1 (clamped) with
+    weight frac(u) -- "the high resolution pixel is weighted combination of the 4 nearest low resolution points"
+     in two dimensions."""
+    A = np.zeros((n_out, n_in))
+    for i in range(n_out):
+        u = min(max((i + 0.5) * n_in / n_out - 0.5, 0.0), n_in - 1.0)
+        i0 = int(np.floor(u))
+        i1 = min(i0 + 1, n_in - 1)
+        w = u - i0
+        A[i, i0] += 1.0 - w
+        A[i, i1] += w
+    return A
+
+
+def upsample(S, N: int) -> np.ndarray:
+    """U(S): [..., n, n] -> [..., N, N], bilinear in both axes (Eq. 1)."""
+    S = np.asarray(S, dtype=np.float64)
+    A = bilinear_matrix(N, S.shape[-1])
+    return np.einsum("ia,...ab,jb->...ij", A, S, A)
+
+
+def huber(a, delta):
+    """Eq. 4 with the lost bar restored: a^2 / 2 for |a| <= delta, delta (|a| - delta / 2) otherwise."""
+    a = np.abs(a)
+    return np.where(a <= delta, 0.5 * a * a, delta * (a - 0.5 * delta))
+
+
+def scatter_loss_grad(D, jitter_xy, delta, beta, S):
+    """Loss of Eq. 2-3 and its gradient for the low-resolution model of Eq. 1,
+         pred_t = U(S_t) + sum_k phi_k(theta_t) beta_k,   L = sum_{t,i,j} L_delta(D_t - pred_t),
+    phi = (1, x, y, x^2, y^2, x y) (background_basis), beta [6, N, N], S [T, n, n].
+    Returns (L, dL/dbeta [6, N, N], dL/dS [T, n, n]) in float64: dL/dpred = -clip(r, -delta, delta), pushed
+    through the transposes of the two linear maps."""
+    D = np.asarray(D, dtype=np.float64)
+    T, N, _ = D.shape
+    phi = background_basis(jitter_xy)
+    beta = np.asarray(beta, dtype=np.float64)
+    S = np.asarray(S, dtype=np.float64)
+    r = D - (upsample(S, N) + np.einsum("tk,kij->tij", phi, beta))
+    L = float(huber(r, delta).sum())
+    psi = np.clip(r, -delta, delta)
+    A = bilinear_matrix(N, S.shape[-1])
+    g_beta = -np.einsum("tk,tij->kij", phi, psi)
+    g_S = -np.einsum("ia,tij,jb->tab", A, psi, A)
+    return L, g_beta, g_S
+
+
+def scatter_fit(D, jitter_xy, delta, n: int, max_iter: int = 500, gtol: float = 1e-8):
+    """Minimise the loss over (beta, S) with L-BFGS from zero ("We minimize this convex loss over
+    B, B_theta, S_t using the L-BFGS (Zhu et al. 1995) algorithm"): scipy's L-BFGS-B, the implementation of that
+    paper, serves as the step.  Returns (beta, S, loss).  The split of a time-constant smooth component between S
+    and B is not determined by the loss; the prediction and the loss are."""
+    import scipy.optimize
+    D = np.asarray(D, dtype=np.float64)
+    T, N, _ = D.shape
+    nb = 6 * N * N
+
+    def fun(x):
+        L, gb, gs = scatter_loss_grad(D, jitter_xy, delta, x[:nb].reshape(6, N, N), x[nb:].reshape(T, n, n))
+        return L, np.concatenate([gb.ravel(), gs.ravel()])
+    res = scipy.optimize.minimize(fun, np.zeros(nb + T * n * n), jac=True, method="L-BFGS-B",
+                                  options={"maxiter": max_iter, "gtol": gtol, "ftol": 0.0, "maxcor": 10,
+                                           "maxfun": 10 * max_iter})
+    return res.x[:nb].reshape(6, N, N), res.x[nb:].reshape(T, n, n), float(res.fun)
+
+
+def downsample(frames, f: int) -> np.ndarray:
+    """Mean over f x f blocks: "the data downsampled to 512 x 512 from 2048 x 2048" (reading s1)."""
+    a = np.asarray(frames, dtype=np.float64)
+    T, H, W = a.shape
+    return a.reshape(T, H // f, f, W // f, f).mean(axis=(2, 4))
