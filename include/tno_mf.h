@@ -267,6 +267,42 @@ int tno_mf_flux(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
 int tno_mf_background(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W,
                       const float *jitter_xy, float delta, int32_t n_iter, float *out_coef, float *out_resid);
 
+/* Low-resolution scattered-light model (section 3.1, Eq. 1-4, second part):
+ *     D_t = U(S_t) + B + B_theta . (x_t, y_t, x_t^2, y_t^2, x_t y_t) + eps_t,      L = sum_{t,i,j} L_delta(D_t - pred_t)
+ * with D the data downsampled to N x N ("N = 512"), S_t an n x n image per frame ("n = 64"), U bilinear upsampling
+ * (output pixel i has its centre at (i + 1/2) n / N - 1/2 input pixels, clamped to [0, n - 1], and takes the two
+ * nearest input pixels per axis: "the 4 nearest low resolution points"), L_delta the Huber loss of Eq. 4.
+ * "We minimize this convex loss over B, B_theta, S_t using the L-BFGS algorithm" (L94).
+ *   D          DEVICE float32 [T][N][N].           jitter_xy  HOST float32 [T][2], px.        delta > 0.
+ *   beta       DEVICE float32 [6][N][N]: B, then the coefficients of x, y, x^2, y^2, xy.
+ *   S          DEVICE float32 [T][n][n].
+ * tno_mf_scatter_lossgrad evaluates L (float64, written to HOST *out_loss) and its gradient (DEVICE g_beta
+ * [6][N][N], g_S [T][n][n]) at (beta, S); it returns after the loss has arrived.
+ * tno_mf_scatter_fit runs L-BFGS (10 pairs, Armijo backtracking) from the (beta, S) it is given -- zeros are the
+ * paper's "regardless of the initial parameters" -- and overwrites them with the minimiser; it stops when
+ * max_i |g_i| <= gtol, after max_iter iterations, when two consecutive iterations each decrease the loss by less
+ * than 1e-9 of its value, or when no step decreases it at all (float32 resolution), and reports the
+ * final loss, the iterations and the loss evaluations (HOST, each may be NULL).  Blocking.  The loss and the
+ * prediction are determined by the data; the split of a time-constant smooth component between S and B is not.
+ * Workspace: about 26 vectors of 6 N^2 + T n^2 floats and one [T][N][N] stack.  Errors: EINVAL, ENOMEM, ECUDA. */
+int tno_mf_scatter_lossgrad(tno_mf_ctx *ctx, const float *D, int32_t T, int32_t N, int32_t n, const float *jitter_xy,
+                            float delta, const float *beta, const float *S, double *out_loss, float *g_beta,
+                            float *g_S);
+int tno_mf_scatter_fit(tno_mf_ctx *ctx, const float *D, int32_t T, int32_t N, int32_t n, const float *jitter_xy,
+                       float delta, int32_t max_iter, float gtol, float *beta, float *S, double *out_loss,
+                       int32_t *out_iters, int32_t *out_evals);
+
+/* The two ends of that solve.  tno_mf_downsample: out[t][y][x] = mean of the factor x factor block of frames
+ * ("the data downsampled to 512 x 512 from 2048 x 2048", L69); frames DEVICE [T][H][W], out DEVICE
+ * [T][H/factor][W/factor], factor divides H and W.  tno_mf_scatter_subtract: frames[t] -= U(S_t) with U from
+ * n x n to H x W (same bilinear rule), in place -- the stack that tno_mf_background expects ("Once we solve for
+ * scattered light S_t at low resolution, we hold it fixed, and re-estimate B, B_theta at high resolution", L98).
+ * T <= 65535.  Asynchronous on the context's stream.  Errors: EINVAL, ECUDA. */
+int tno_mf_downsample(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W, int32_t factor,
+                      float *out);
+int tno_mf_scatter_subtract(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W, const float *S,
+                            int32_t n);
+
 /* Host-only planning query (no device work; ctx may be NULL): how the search would group
  * `trajectories` into batches that share one x-motion (vx, ax) -- the unit of work of the
  * separable kernel.  Writes, for each trajectory, its batch index and slot

@@ -66,6 +66,16 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
+    f64p = ctypes.POINTER(ctypes.c_double)
+    i32p = ctypes.POINTER(i32)
+    lib.tno_mf_scatter_lossgrad.restype = i32
+    lib.tno_mf_scatter_lossgrad.argtypes = [vp, vp, i32, i32, i32, vp, f32, vp, vp, f64p, vp, vp]
+    lib.tno_mf_scatter_fit.restype = i32
+    lib.tno_mf_scatter_fit.argtypes = [vp, vp, i32, i32, i32, vp, f32, i32, f32, vp, vp, f64p, i32p, i32p]
+    lib.tno_mf_downsample.restype = i32
+    lib.tno_mf_downsample.argtypes = [vp, vp, i32, i32, i32, i32, vp]
+    lib.tno_mf_scatter_subtract.restype = i32
+    lib.tno_mf_scatter_subtract.argtypes = [vp, vp, i32, i32, i32, vp, i32]
     lib.tno_mf_peaks.restype = i32
     lib.tno_mf_peaks.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     lib.tno_mf_set_prf_table.restype = i32
@@ -281,6 +291,55 @@ def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float)
     src = np.ascontiguousarray(sources, dtype=SOURCE_DTYPE)
     _check(_lib.tno_mf_inject(ctx, frames.data_ptr(), T, H, W, src.ctypes.data, src.shape[0],
                               float(prf_sigma), float(t0)), ctx)
+
+
+def _dev3(t, shape=None):
+    assert t.is_cuda and t.is_contiguous() and t.dim() == 3 and t.element_size() == 4 and t.dtype.is_floating_point
+    assert shape is None or tuple(t.shape) == tuple(shape), (tuple(t.shape), shape)
+    return t.data_ptr()
+
+
+def _jitter(jitter_xy, T):
+    jt = np.ascontiguousarray(jitter_xy, dtype=np.float32)
+    if jt.shape != (T, 2):
+        raise ValueError("jitter_xy must have shape [T, 2]")
+    return jt
+
+
+def tno_mf_scatter_lossgrad(ctx, D, jitter_xy, delta: float, beta, S, g_beta, g_S) -> float:
+    """D [T, N, N], beta / g_beta [6, N, N], S / g_S [T, n, n]: CUDA float32 tensors.  Returns the loss."""
+    T, N, _ = D.shape
+    n = S.shape[-1]
+    jt = _jitter(jitter_xy, T)
+    loss = ctypes.c_double()
+    _check(_lib.tno_mf_scatter_lossgrad(ctx, _dev3(D, (T, N, N)), T, N, n, jt.ctypes.data, float(delta),
+                                        _dev3(beta, (6, N, N)), _dev3(S, (T, n, n)), ctypes.byref(loss),
+                                        _dev3(g_beta, (6, N, N)), _dev3(g_S, (T, n, n))), ctx)
+    return loss.value
+
+
+def tno_mf_scatter_fit(ctx, D, jitter_xy, delta: float, max_iter: int, gtol: float, beta, S) -> Tuple[float, int, int]:
+    """L-BFGS from (beta, S), overwritten with the minimiser.  Returns (loss, iterations, loss evaluations)."""
+    T, N, _ = D.shape
+    n = S.shape[-1]
+    jt = _jitter(jitter_xy, T)
+    loss, iters, evals = ctypes.c_double(), ctypes.c_int32(), ctypes.c_int32()
+    _check(_lib.tno_mf_scatter_fit(ctx, _dev3(D, (T, N, N)), T, N, n, jt.ctypes.data, float(delta), int(max_iter),
+                                   float(gtol), _dev3(beta, (6, N, N)), _dev3(S, (T, n, n)), ctypes.byref(loss),
+                                   ctypes.byref(iters), ctypes.byref(evals)), ctx)
+    return loss.value, iters.value, evals.value
+
+
+def tno_mf_downsample(ctx, frames, factor: int, out) -> None:
+    T, H, W = frames.shape
+    _check(_lib.tno_mf_downsample(ctx, _dev3(frames), T, H, W, int(factor),
+                                  _dev3(out, (T, H // factor, W // factor))), ctx)
+
+
+def tno_mf_scatter_subtract(ctx, frames, S) -> None:
+    T, H, W = frames.shape
+    n = S.shape[-1]
+    _check(_lib.tno_mf_scatter_subtract(ctx, _dev3(frames), T, H, W, _dev3(S, (T, n, n)), n), ctx)
 
 
 def tno_mf_peaks(ctx, score, argk, radius: int, out_peaks, out_topk) -> None:

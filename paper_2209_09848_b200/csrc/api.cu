@@ -40,7 +40,7 @@ struct tno_mf_ctx {
     float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
     const float *down_dev = nullptr;
     int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
-    DevBuf stack, hmaps, htopk, bgq, prf_tab, maxkeys;
+    DevBuf stack, hmaps, htopk, bgq, prf_tab, maxkeys, scat;
     int32_t prf_phases = 0;          // rows of prf_tab (tno_mf_set_prf_table), 0 = none
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
@@ -253,7 +253,7 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
                       &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
-                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq, &ctx->prf_tab, &ctx->maxkeys};
+                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq, &ctx->prf_tab, &ctx->maxkeys, &ctx->scat};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -292,6 +292,130 @@ int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, floa
             if (out_slot) out_slot[plan.batches[b].traj[s]] = (int32_t)s;
         }
     return (int)plan.batches.size();
+}
+
+// ---- low-resolution scattered-light model (section 3.1) -------------------------------------------------
+static int scatter_setup(tno_mf_ctx *ctx, const char *who, const float *D, int32_t T, int32_t N, int32_t n,
+                         const float *jitter_xy, float delta, const float *beta, const float *S, size_t extra_bytes,
+                         ScatterProblem *pb, unsigned char **ws) {
+    if (!D || !jitter_xy || !beta || !S) return fail(ctx, TNO_MF_EINVAL, "%s: NULL pointer", who);
+    if (T < 1 || N < 1 || n < 1 || n > N || (int64_t)T * N * N > ((int64_t)1 << 40))
+        return fail(ctx, TNO_MF_EINVAL, "%s: need T >= 1 and 1 <= n <= N", who);
+    if (!(delta > 0.f) || std::isnan(delta)) return fail(ctx, TNO_MF_EINVAL, "%s: delta must be > 0", who);
+    std::vector<float> phi((size_t)T * 8, 0.f);
+    for (int32_t t = 0; t < T; ++t) {
+        const double x = jitter_xy[2 * t], y = jitter_xy[2 * t + 1];
+        if (!finite_f(jitter_xy[2 * t]) || !finite_f(jitter_xy[2 * t + 1]))
+            return fail(ctx, TNO_MF_EINVAL, "%s: jitter_xy[%d] is not finite", who, t);
+        float *row = &phi[(size_t)t * 8];
+        row[0] = 1.f; row[1] = (float)x; row[2] = (float)y; row[3] = (float)(x * x); row[4] = (float)(y * y);
+        row[5] = (float)(x * y);
+    }
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc;
+    // one upload: phi [T][8] floats, then the bilinear table (first input pixel [N] int32, weight [N] float)
+    const size_t phi_words = (size_t)T * 8;
+    std::vector<int32_t> head(phi_words + 2 * (size_t)N + 2 * (size_t)n);
+    std::memcpy(head.data(), phi.data(), phi_words * 4);
+    int32_t *hi0 = head.data() + phi_words, *hlo = hi0 + 2 * (size_t)N, *hhi = hlo + n;
+    bilinear_table(N, n, hi0, reinterpret_cast<float *>(hi0 + N));
+    for (int32_t b = 0; b < n; ++b) { hlo[b] = N; hhi[b] = -1; }
+    for (int32_t i = 0; i < N; ++i)
+        for (int32_t b : {hi0[i], std::min(hi0[i] + 1, n - 1)}) {
+            hlo[b] = std::min(hlo[b], i);
+            hhi[b] = std::max(hhi[b], i);
+        }
+    const size_t phi_bytes = (head.size() * 4 + 255) & ~(size_t)255;
+    if ((rc = reserve(ctx, ctx->scat, phi_bytes + extra_bytes))) return rc;
+    unsigned char *base = static_cast<unsigned char *>(ctx->scat.p);
+    CU_TRY(ctx, cudaMemcpyAsync(base, head.data(), head.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));      // head is a local buffer
+    pb->D = D; pb->T = T; pb->N = N; pb->n = n; pb->phi = reinterpret_cast<const float *>(base); pb->delta = delta;
+    pb->bi0 = reinterpret_cast<const int32_t *>(base) + phi_words;
+    pb->bw = reinterpret_cast<const float *>(base) + phi_words + N;
+    pb->blo = pb->bi0 + 2 * (size_t)N;
+    pb->bhi = pb->blo + n;
+    *ws = base + phi_bytes;
+    return TNO_MF_OK;
+}
+
+int tno_mf_scatter_lossgrad(tno_mf_ctx *ctx, const float *D, int32_t T, int32_t N, int32_t n, const float *jitter_xy,
+                            float delta, const float *beta, const float *S, double *out_loss, float *g_beta,
+                            float *g_S) {
+    if (!ctx) return TNO_MF_EINVAL;
+    ctx->last_launches = 0;
+    if (!out_loss || !g_beta || !g_S) return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_lossgrad: NULL output");
+    ScatterProblem pb;
+    unsigned char *ws = nullptr;
+    const size_t blocks = std::max<size_t>(1024, ((size_t)N * N + 255) / 256);
+    const size_t psi_bytes = ((size_t)T * N * N * 4 + 255) & ~(size_t)255;
+    int rc = scatter_setup(ctx, "tno_mf_scatter_lossgrad", D, T, N, n, jitter_xy, delta, beta, S,
+                           psi_bytes + (blocks + 8) * 8, &pb, &ws);
+    if (rc) return rc;
+    double *partials = reinterpret_cast<double *>(ws + psi_bytes);
+    ctx->last_launches = scatter_lossgrad(ctx->stream, pb, beta, S, reinterpret_cast<float *>(ws), partials, g_beta, g_S,
+                                          partials + blocks);
+    CU_TRY(ctx, cudaMemcpyAsync(out_loss, partials + blocks, 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
+}
+
+int tno_mf_scatter_fit(tno_mf_ctx *ctx, const float *D, int32_t T, int32_t N, int32_t n, const float *jitter_xy,
+                       float delta, int32_t max_iter, float gtol, float *beta, float *S, double *out_loss,
+                       int32_t *out_iters, int32_t *out_evals) {
+    if (!ctx) return TNO_MF_EINVAL;
+    ctx->last_launches = 0;
+    if (max_iter < 0 || !(gtol >= 0.f)) return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_fit: max_iter, gtol must be >= 0");
+    ScatterProblem pb;
+    unsigned char *ws = nullptr;
+    int rc = scatter_setup(ctx, "tno_mf_scatter_fit", D, T, N, n, jitter_xy, delta, beta, S,
+                           scatter_ws_bytes(T, N, n), &pb, &ws);
+    if (rc) return rc;
+    double loss = 0.0;
+    int32_t iters = 0, evals = 0, launches = 0;
+    const int32_t e = scatter_fit(ctx->stream, pb, beta, S, ws, max_iter, gtol, &loss, &iters, &evals, &launches);
+    ctx->last_launches = launches;
+    if (e != 0) return fail(ctx, TNO_MF_ECUDA, "tno_mf_scatter_fit: %s", cudaGetErrorString((cudaError_t)e));
+    if (out_loss) *out_loss = loss;
+    if (out_iters) *out_iters = iters;
+    if (out_evals) *out_evals = evals;
+    return TNO_MF_OK;
+}
+
+int tno_mf_downsample(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H, int32_t W, int32_t factor,
+                      float *out) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (!frames || !out) return fail(ctx, TNO_MF_EINVAL, "tno_mf_downsample: NULL pointer");
+    if (T < 1 || T > 65535 || H < 1 || W < 1 || factor < 1 || H % factor || W % factor)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_downsample: need 1 <= T <= 65535 and factor dividing H and W");
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    launch_downsample(ctx->stream, frames, T, H, W, factor, out);
+    ctx->last_launches = 1;
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
+}
+
+int tno_mf_scatter_subtract(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W, const float *S,
+                            int32_t n) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (!frames || !S) return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_subtract: NULL pointer");
+    if (T < 1 || T > 65535 || H < 1 || W < 1 || n < 1 || n > H || n > W)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_subtract: need 1 <= T <= 65535 and 1 <= n <= min(H, W)");
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    std::vector<int32_t> tabs(2 * ((size_t)H + W));          // y: first pixel [H], weight [H]; x: the same [W]
+    bilinear_table(H, n, tabs.data(), reinterpret_cast<float *>(tabs.data() + H));
+    bilinear_table(W, n, tabs.data() + 2 * H, reinterpret_cast<float *>(tabs.data() + 2 * H + W));
+    int rc = reserve(ctx, ctx->scat, tabs.size() * 4);
+    if (rc) return rc;
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->scat.p, tabs.data(), tabs.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));      // tabs is a local buffer
+    const int32_t *d = static_cast<const int32_t *>(ctx->scat.p);
+    launch_scatter_subtract(ctx->stream, frames, T, H, W, S, n, d, reinterpret_cast<const float *>(d + H), d + 2 * H,
+                            reinterpret_cast<const float *>(d + 2 * H + W));
+    ctx->last_launches = 1;
+    CU_TRY(ctx, cudaGetLastError());
+    return TNO_MF_OK;
 }
 
 int tno_mf_set_prf_table(tno_mf_ctx *ctx, const float *table, int32_t n_phase) {

@@ -56,6 +56,29 @@ struct BgRinv { float v[36]; };      // R^{-1} of the orthonormalised basis, row
 void launch_background(cudaStream_t st, const float *frames, int32_t T, int64_t n_px, const float *Q,
                        const BgRinv &rinv, float delta, int32_t n_iter, float *out_coef, float *out_resid);
 
+// ---- scatter.cu ---- (section 3.1: low-resolution scattered-light model, L-BFGS)
+constexpr int kScatterHistory = 10;
+struct ScatterProblem {
+    const float *D;        // DEVICE [T][N][N] downsampled data
+    int32_t T, N, n;
+    const float *phi;      // DEVICE [T][8]: (1, x, y, x^2, y^2, xy, 0, 0) of the jitter
+    const int32_t *bi0;    // DEVICE [N]: first input pixel of output pixel i (bilinear_table)
+    const float *bw;       // DEVICE [N]: weight of the second input pixel
+    const int32_t *blo, *bhi;   // DEVICE [n]: first and last output pixel whose stencil touches input pixel b
+    float delta;
+};
+void bilinear_table(int32_t N, int32_t n, int32_t *i0, float *w);      // host
+void launch_downsample(cudaStream_t st, const float *frames, int32_t T, int32_t H, int32_t W, int32_t f, float *out);
+void launch_scatter_subtract(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W, const float *S, int32_t n,
+                             const int32_t *yi0, const float *yw, const int32_t *xi0, const float *xw);
+// launches only; returns the number of kernels launched
+int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float *beta, const float *S, float *psi,
+                         double *partials, float *g_beta, float *g_S, double *loss_dev);
+size_t scatter_ws_bytes(int32_t T, int32_t N, int32_t n);
+// beta, S: DEVICE, start point in, minimiser out; synchronises the stream; returns 0 or a cudaError_t
+int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, float *S, void *ws, int32_t max_iter,
+                    float gtol, double *out_loss, int32_t *out_iters, int32_t *out_evals, int32_t *out_launches);
+
 // ---- inject.cu ----
 struct SourceDev { float vx, vy, ax, ay; int32_t x, y; float amp; };
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,

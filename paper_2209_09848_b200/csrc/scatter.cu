@@ -1,0 +1,410 @@
+// Low-resolution scattered-light model (section 3.1, Eq. 1-4, second part):
+//     D_t = U(S_t) + B + B_theta . theta_t^k + eps,      L = sum_{t,i,j} L_delta(D_t - pred_t)_{ij}
+// D: the data downsampled to N x N (512), S_t: n x n (64) per frame, U: bilinear upsampling, the background terms
+// as in background.cu.  "We minimize this convex loss over B, B_theta, S_t using the L-BFGS algorithm" (L94).
+//   k_downsample        block means, 2048^2 -> 512^2 (L69)
+//   k_scatter_resid     one thread per low-resolution pixel walks the frames: residual, loss, dL/dbeta in registers,
+//                       psi = clip(r) to a scratch stack
+//   k_scatter_gs        dL/dS_t = -U^T psi_t as a gather: one thread per (t, a, b) sums its footprint (no atomics)
+//   k_dot / k_sum_partials / k_axpy / k_absmax   the vector algebra of L-BFGS, two-stage reductions in a fixed
+//                       order (float64), so a fit is reproducible run to run
+//   scatter_fit         the L-BFGS driver (host loop, two-loop recursion, Armijo backtracking)
+//   k_scatter_subtract  frames -= U(S_t) at full resolution, the hand-over to tno_mf_background
+// Everything is HBM-bound streaming over a 1 GB stack (T = 1000, N = 512); the paper quotes ~40 s for this solve.
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "kernels.h"
+
+namespace tno {
+
+// 1-D bilinear stencil of output pixel i (reading s2): centre at u = (i + 1/2) n / N - 1/2, clamped to [0, n - 1];
+// inputs floor(u) and floor(u) + 1 (clamped) with weights 1 - frac(u), frac(u).  The host tabulates floor(u) and
+// frac(u) per output pixel in float64 (bilinear_table) -- the kernels only look them up.
+void bilinear_table(int32_t N, int32_t n, int32_t *i0, float *w) {
+    for (int32_t i = 0; i < N; ++i) {
+        double u = ((double)i + 0.5) * (double)n / (double)N - 0.5;
+        u = std::min(std::max(u, 0.0), (double)(n - 1));
+        const double f = std::floor(u);
+        i0[i] = (int32_t)f;
+        w[i] = (float)(u - f);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_downsample(const float *__restrict__ frames, int32_t H, int32_t W, int32_t f, float *__restrict__ out) {
+    const int32_t Wo = W / f, Ho = H / f;
+    const int32_t x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6), t = blockIdx.z;
+    if (x >= Wo || y >= Ho) return;
+    const float *src = frames + ((int64_t)t * H + (int64_t)y * f) * W + (int64_t)x * f;
+    double s = 0.0;
+    for (int32_t j = 0; j < f; ++j)
+        for (int32_t i = 0; i < f; ++i) s += (double)__ldg(src + (int64_t)j * W + i);
+    out[((int64_t)t * Ho + y) * Wo + x] = (float)(s / ((double)f * f));
+}
+
+constexpr int kRedBlocks = 1024;       // partial sums of every reduction
+
+// block-wide sum in a fixed order -> partials[blockIdx.x]
+__device__ __forceinline__ void block_sum_to(double v, double *__restrict__ partials) {
+    __shared__ double sh[8];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += sh[w];
+        partials[blockIdx.x] = s;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_scatter_resid(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, const float *__restrict__ phi /* [T][8] */,
+                const int32_t *__restrict__ bi0, const float *__restrict__ bw, float delta, const float *__restrict__ beta, const float *__restrict__ S, float *__restrict__ psi,
+                float *__restrict__ g_beta, double *__restrict__ partials) {
+    const int64_t n_px = (int64_t)N * N;
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double loss = 0.0;
+    if (p < n_px) {
+        const int32_t i = (int32_t)(p / N), j = (int32_t)(p % N);
+        const int32_t i0 = bi0[i], j0 = bi0[j], i1 = min(i0 + 1, n - 1), j1 = min(j0 + 1, n - 1);
+        const float wy = bw[i], wx = bw[j];
+        const float w00 = (1.f - wy) * (1.f - wx), w01 = (1.f - wy) * wx, w10 = wy * (1.f - wx), w11 = wy * wx;
+        const int32_t o00 = i0 * n + j0, o01 = i0 * n + j1, o10 = i1 * n + j0, o11 = i1 * n + j1;
+        float b[6], g[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { b[k] = beta[k * n_px + p]; g[k] = 0.f; }
+#pragma unroll 4
+        for (int32_t t = 0; t < T; ++t) {
+            const float4 qa = __ldg(reinterpret_cast<const float4 *>(phi + 8 * (int64_t)t));
+            const float2 qb = __ldg(reinterpret_cast<const float2 *>(phi + 8 * (int64_t)t + 4));
+            const float q[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
+            const float *St = S + (int64_t)t * n * n;
+            float pred = w00 * __ldg(St + o00) + w01 * __ldg(St + o01) + w10 * __ldg(St + o10) + w11 * __ldg(St + o11);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) pred = fmaf(q[k], b[k], pred);
+            const float r = D[(int64_t)t * n_px + p] - pred;
+            const float a = fabsf(r);
+            loss += (double)(a <= delta ? 0.5f * r * r : delta * (a - 0.5f * delta));       // Eq. 4
+            const float c = fminf(fmaxf(r, -delta), delta);
+            psi[(int64_t)t * n_px + p] = c;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) g[k] = fmaf(q[k], c, g[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) g_beta[k * n_px + p] = -g[k];
+    }
+    block_sum_to(loss, partials);
+}
+
+// dL/dS[t][a][b] = - sum_{i,j} wy(i, a) wx(j, b) psi[t][i][j]: only pixels within one input pixel of (a, b) count
+__global__ void __launch_bounds__(256)
+k_scatter_gs(const float *__restrict__ psi, int32_t T, int32_t N, int32_t n, const int32_t *__restrict__ bi0,
+             const float *__restrict__ bw, float *__restrict__ g_S) {
+    const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (int64_t)T * n * n) return;
+    const int32_t b = (int32_t)(id % n), a = (int32_t)((id / n) % n), t = (int32_t)(id / ((int64_t)n * n));
+    const int32_t f = (N + n - 1) / n;
+    const int32_t ilo = max(0, (a - 1) * f - 1), ihi = min(N - 1, (a + 2) * f), jlo = max(0, (b - 1) * f - 1),
+                  jhi = min(N - 1, (b + 2) * f);
+    const float *P = psi + (int64_t)t * N * N;
+    float acc = 0.f;
+    for (int32_t i = ilo; i <= ihi; ++i) {
+        const int32_t i0 = __ldg(bi0 + i), i1 = min(i0 + 1, n - 1);
+        const float w = __ldg(bw + i);
+        const float wy = (i0 == a ? 1.f - w : 0.f) + (i1 == a ? w : 0.f);
+        if (wy == 0.f) continue;
+        float row = 0.f;
+        for (int32_t j = jlo; j <= jhi; ++j) {
+            const int32_t j0 = __ldg(bi0 + j), j1 = min(j0 + 1, n - 1);
+            const float v = __ldg(bw + j);
+            const float wx = (j0 == b ? 1.f - v : 0.f) + (j1 == b ? v : 0.f);
+            if (wx != 0.f) row = fmaf(wx, __ldg(P + (int64_t)i * N + j), row);
+        }
+        acc = fmaf(wy, row, acc);
+    }
+    g_S[id] = -acc;
+}
+
+// The same sum, separably and with every psi read exactly once, coalesced: one block per frame, one thread per
+// column j walks down the rows; row i feeds the two input rows a = bi0[i] (weight 1 - w) and a + 1 (weight w), which
+// are the same for the whole block, so two running sums per thread suffice; when a advances, the finished column
+// sums C_a[j] go through shared memory and threads b < n reduce them along j over their support [blo[b], bhi[b]].
+__global__ void __launch_bounds__(1024)
+k_scatter_gs_cols(const float *__restrict__ psi, int32_t N, int32_t n, const int32_t *__restrict__ bi0,
+                  const float *__restrict__ bw, const int32_t *__restrict__ blo, const int32_t *__restrict__ bhi,
+                  float *__restrict__ g_S) {
+    extern __shared__ float C[];                 // [N]
+    const int32_t t = blockIdx.x, j = threadIdx.x;
+    const bool active = j < N;
+    const float *P = psi + (int64_t)t * N * N;
+    float *out = g_S + (int64_t)t * n * n;
+    const int32_t my_lo = j < n ? blo[j] : 0, my_hi = j < n ? bhi[j] : -1;
+    auto flush = [&](int32_t a, float acc) {
+        if (active) C[j] = acc;
+        __syncthreads();
+        if (j < n) {
+            float sum = 0.f;
+            for (int32_t c = my_lo; c <= my_hi; ++c) {
+                const int32_t c0 = __ldg(bi0 + c), c1 = min(c0 + 1, n - 1);
+                const float v = __ldg(bw + c);
+                const float wx = (c0 == j ? 1.f - v : 0.f) + (c1 == j ? v : 0.f);
+                sum = fmaf(wx, C[c], sum);
+            }
+            out[a * n + j] = -sum;
+        }
+        __syncthreads();
+    };
+    float acc0 = 0.f, acc1 = 0.f;
+    int32_t cur = __ldg(bi0);
+    for (int32_t i = 0; i < N; ++i) {
+        const int32_t a0 = __ldg(bi0 + i);
+        const float w = __ldg(bw + i);
+        if (a0 != cur) {                         // uniform over the block: the input row advances by one
+            flush(cur, acc0);
+            acc0 = acc1;
+            acc1 = 0.f;
+            cur = a0;
+        }
+        const float v = active ? __ldcs(P + (int64_t)i * N + j) : 0.f;
+        if (a0 + 1 <= n - 1) {
+            acc0 = fmaf(1.f - w, v, acc0);
+            acc1 = fmaf(w, v, acc1);
+        } else {
+            acc0 += v;                           // clamped: both stencil points are the last input row
+        }
+    }
+    flush(cur, acc0);
+    for (int32_t a = cur + 1; a < n; ++a) {      // input rows below the last stencil (only if N < n, never here)
+        flush(a, a == cur + 1 ? acc1 : 0.f);
+    }
+}
+
+// ---- vector algebra of L-BFGS (float32 vectors, float64 reductions in a fixed order) -----------------------------
+__global__ void __launch_bounds__(256)
+k_dot(const float *__restrict__ x, const float *__restrict__ y, int64_t n, double *__restrict__ partials) {
+    double s = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        s += (double)x[i] * (double)y[i];
+    block_sum_to(s, partials);
+}
+__global__ void __launch_bounds__(256)
+k_absmax(const float *__restrict__ x, int64_t n, double *__restrict__ partials) {
+    __shared__ double sh[8];
+    double m = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        m = fmax(m, fabs((double)x[i]));
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) m = fmax(m, sh[w]);
+        partials[blockIdx.x] = fmax(m, sh[0]);
+    }
+}
+// out[0] = sum (or max) of the n partials, one block, fixed tree
+__global__ void __launch_bounds__(256)
+k_sum_partials(const double *__restrict__ partials, int32_t n, int32_t take_max, double *__restrict__ out) {
+    __shared__ double sh[256];
+    double s = 0.0;
+    for (int32_t i = threadIdx.x; i < n; i += 256) s = take_max ? fmax(s, partials[i]) : s + partials[i];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o)
+            sh[threadIdx.x] = take_max ? fmax(sh[threadIdx.x], sh[threadIdx.x + o]) : sh[threadIdx.x] + sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[0] = sh[0];
+}
+// z = a x + b y   (z may alias x or y)
+__global__ void __launch_bounds__(256)
+k_axpby(float a, const float *x, float b, const float *y, int64_t n, float *z) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) z[i] = a * x[i] + (b != 0.f ? b * y[i] : 0.f);
+}
+
+// VEC: four neighbouring pixels per thread (W % 4 == 0, 16-byte aligned frames)
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+k_scatter_subtract(float *__restrict__ frames, int32_t H, int32_t W, const float *__restrict__ S, int32_t n,
+                   const int32_t *__restrict__ yi0, const float *__restrict__ yw, const int32_t *__restrict__ xi0,
+                   const float *__restrict__ xw) {
+    constexpr int PX = VEC ? 4 : 1;
+    const int32_t x = (blockIdx.x * 64 + (threadIdx.x & 63)) * PX, y = blockIdx.y * 4 + (threadIdx.x >> 6), t = blockIdx.z;
+    if (x >= W || y >= H) return;
+    const int32_t i0 = yi0[y], i1 = min(i0 + 1, n - 1);
+    const float wy = yw[y];
+    const float *r0 = S + (int64_t)t * n * n + i0 * n, *r1 = S + (int64_t)t * n * n + i1 * n;
+    float u[PX];
+#pragma unroll
+    for (int k = 0; k < PX; ++k) {
+        const int32_t j0 = xi0[x + k], j1 = min(j0 + 1, n - 1);
+        const float wx = xw[x + k];
+        u[k] = (1.f - wy) * ((1.f - wx) * __ldg(r0 + j0) + wx * __ldg(r0 + j1)) +
+               wy * ((1.f - wx) * __ldg(r1 + j0) + wx * __ldg(r1 + j1));
+    }
+    float *p = frames + ((int64_t)t * H + y) * W + x;
+    if (VEC) {
+        float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
+        v.x -= u[0]; v.y -= u[1]; v.z -= u[2]; v.w -= u[3];
+        __stcs(reinterpret_cast<float4 *>(p), v);
+    } else {
+        p[0] -= u[0];
+    }
+}
+
+void launch_downsample(cudaStream_t st, const float *frames, int32_t T, int32_t H, int32_t W, int32_t f, float *out) {
+    dim3 grid((unsigned)((W / f + 63) / 64), (unsigned)((H / f + 3) / 4), (unsigned)T);
+    k_downsample<<<grid, 256, 0, st>>>(frames, H, W, f, out);
+}
+
+void launch_scatter_subtract(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W, const float *S, int32_t n,
+                             const int32_t *yi0, const float *yw, const int32_t *xi0, const float *xw) {
+    if (W % 4 == 0 && (reinterpret_cast<uintptr_t>(frames) & 15u) == 0) {
+        dim3 grid((unsigned)((W / 4 + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)T);
+        k_scatter_subtract<true><<<grid, 256, 0, st>>>(frames, H, W, S, n, yi0, yw, xi0, xw);
+    } else {
+        dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)T);
+        k_scatter_subtract<false><<<grid, 256, 0, st>>>(frames, H, W, S, n, yi0, yw, xi0, xw);
+    }
+}
+
+// loss -> loss_dev[0] (DEVICE double), gradient -> g_beta, g_S.  psi: [T][N][N] scratch, partials: [>= blocks] doubles
+int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float *beta, const float *S, float *psi,
+                         double *partials, float *g_beta, float *g_S, double *loss_dev) {
+    const int64_t n_px = (int64_t)pb.N * pb.N;
+    const int32_t blocks = (int32_t)((n_px + 255) / 256);
+    k_scatter_resid<<<(unsigned)blocks, 256, 0, st>>>(pb.D, pb.T, pb.N, pb.n, pb.phi, pb.bi0, pb.bw, pb.delta, beta, S, psi,
+                                                     g_beta, partials);
+    k_sum_partials<<<1, 256, 0, st>>>(partials, blocks, 0, loss_dev);
+    if (pb.N <= 1024) {
+        const int32_t threads = ((std::max(pb.N, pb.n) + 31) / 32) * 32;
+        k_scatter_gs_cols<<<(unsigned)pb.T, threads, (size_t)pb.N * 4, st>>>(psi, pb.N, pb.n, pb.bi0, pb.bw, pb.blo, pb.bhi,
+                                                                           g_S);
+    } else {
+        const int64_t ns = (int64_t)pb.T * pb.n * pb.n;
+        k_scatter_gs<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(psi, pb.T, pb.N, pb.n, pb.bi0, pb.bw, g_S);
+    }
+    return 3;
+}
+
+// ---- L-BFGS --------------------------------------------------------------------------------------
+// x = [beta (6 N^2) | S (T n^2)].  Two-loop recursion over the last kScatterHistory (s, y) pairs, initial scaling
+// s.y / y.y, Armijo backtracking from step 1 (first iteration: 1 / |g|); a pair enters the history only if
+// s.y > 1e-10 |y|^2; a non-descent direction resets the history.  Stops at |g|_inf <= gtol, after max_iter
+// iterations, when two consecutive iterations each decrease the loss by less than 1e-9 of its value, or when the
+// line search cannot decrease it at all (float32 resolution reached).
+size_t scatter_ws_bytes(int32_t T, int32_t N, int32_t n) {
+    const size_t P = (size_t)6 * N * N + (size_t)T * n * n;
+    const size_t blocks = std::max<size_t>(kRedBlocks, ((size_t)N * N + 255) / 256);
+    return (5 + 2 * (size_t)kScatterHistory) * P * 4 + (size_t)T * N * N * 4 + (blocks + 8) * 8 + 256;
+}
+
+int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, float *S, void *ws, int32_t max_iter,
+                    float gtol, double *out_loss, int32_t *out_iters, int32_t *out_evals, int32_t *out_launches) {
+    const int64_t nb = (int64_t)6 * pb.N * pb.N, ns = (int64_t)pb.T * pb.n * pb.n, P = nb + ns;
+    const size_t blocks = std::max<size_t>(kRedBlocks, ((size_t)pb.N * pb.N + 255) / 256);
+    float *x = static_cast<float *>(ws), *g = x + P, *xn = g + P, *gn = xn + P, *d = gn + P;
+    float *hs = d + P, *hy = hs + (size_t)kScatterHistory * P, *psi = hy + (size_t)kScatterHistory * P;
+    double *partials = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(psi + (size_t)pb.T * pb.N * pb.N) + 15) &
+                                                  ~(uintptr_t)15);
+    double *scal = partials + blocks;
+    int32_t launches = 0, evals = 0;
+    cudaError_t err = cudaSuccess;
+    auto fetch = [&](double *dev) -> double {
+        double h = 0.0;
+        cudaError_t e = cudaMemcpyAsync(&h, dev, 8, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) err = e;
+        return h;
+    };
+    auto dot = [&](const float *a, const float *b) -> double {
+        k_dot<<<kRedBlocks, 256, 0, st>>>(a, b, P, partials);
+        k_sum_partials<<<1, 256, 0, st>>>(partials, kRedBlocks, 0, scal);
+        launches += 2;
+        return fetch(scal);
+    };
+    auto axpby = [&](float a, const float *xx, float b, const float *yy, float *zz) {
+        k_axpby<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(a, xx, b, yy, P, zz);
+        launches += 1;
+    };
+    auto eval = [&](const float *xx, float *gg) -> double {
+        launches += scatter_lossgrad(st, pb, xx, xx + nb, psi, partials, gg, gg + nb, scal + 1);
+        ++evals;
+        return fetch(scal + 1);
+    };
+    cudaMemcpyAsync(x, beta, nb * 4, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(x + nb, S, ns * 4, cudaMemcpyDeviceToDevice, st);
+    double f = eval(x, g);
+    std::vector<double> rho(kScatterHistory), alpha(kScatterHistory);
+    int32_t hist = 0, head = 0, it = 0;          // pairs stored, slot of the next pair
+    int32_t stalled = 0;                         // consecutive iterations without a relevant decrease
+    for (; it < max_iter && err == cudaSuccess; ++it) {
+        k_absmax<<<kRedBlocks, 256, 0, st>>>(g, P, partials);
+        k_sum_partials<<<1, 256, 0, st>>>(partials, kRedBlocks, 1, scal);
+        launches += 2;
+        if (fetch(scal) <= (double)gtol) break;
+        // d = -H g
+        axpby(1.f, g, 0.f, g, d);
+        for (int32_t c = 0; c < hist; ++c) {
+            const int32_t i = (head - 1 - c + 2 * kScatterHistory) % kScatterHistory;
+            alpha[i] = rho[i] * dot(hs + (size_t)i * P, d);
+            axpby(1.f, d, (float)-alpha[i], hy + (size_t)i * P, d);
+        }
+        if (hist > 0) {
+            const int32_t l = (head - 1 + kScatterHistory) % kScatterHistory;
+            const double yy = dot(hy + (size_t)l * P, hy + (size_t)l * P);
+            axpby((float)(1.0 / (rho[l] * yy)), d, 0.f, d, d);
+        }
+        for (int32_t c = hist - 1; c >= 0; --c) {
+            const int32_t i = (head - 1 - c + 2 * kScatterHistory) % kScatterHistory;
+            const double b = rho[i] * dot(hy + (size_t)i * P, d);
+            axpby(1.f, d, (float)(alpha[i] - b), hs + (size_t)i * P, d);
+        }
+        double dg = -dot(g, d);                  // directional derivative along -d
+        if (!(dg < 0.0)) {                       // not a descent direction: steepest descent, empty history
+            hist = 0;
+            axpby(1.f, g, 0.f, g, d);
+            dg = -dot(g, g);
+            if (!(dg < 0.0)) break;
+        }
+        double step = (hist == 0) ? std::min(1.0, 1.0 / std::sqrt(-dg)) : 1.0;
+        double fn = f;
+        bool ok = false;
+        for (int32_t ls = 0; ls < 40 && err == cudaSuccess; ++ls) {
+            axpby(1.f, x, (float)-step, d, xn);
+            fn = eval(xn, gn);
+            if (fn <= f + 1e-4 * step * dg) { ok = true; break; }
+            step *= 0.5;
+        }
+        if (!ok) break;
+        // s = xn - x, y = gn - g into the history slot
+        float *s_new = hs + (size_t)head * P, *y_new = hy + (size_t)head * P;
+        axpby(1.f, xn, -1.f, x, s_new);
+        axpby(1.f, gn, -1.f, g, y_new);
+        const double sy = dot(s_new, y_new), yy = dot(y_new, y_new);
+        if (sy > 1e-10 * yy && yy > 0.0) {
+            rho[head] = 1.0 / sy;
+            head = (head + 1) % kScatterHistory;
+            hist = std::min(hist + 1, kScatterHistory);
+        }
+        std::swap(x, xn);
+        std::swap(g, gn);
+        stalled = (f - fn <= 1e-9 * std::fabs(f)) ? stalled + 1 : 0;
+        f = fn;
+        if (stalled >= 2) { ++it; break; }
+    }
+    cudaMemcpyAsync(beta, x, nb * 4, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(S, x + nb, ns * 4, cudaMemcpyDeviceToDevice, st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err == cudaSuccess) err = cudaGetLastError();
+    *out_loss = f;
+    *out_iters = it;
+    *out_evals = evals;
+    *out_launches = launches;
+    return err == cudaSuccess ? 0 : (int32_t)err;
+}
+
+}  // namespace tno

@@ -1,0 +1,128 @@
+"""GPU parity of the low-resolution scattered-light model (section 3.1, Eq. 1-4) against the oracle, through
+the C ABI: block-mean downsampling, loss and gradient, the L-BFGS fit (loss and prediction of the minimiser), and
+the subtraction of the upsampled scattered light."""
+import numpy as np
+import pytest
+
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _problem(seed, T, N, n, noise=0.3, outliers=0.02):
+    """Smooth scattered light that changes from frame to frame over a static background that moves with the
+    jitter, plus noise and a few outliers (the shape of the paper's problem)."""
+    rng = np.random.default_rng(seed)
+    jit = (0.15 * rng.standard_normal((T, 2))).astype(np.float32)
+    beta = rng.standard_normal((6, N, N)) * np.array([20, 3, 3, 1, 1, 1])[:, None, None]
+    S = 10.0 + 5.0 * rng.standard_normal((T, n, n))
+    D = oracle.upsample(S, N) + np.einsum("tk,kij->tij", oracle.background_basis(jit), beta)
+    D += noise * rng.standard_normal(D.shape)
+    D += (rng.uniform(size=D.shape) < outliers) * rng.laplace(0, 15, size=D.shape)
+    return D.astype(np.float32), jit, beta, S
+
+
+@pytest.mark.parametrize("T,N,n", [(9, 24, 3), (5, 64, 8), (17, 40, 5), (3, 16, 16), (6, 33, 4),
+                                   (2, 1040, 13)])          # N > 1024: the gather form of the S gradient
+def test_loss_and_gradient_match_oracle(T, N, n):
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    D, jit, beta, S = _problem(T + N + n, T, N, n)
+    rng = np.random.default_rng(1)
+    b0 = (beta + rng.standard_normal(beta.shape)).astype(np.float32)
+    S0 = (S + rng.standard_normal(S.shape)).astype(np.float32)
+    delta = 0.8
+    L, gb, gs = oracle.scatter_loss_grad(D, jit, delta, b0, S0)
+    with MatchedFilter(0) as mf:
+        d = [torch.from_numpy(a).cuda() for a in (D, b0, S0)]
+        ggb, ggs = torch.empty_like(d[1]), torch.empty_like(d[2])
+        loss = P.tno_mf_scatter_lossgrad(mf.ctx, d[0], jit, delta, d[1], d[2], ggb, ggs)
+        torch.cuda.synchronize()
+    assert abs(loss - L) <= 2e-5 * L
+    # float32 sums of up to T (beta) and (2N/n)^2 (S) terms of size <= delta * weight
+    assert np.abs(ggb.cpu().numpy() - gb).max() <= 2e-5 * max(1.0, np.abs(gb).max())
+    assert np.abs(ggs.cpu().numpy() - gs).max() <= 2e-5 * max(1.0, np.abs(gs).max())
+
+
+def test_downsample_and_subtract():
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    rng = np.random.default_rng(2)
+    f = (100.0 + rng.standard_normal((5, 48, 64))).astype(np.float32)
+    with MatchedFilter(0) as mf:
+        d = torch.from_numpy(f).cuda()
+        out = torch.empty((5, 12, 16), device="cuda")
+        P.tno_mf_downsample(mf.ctx, d, 4, out)
+        torch.cuda.synchronize()
+        assert np.abs(out.cpu().numpy() - oracle.downsample(f, 4)).max() <= 1e-5
+        for side in (64, 45):                                        # 16-byte path and the scalar path
+            sq = (100.0 + rng.standard_normal((4, side, side))).astype(np.float32)
+            S = (10.0 * rng.standard_normal((4, 8, 8))).astype(np.float32)
+            dsq = torch.from_numpy(sq).cuda()
+            P.tno_mf_scatter_subtract(mf.ctx, dsq, torch.from_numpy(S).cuda())
+            torch.cuda.synchronize()
+            assert np.abs(dsq.cpu().numpy() - (sq - oracle.upsample(S, side))).max() <= 2e-5
+        with pytest.raises(P.TnoMfError):
+            P.tno_mf_downsample(mf.ctx, d, 5, torch.empty((5, 9, 12), device="cuda"))      # 5 does not divide 48
+
+
+def test_fit_reaches_the_oracles_minimum():
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    T, N, n = 40, 32, 4
+    D, jit, beta, S = _problem(7, T, N, n)
+    delta = 1.0
+    ob, oS, oL = oracle.scatter_fit(D, jit, delta, n, max_iter=2000)
+    with MatchedFilter(0) as mf:
+        d = torch.from_numpy(D).cuda()
+        b = torch.zeros((6, N, N), device="cuda")
+        s = torch.zeros((T, n, n), device="cuda")
+        loss, iters, evals = P.tno_mf_scatter_fit(mf.ctx, d, jit, delta, 2000, 0.0, b, s)
+        assert mf.stats()[0] > 3 * evals
+        # the reported loss is the loss of the returned parameters
+        gb, gs = torch.empty_like(b), torch.empty_like(s)
+        again = P.tno_mf_scatter_lossgrad(mf.ctx, d, jit, delta, b, s, gb, gs)
+        torch.cuda.synchronize()
+        # reproducible: the same call gives the same bits
+        b2 = torch.zeros_like(b)
+        s2 = torch.zeros_like(s)
+        loss2, iters2, _ = P.tno_mf_scatter_fit(mf.ctx, d, jit, delta, 2000, 0.0, b2, s2)
+        assert loss2 == loss and iters2 == iters and torch.equal(b2, b) and torch.equal(s2, s)
+    assert abs(again - loss) <= 1e-6 * loss
+    start = oracle.scatter_loss_grad(D, jit, delta, np.zeros_like(beta), np.zeros_like(S))[0]
+    assert loss < 0.05 * start and 0 < iters <= 2000
+    assert abs(loss - oL) <= 1e-4 * oL, (loss, oL, iters, evals)         # the convex minimum, to float32 resolution
+    pred_g = oracle.upsample(s.cpu().numpy(), N) + np.einsum("tk,kij->tij", oracle.background_basis(jit),
+                                                             b.cpu().numpy().astype(np.float64))
+    pred_o = oracle.upsample(oS, N) + np.einsum("tk,kij->tij", oracle.background_basis(jit), ob)
+    assert np.sqrt(np.mean((pred_g - pred_o) ** 2)) < 0.02           # noise is 0.3: the fits agree far below it
+
+
+def test_fit_on_exact_data_and_errors():
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    T, N, n = 8, 24, 3
+    D, jit, beta, S = _problem(9, T, N, n, noise=0.0, outliers=0.0)
+    with MatchedFilter(0) as mf:
+        d = torch.from_numpy(D).cuda()
+        b = torch.zeros((6, N, N), device="cuda")
+        s = torch.zeros((T, n, n), device="cuda")
+        loss, iters, _ = P.tno_mf_scatter_fit(mf.ctx, d, jit, 1.0, 3000, 0.0, b, s)
+        torch.cuda.synchronize()
+        pred = oracle.upsample(s.cpu().numpy(), N) + np.einsum("tk,kij->tij", oracle.background_basis(jit),
+                                                               b.cpu().numpy().astype(np.float64))
+        assert np.abs(pred - D).max() < 0.05 and loss < 1e-3 * T * N * N
+        for bad in ((0.0, 10, 0.0), (1.0, -1, 0.0), (1.0, 10, -1.0)):
+            with pytest.raises(P.TnoMfError):
+                P.tno_mf_scatter_fit(mf.ctx, d, jit, bad[0], bad[1], bad[2], b, s)
