@@ -66,7 +66,7 @@ k_background_plain(const float *frames, int32_t T, int64_t n_px, const float *__
 // with ordinary loads touches a different 2 MB page at every step, and once T exceeds the reach of the TLB
 // (measured: the plain kernel drops from 5.3 TB/s at T = 50 to 2.9 TB/s at T >= 100, whatever H and W are)
 // every warp-load pays a miss.  Here one elected thread requests each frame's NT*4 pixels as ONE bulk copy
-// (cp.async.bulk, one translation per 2 KB) into a ring of NS shared-memory stages of FS frames each,
+// (cp.async.bulk, one translation per 2 KB; a fifth warp does nothing else) into a ring of NS stages of FS frames,
 // together with the FS rows of Q, completion on the stage's mbarrier; the ring runs on through the passes, so
 // the first frames of the next pass are in flight while the last ones of this pass are consumed.  The
 // arithmetic is packed (FFMA2 on pixel pairs): 24 FFMA2 + 8 FMNMX per 4 pixels and frame.
@@ -88,7 +88,7 @@ __device__ __forceinline__ void bg_bulk(uint32_t dst, const void *src, uint32_t 
 }
 
 template <int NT, int NS, int FS, int MB>
-__global__ void __launch_bounds__(NT, MB)
+__global__ void __launch_bounds__(NT + 32, MB)
 k_background_bulk(const float *frames, int32_t T, int64_t n_px, const float *__restrict__ Q /* [T][16] */,
                   BgRinv rinv, float delta, int32_t n_iter, float *__restrict__ out_coef, float *out_resid) {
     constexpr int PXF = NT * 4;                                  // floats of one frame's pixels in a stage
@@ -128,8 +128,16 @@ k_background_bulk(const float *frames, int32_t T, int64_t n_px, const float *__r
         iss_t0 += FS;
         if (iss_t0 >= T) iss_t0 = 0;
     };
-    if (tid == 0)
-        for (int s = 0; s < NS && iss < total; ++s) issue();
+    if (tid >= NT) {
+        // producer warp: one lane keeps the ring full -- a stage is requested again as soon as the NT / 32 consumer
+        // warps have released it; the consumers never issue a copy
+        if (lane == 0)
+            for (int32_t gq = 0; gq < total; ++gq) {
+                if (gq >= NS) bg_wait(empty + 8 * iss_s, ((uint32_t)(gq / NS) - 1u) & 1u);
+                issue();
+            }
+        return;
+    }
 
     float2 cn[6][2];                                             // MINUS the coefficients, two pixel pairs
 #pragma unroll
@@ -154,11 +162,6 @@ k_background_bulk(const float *frames, int32_t T, int64_t n_px, const float *__r
             }
             __syncwarp();
             if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty + 8 * st) : "memory");
-            // refill the stage before this one: every warp has most likely left it by now
-            if (tid == 0 && g >= 1 && iss < total) {
-                bg_wait(empty + 8 * iss_s, st == 0 ? par ^ 1u : par);
-                issue();
-            }
             if (++st == NS) { st = 0; par ^= 1u; }
         }
     };
@@ -224,12 +227,13 @@ void launch_background(cudaStream_t st, const float *frames, int32_t T, int64_t 
     const bool vec = (n_px % 4 == 0) && ((reinterpret_cast<uintptr_t>(frames) | reinterpret_cast<uintptr_t>(out_coef) |
                                           reinterpret_cast<uintptr_t>(out_resid)) & 15u) == 0;
     if (vec) {
-        // 128 threads x 4 pixels, 3 stages of 8 frames (50.7 KB), 4 CTAs per SM: the best of the swept
+        // 128 consumer threads x 4 pixels + a producer warp, 3 stages of 8 frames (50.7 KB), 4 CTAs per SM: the best
+        // of the swept
         // (NT, NS, FS, CTAs/SM) on config 3 -- see DESIGN.md 8f
         constexpr int NT = 128, NS = 3, FS = 8, MB = 4;
         constexpr int smem = NS * FS * (NT * 4 + 16) * 4;
         cudaFuncSetAttribute(k_background_bulk<NT, NS, FS, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        k_background_bulk<NT, NS, FS, MB><<<(unsigned)((n_px + NT * 4 - 1) / (NT * 4)), NT, smem, st>>>(
+        k_background_bulk<NT, NS, FS, MB><<<(unsigned)((n_px + NT * 4 - 1) / (NT * 4)), NT + 32, smem, st>>>(
             frames, T, n_px, Q, rinv, delta, n_iter, out_coef, out_resid);
     } else {
         k_background_plain<<<(unsigned)((n_px + 255) / 256), 256, 0, st>>>(frames, T, n_px, Q, rinv, delta, n_iter,
