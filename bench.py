@@ -335,6 +335,35 @@ def run_ours(args, cfg):
             gb = 2.0 * out_snr.numel() * 4 / 1e9
             extras["flux"] = {"ms": ms, "achieved_gbs": gb / ms * 1e3, "peak_gbs": hbm}
         jit = (0.4 * np.random.default_rng(cfg.idx).standard_normal((cfg.T, 2))).astype(np.float32)
+        if cfg.H % 4 == 0 and cfg.W == cfg.H and cfg.H >= 64:
+            # the paper's low-resolution scattered-light solve (section 3.1) at this stack's size: N = H / 4, n = N / 8;
+            # synthetic input of its own (DESIGN 8g): scattered light per frame + jittered background + noise
+            import paper_2209_09848_b200 as P
+            N, n = cfg.H // 4, cfg.H // 32
+            gen = torch.Generator(device=dev)
+            gen.manual_seed(cfg.idx)
+            low = torch.empty((cfg.T, N, N), device=dev)
+            ms = timed(lambda: P.tno_mf_downsample(mf.ctx, frames, 4, low))
+            extras["downsample"] = {"ms": ms, "achieved_gbs": frames.numel() * 4 * (1 + 1 / 16) / 1e6 / ms, "peak_gbs": hbm}
+            phi = torch.from_numpy(np.stack([np.ones(cfg.T), jit[:, 0], jit[:, 1], jit[:, 0] ** 2, jit[:, 1] ** 2,
+                                             jit[:, 0] * jit[:, 1]], 1).astype(np.float32)).to(dev)
+            beta = torch.randn((6, N, N), device=dev, generator=gen) * torch.tensor([20., 3, 3, 1, 1, 1], device=dev)[:, None, None]
+            S = 10 + 5 * torch.randn((cfg.T, n, n), device=dev, generator=gen)
+            low = torch.nn.functional.interpolate(S[None], size=(N, N), mode="bilinear", align_corners=False)[0]
+            low = (low + torch.einsum("tk,kij->tij", phi, beta)
+                   + 0.3 * torch.randn((cfg.T, N, N), device=dev, generator=gen)).contiguous()
+            b = torch.zeros((6, N, N), device=dev)
+            s = torch.zeros((cfg.T, n, n), device=dev)
+            torch.cuda.synchronize()
+            t_fit = time.perf_counter()
+            loss, iters, evals = P.tno_mf_scatter_fit(mf.ctx, low, jit, 1.0, 1000, 0.0, b, s)      # blocking call
+            t_fit = time.perf_counter() - t_fit
+            extras["scatter_fit"] = {"seconds": t_fit, "iterations": iters, "loss_evaluations": evals,
+                                     "launches": mf.stats()[0], "final_loss_per_sample": loss / low.numel(),
+                                     "N": N, "n": n, "paper_a100_seconds": 40.0}
+            ms = timed(lambda: P.tno_mf_scatter_subtract(mf.ctx, frames, s), reps=1)
+            extras["scatter_subtract"] = {"ms": ms, "achieved_gbs": 2.0 * frames.numel() * 4 / 1e6 / ms, "peak_gbs": hbm}
+            del low, beta, S, b, s
         for n_iter in (0, 10):
             ms = timed(lambda: mf.background(frames, jit, 1.0, n_iter, in_place=True), reps=2)
             gb = (n_iter + 3.0) * frames.numel() * 4 / 1e9
