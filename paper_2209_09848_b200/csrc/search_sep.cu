@@ -530,9 +530,11 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
 }
 
 // ------------------------------------------------------------------------------------ host side
-// (rows per thread, entries per batch, consumer warps, box stages, X buffers): tile 60 positions x
-// 64 columns, 384 consumer + 128 producer threads
-using V0 = SepCfg<5, 8, 12, 4, 4>;
+// (rows per thread, entries per batch, consumer warps, box stages, X buffers): tiles of 12 R positions x
+// 64 columns, 384 consumer + 128 producer threads.  Both variants fill the consumers' 152 registers with
+// accumulators: 7 rows x 8 entries (112 + 22 window registers, 280 FFMA2 per frame and warp) and 5 rows x 10
+// entries (100 + 18, 250 FFMA2); 6 x 10 spills and is slower, 5 x 8 leaves registers idle (measured: DESIGN.md)
+using V0 = SepCfg<7, 8, 12, 4, 4>;
 using V1 = SepCfg<5, 10, 12, 4, 4>;
 
 int32_t sep_num_variants() { return 2; }
