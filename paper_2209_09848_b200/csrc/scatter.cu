@@ -158,21 +158,31 @@ k_scatter_gs_cols(const float *__restrict__ psi, int32_t N, int32_t n, const int
     };
     float acc0 = 0.f, acc1 = 0.f;
     int32_t cur = __ldg(bi0);
-    for (int32_t i = 0; i < N; ++i) {
-        const int32_t a0 = __ldg(bi0 + i);
-        const float w = __ldg(bw + i);
-        if (a0 != cur) {                         // uniform over the block: the input row advances by one
-            flush(cur, acc0);
-            acc0 = acc1;
-            acc1 = 0.f;
-            cur = a0;
-        }
-        const float v = active ? __ldcs(P + (int64_t)i * N + j) : 0.f;
-        if (a0 + 1 <= n - 1) {
-            acc0 = fmaf(1.f - w, v, acc0);
-            acc1 = fmaf(w, v, acc1);
-        } else {
-            acc0 += v;                           // clamped: both stencil points are the last input row
+    constexpr int kAhead = 8;                    // rows loaded before they are used: 8 loads in flight per thread
+    for (int32_t ib = 0; ib < N; ib += kAhead) {
+        float vv[kAhead];
+#pragma unroll
+        for (int k = 0; k < kAhead; ++k)
+            vv[k] = (active && ib + k < N) ? __ldcs(P + (int64_t)(ib + k) * N + j) : 0.f;
+#pragma unroll
+        for (int k = 0; k < kAhead; ++k) {
+            const int32_t i = ib + k;
+            if (i < N) {
+                const int32_t a0 = __ldg(bi0 + i);
+                const float w = __ldg(bw + i);
+                if (a0 != cur) {                 // uniform over the block: the input row advances by one
+                    flush(cur, acc0);
+                    acc0 = acc1;
+                    acc1 = 0.f;
+                    cur = a0;
+                }
+                if (a0 + 1 <= n - 1) {
+                    acc0 = fmaf(1.f - w, vv[k], acc0);
+                    acc1 = fmaf(w, vv[k], acc1);
+                } else {
+                    acc0 += vv[k];               // clamped: both stencil points are the last input row
+                }
+            }
         }
     }
     flush(cur, acc0);
