@@ -164,3 +164,43 @@ def test_config5_curved_topk_only():
         v = c[k][c[k]["x"] >= 0]
         assert np.all(v["snr"][:-1] >= v["snr"][1:]) and np.all(v["snr"] >= cfg.threshold)
     mf.close()
+
+
+def test_background_and_fused_max_at_full_size():
+    """tno_mf_background on the config-3 stack (16.8 GB, in place, the launch bench.py --extras times): every pixel's
+    fit is independent, so the oracle computes 4000 sampled pixels (and the four corners) exactly as it would the whole
+    stack.  Then tno_mf_search_max on the residual stack against tno_mf_best of the same maps at full size."""
+    cfg = tno_synth.CONFIGS[3]
+    torch, mf, p, frames = _setup(cfg)
+    T, H, W = frames.shape
+    rng = np.random.default_rng(5)
+    jit = (0.3 * rng.standard_normal((T, 2))).astype(np.float32)
+    # give the stack something to fit: a per-pixel background that moves with the jitter (on the device)
+    gen = torch.Generator(device=frames.device)
+    gen.manual_seed(3)
+    phi = torch.from_numpy(oracle.background_basis(jit).astype(np.float32)).to(frames.device)
+    beta = torch.randn((6, H, W), device=frames.device, generator=gen) * \
+        torch.tensor([30.0, 4, 4, 1.5, 1.5, 1.5], device=frames.device)[:, None, None]
+    for t0 in range(0, T, 50):
+        frames[t0:t0 + 50] += torch.einsum("tk,khw->thw", phi[t0:t0 + 50], beta)
+    del beta
+    ys = np.concatenate([rng.integers(0, H, 4000), [0, 0, H - 1, H - 1]])
+    xs = np.concatenate([rng.integers(0, W, 4000), [0, W - 1, 0, W - 1]])
+    iy, ix = torch.from_numpy(ys).to(frames.device), torch.from_numpy(xs).to(frames.device)
+    before = frames[:, iy, ix].cpu().numpy()                       # [T, n_sample]
+    delta, n_iter = 1.5, 6
+    coef, resid = mf.background(frames, jit, delta, n_iter, in_place=True)
+    torch.cuda.synchronize()
+    assert resid.data_ptr() == frames.data_ptr()
+    ob, orr = oracle.background(before[:, None, :], jit, delta, n_iter)     # a [T, 1, n_sample] "stack"
+    scale = float(np.abs(before).max())
+    got_r = frames[:, iy, ix].cpu().numpy()
+    got_c = coef[:, iy, ix].cpu().numpy()
+    assert np.abs(got_r - orr[:, 0, :]).max() <= 5e-5 * scale           # float32 sums over 1000 frames
+    assert np.abs(got_c - ob[:, 0, :]).max() <= 5e-4 * scale
+    # fused max over the bank on the residual stack == best() of the maps of the same search
+    mx, ak, maps, _ = mf.search_max(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0, want_maps=True)
+    bm, ba, _, _ = mf.best(maps)
+    torch.cuda.synchronize()
+    assert torch.equal(mx, bm) and torch.equal(ak, ba)
+    mf.close()
