@@ -98,6 +98,156 @@ k_scatter_resid(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, co
     block_sum_to(loss, partials);
 }
 
+// ---- bulk-copy staged variant of k_scatter_resid (N % 4 == 0, aligned): the structure of k_background_bulk --------
+// 128 consumer threads own four neighbouring pixels of a row each; a fifth warp requests every frame's 512 pixels
+// as one cp.async.bulk (2 KB, one address translation) into a ring of 3 stages x 8 frames together with the 8 rows of
+// phi.  The walk over the frames with ordinary loads (k_scatter_resid) is bound by TLB misses and by the few
+// loads a thread can keep in flight (1.7 TB/s); see DESIGN.md 8f / 8g.
+__device__ __forceinline__ uint32_t sc_smem(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sc_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}\n"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+
+template <int NT, int NS, int FS, int SF /* floats of S staged per frame */>
+__global__ void __launch_bounds__(NT + 32, 2048 / (NT + 32) > 4 ? 4 : 2048 / (NT + 32))
+k_scatter_resid_bulk(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, const float *__restrict__ phi,
+                     const int32_t *__restrict__ bi0, const float *__restrict__ bw, float delta,
+                     const float *__restrict__ beta, const float *__restrict__ S, float *__restrict__ psi,
+                     float *__restrict__ g_beta, double *__restrict__ partials) {
+    constexpr int PX = 2;                                        // neighbouring pixels per thread
+    constexpr int PXF = NT * PX, STAGE = FS * (PXF + 8 + SF);
+    extern __shared__ __align__(128) float ring[];               // [NS][STAGE]: FS x pixels, FS x phi, FS x rows of S_t
+    __shared__ __align__(8) uint64_t bars[2 * NS];
+    __shared__ double wsum[NT / 32];
+    const uint32_t full = sc_smem(bars), empty = full + 8 * NS;
+    const int32_t tid = threadIdx.x, lane = tid & 31;
+    const int64_t n_px = (int64_t)N * N;
+    const int64_t p0 = (int64_t)blockIdx.x * PXF, left = n_px - p0;
+    const uint32_t bytes = (uint32_t)(left < PXF ? left : PXF) * 4u;
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(full + 8 * s), "r"(1));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty + 8 * s), "r"(NT / 32));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int32_t total = (T + FS - 1) / FS;
+    // the rows of S_t that the pixels of this block touch: [ra, ra + nr), nr * n <= SF floats (checked by the host)
+    const int64_t p_last = p0 + (left < PXF ? left : PXF) - 1;
+    const int32_t ra = bi0[(int32_t)(p0 / N)], rb = min(bi0[(int32_t)(p_last / N)] + 1, n - 1);
+    const uint32_t sbytes = (uint32_t)(rb - ra + 1) * n * 4u;
+    if (tid >= NT) {
+        if (lane == 0) {
+            for (int32_t g = 0; g < total; ++g) {
+                const uint32_t s = (uint32_t)g % NS, bar = full + 8 * s, dst = sc_smem(ring + s * STAGE);
+                if (g >= NS) sc_wait(empty + 8 * s, ((uint32_t)(g / NS) - 1u) & 1u);
+                const int32_t t0 = g * FS, nf = min(FS, T - t0);
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(nf * (bytes + 32u + sbytes))
+                             : "memory");
+                for (int32_t f = 0; f < nf; ++f)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                                     "r"(dst + f * (PXF * 4)), "l"(D + (int64_t)(t0 + f) * n_px + p0), "r"(bytes), "r"(bar)
+                                 : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                                 "r"(dst + FS * (PXF * 4)), "l"(phi + 8 * (int64_t)t0), "r"(nf * 32u), "r"(bar)
+                             : "memory");
+                for (int32_t f = 0; f < nf; ++f)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                                     "r"(dst + (FS * (PXF + 8) + f * SF) * 4), "l"(S + ((int64_t)(t0 + f) * n + ra) * n),
+                                     "r"(sbytes), "r"(bar)
+                                 : "memory");
+            }
+        }
+        return;
+    }
+    const bool live = (int64_t)tid * PX < left;
+    const int64_t p = p0 + (int64_t)tid * PX;
+    const int32_t i = live ? (int32_t)(p / N) : 0, j = live ? (int32_t)(p % N) : 0;     // PX pixels of one row: N % 4 == 0
+    const int32_t i0 = bi0[i], i1 = min(i0 + 1, n - 1);
+    const float wy = bw[i];
+    int32_t o0[PX], dj[PX];
+    float wx[PX];
+#pragma unroll
+    for (int k = 0; k < PX; ++k) {
+        const int32_t j0 = bi0[j + k];
+        o0[k] = (i0 - ra) * n + j0;
+        dj[k] = min(j0 + 1, n - 1) - j0;
+        wx[k] = bw[j + k];
+    }
+    const int32_t di = (i1 - i0) * n;
+    float b[6][PX], g[6][PX];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float2 v = live ? *reinterpret_cast<const float2 *>(beta + k * n_px + p) : make_float2(0.f, 0.f);
+        b[k][0] = v.x; b[k][1] = v.y;
+        g[k][0] = g[k][1] = 0.f;
+    }
+    double loss = 0.0;
+    uint32_t st = 0, par = 0;
+    for (int32_t t0 = 0; t0 < T; t0 += FS) {
+        sc_wait(full + 8 * st, par);
+        const float *sp = ring + st * STAGE;
+        float lsum = 0.f;
+#pragma unroll
+        for (int f = 0; f < FS; ++f) {
+            if (t0 + f < T) {
+                const float2 dv = reinterpret_cast<const float2 *>(sp + f * PXF)[tid];
+                const float4 qa = *reinterpret_cast<const float4 *>(sp + FS * PXF + f * 8);
+                const float2 qb = *reinterpret_cast<const float2 *>(sp + FS * PXF + f * 8 + 4);
+                const float q[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
+                const float d4[PX] = {dv.x, dv.y};
+                const float *St = sp + FS * (PXF + 8) + f * SF;
+                float c4[PX];
+#pragma unroll
+                for (int k = 0; k < PX; ++k) {
+                    const float a00 = St[o0[k]], a01 = St[o0[k] + dj[k]];
+                    const float a10 = St[o0[k] + di], a11 = St[o0[k] + di + dj[k]];
+                    // the same expression as k_scatter_resid: four weights times four values
+                    float pred = (1.f - wy) * (1.f - wx[k]) * a00 + (1.f - wy) * wx[k] * a01 + wy * (1.f - wx[k]) * a10 +
+                                 wy * wx[k] * a11;
+#pragma unroll
+                    for (int m = 0; m < 6; ++m) pred = fmaf(q[m], b[m][k], pred);
+                    const float r = d4[k] - pred;
+                    const float a = fabsf(r);
+                    lsum += a <= delta ? 0.5f * r * r : delta * (a - 0.5f * delta);       // Eq. 4
+                    const float c = fminf(fmaxf(r, -delta), delta);
+                    c4[k] = c;
+#pragma unroll
+                    for (int m = 0; m < 6; ++m) g[m][k] = fmaf(q[m], c, g[m][k]);
+                }
+                if (live)
+                    *reinterpret_cast<float2 *>(psi + (int64_t)(t0 + f) * n_px + p) = make_float2(c4[0], c4[1]);
+            }
+        }
+        if (live) loss += (double)lsum;
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty + 8 * st) : "memory");
+        if (++st == NS) { st = 0; par ^= 1u; }
+    }
+    if (live) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k)
+            *reinterpret_cast<float2 *>(g_beta + k * n_px + p) = make_float2(-g[k][0], -g[k][1]);
+    }
+    // loss of the block in a fixed order (consumer warps only: the producer warp has left)
+    for (int o = 16; o > 0; o >>= 1) loss += __shfl_down_sync(0xffffffffu, loss, o);
+    if (lane == 0) wsum[tid >> 5] = loss;
+    asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory");
+    if (tid == 0) {
+        double s = 0.0;
+        for (int w = 0; w < NT / 32; ++w) s += wsum[w];
+        partials[blockIdx.x] = s;
+    }
+}
+
 // dL/dS[t][a][b] = - sum_{i,j} wy(i, a) wx(j, b) psi[t][i][j]: only pixels within one input pixel of (a, b) count
 __global__ void __launch_bounds__(256)
 k_scatter_gs(const float *__restrict__ psi, int32_t T, int32_t N, int32_t n, const int32_t *__restrict__ bi0,
@@ -285,9 +435,25 @@ void launch_scatter_subtract(cudaStream_t st, float *frames, int32_t T, int32_t 
 int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float *beta, const float *S, float *psi,
                          double *partials, float *g_beta, float *g_S, double *loss_dev) {
     const int64_t n_px = (int64_t)pb.N * pb.N;
-    const int32_t blocks = (int32_t)((n_px + 255) / 256);
-    k_scatter_resid<<<(unsigned)blocks, 256, 0, st>>>(pb.D, pb.T, pb.N, pb.n, pb.phi, pb.bi0, pb.bw, pb.delta, beta, S, psi,
-                                                     g_beta, partials);
+    int32_t blocks;
+    const bool aligned = ((reinterpret_cast<uintptr_t>(pb.D) | reinterpret_cast<uintptr_t>(beta) |
+                           reinterpret_cast<uintptr_t>(psi) | reinterpret_cast<uintptr_t>(g_beta)) & 15u) == 0;
+    constexpr int NT = 256, NS = 2, FS = 8, SF = 192;     // 45.6 KB per CTA: four CTAs per SM, all 512 blocks of N = 512 resident
+    // rows of S a block of NT * 2 pixels can touch: those under its first and last image row, plus one
+    const int64_t img_rows = std::min<int64_t>(pb.N, (NT * 2 + pb.N - 2) / pb.N + 1);
+    const int64_t s_rows = std::min<int64_t>(pb.n, (img_rows * pb.n + pb.N - 1) / pb.N + 2);
+    if (pb.N % 4 == 0 && pb.n % 4 == 0 && s_rows * pb.n <= SF && aligned &&
+        (reinterpret_cast<uintptr_t>(S) & 15u) == 0) {
+        constexpr int smem = NS * FS * (NT * 2 + 8 + SF) * 4;
+        blocks = (int32_t)((n_px + NT * 2 - 1) / (NT * 2));
+        cudaFuncSetAttribute(k_scatter_resid_bulk<NT, NS, FS, SF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        k_scatter_resid_bulk<NT, NS, FS, SF><<<(unsigned)blocks, NT + 32, smem, st>>>(pb.D, pb.T, pb.N, pb.n, pb.phi, pb.bi0, pb.bw,
+                                                                                pb.delta, beta, S, psi, g_beta, partials);
+    } else {
+        blocks = (int32_t)((n_px + 255) / 256);
+        k_scatter_resid<<<(unsigned)blocks, 256, 0, st>>>(pb.D, pb.T, pb.N, pb.n, pb.phi, pb.bi0, pb.bw, pb.delta, beta, S,
+                                                         psi, g_beta, partials);
+    }
     k_sum_partials<<<1, 256, 0, st>>>(partials, blocks, 0, loss_dev);
     if (pb.N <= 1024) {
         const int32_t threads = ((std::max(pb.N, pb.n) + 31) / 32) * 32;

@@ -30,7 +30,8 @@ def _problem(seed, T, N, n, noise=0.3, outliers=0.02):
 
 
 @pytest.mark.parametrize("T,N,n", [(9, 24, 3), (5, 64, 8), (17, 40, 5), (3, 16, 16), (6, 33, 4),
-                                   (2, 1040, 13)])          # N > 1024: the gather form of the S gradient
+                                   (2, 1040, 13),           # N > 1024: the gather form of the S gradient
+                                   (11, 36, 4), (3, 512, 64)])    # staged kernel: ragged last block, T % 8 != 0; paper size
 def test_loss_and_gradient_match_oracle(T, N, n):
     torch = _torch()
     import paper_2209_09848_b200 as P
