@@ -378,6 +378,38 @@ k_sum_partials(const double *__restrict__ partials, int32_t n, int32_t take_max,
     }
     if (threadIdx.x == 0) out[0] = sh[0];
 }
+// The scalars of the two-loop recursion stay on the device (sc[]): the final stage of a reduction applies the
+// recursion's formula and leaves the coefficient of the next vector update in sc[2], so the host enqueues the whole
+// recursion without reading anything back.  sc[0], sc[1]: results for the host; sc[3]: |g|_inf;
+// sc[8 + i]: rho_i; sc[8 + kScatterHistory + i]: alpha_i.
+enum ScalarOp { kStore0 = 0, kAlpha = 1, kBeta = 3, kStore1 = 4 };
+__global__ void __launch_bounds__(256)
+k_reduce_op(const double *__restrict__ partials, int32_t n, int32_t op, int32_t i, double *__restrict__ sc) {
+    __shared__ double sh[256];
+    double s = 0.0;
+    for (int32_t k = threadIdx.x; k < n; k += 256) s += partials[k];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        s = sh[0];
+        double *rho = sc + 8, *alpha = sc + 8 + kScatterHistory;
+        if (op == kStore0) sc[0] = s;
+        else if (op == kStore1) sc[1] = s;
+        else if (op == kAlpha) { alpha[i] = rho[i] * s; sc[2] = -alpha[i]; }          // q -= alpha_i y_i
+        else if (op == kBeta) sc[2] = alpha[i] - rho[i] * s;                           // r += (alpha_i - beta) s_i
+    }
+}
+// z = x + (float)coef[0] * y   (z may alias x or y)
+__global__ void __launch_bounds__(256)
+k_axpy_dev(const float *x, const double *__restrict__ coef, const float *y, int64_t n, float *z) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const float c = (float)coef[0];
+    if (i < n) z[i] = x[i] + c * y[i];
+}
 // z = a x + b y   (z may alias x or y)
 __global__ void __launch_bounds__(256)
 k_axpby(float a, const float *x, float b, const float *y, int64_t n, float *z) {
@@ -475,7 +507,7 @@ int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float 
 size_t scatter_ws_bytes(int32_t T, int32_t N, int32_t n) {
     const size_t P = (size_t)6 * N * N + (size_t)T * n * n;
     const size_t blocks = std::max<size_t>(kRedBlocks, ((size_t)N * N + 255) / 256);
-    return (5 + 2 * (size_t)kScatterHistory) * P * 4 + (size_t)T * N * N * 4 + (blocks + 8) * 8 + 256;
+    return (5 + 2 * (size_t)kScatterHistory) * P * 4 + (size_t)T * N * N * 4 + (blocks + 8 + 2 * kScatterHistory) * 8 + 256;
 }
 
 int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, float *S, void *ws, int32_t max_iter,
@@ -486,7 +518,7 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
     float *hs = d + P, *hy = hs + (size_t)kScatterHistory * P, *psi = hy + (size_t)kScatterHistory * P;
     double *partials = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(psi + (size_t)pb.T * pb.N * pb.N) + 15) &
                                                   ~(uintptr_t)15);
-    double *scal = partials + blocks;
+    double *scal = partials + blocks;            // 8 + 2 * kScatterHistory doubles (k_reduce_op)
     int32_t launches = 0, evals = 0;
     cudaError_t err = cudaSuccess;
     auto fetch = [&](double *dev) -> double {
@@ -496,14 +528,21 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
         if (e != cudaSuccess) err = e;
         return h;
     };
-    auto dot = [&](const float *a, const float *b) -> double {
+    auto dot_to = [&](const float *a, const float *b, int32_t op, int32_t i) {      // no read-back
         k_dot<<<kRedBlocks, 256, 0, st>>>(a, b, P, partials);
-        k_sum_partials<<<1, 256, 0, st>>>(partials, kRedBlocks, 0, scal);
+        k_reduce_op<<<1, 256, 0, st>>>(partials, kRedBlocks, op, i, scal);
         launches += 2;
+    };
+    auto dot = [&](const float *a, const float *b) -> double {
+        dot_to(a, b, kStore0, 0);
         return fetch(scal);
     };
     auto axpby = [&](float a, const float *xx, float b, const float *yy, float *zz) {
         k_axpby<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(a, xx, b, yy, P, zz);
+        launches += 1;
+    };
+    auto axpy_dev = [&](const float *xx, const float *yy, float *zz) {                // zz = xx + sc[2] * yy
+        k_axpy_dev<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(xx, scal + 2, yy, P, zz);
         launches += 1;
     };
     auto eval = [&](const float *xx, float *gg) -> double {
@@ -514,32 +553,35 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
     cudaMemcpyAsync(x, beta, nb * 4, cudaMemcpyDeviceToDevice, st);
     cudaMemcpyAsync(x + nb, S, ns * 4, cudaMemcpyDeviceToDevice, st);
     double f = eval(x, g);
-    std::vector<double> rho(kScatterHistory), alpha(kScatterHistory);
+    std::vector<double> gamma(kScatterHistory);          // s.y / y.y of each pair (initial scaling of the recursion)
     int32_t hist = 0, head = 0, it = 0;          // pairs stored, slot of the next pair
     int32_t stalled = 0;                         // consecutive iterations without a relevant decrease
     for (; it < max_iter && err == cudaSuccess; ++it) {
         k_absmax<<<kRedBlocks, 256, 0, st>>>(g, P, partials);
-        k_sum_partials<<<1, 256, 0, st>>>(partials, kRedBlocks, 1, scal);
+        k_sum_partials<<<1, 256, 0, st>>>(partials, kRedBlocks, 1, scal + 3);
         launches += 2;
-        if (fetch(scal) <= (double)gtol) break;
-        // d = -H g
+        // d = H g by the two-loop recursion, every scalar of it on the device
         axpby(1.f, g, 0.f, g, d);
         for (int32_t c = 0; c < hist; ++c) {
             const int32_t i = (head - 1 - c + 2 * kScatterHistory) % kScatterHistory;
-            alpha[i] = rho[i] * dot(hs + (size_t)i * P, d);
-            axpby(1.f, d, (float)-alpha[i], hy + (size_t)i * P, d);
+            dot_to(hs + (size_t)i * P, d, kAlpha, i);
+            axpy_dev(d, hy + (size_t)i * P, d);
         }
-        if (hist > 0) {
-            const int32_t l = (head - 1 + kScatterHistory) % kScatterHistory;
-            const double yy = dot(hy + (size_t)l * P, hy + (size_t)l * P);
-            axpby((float)(1.0 / (rho[l] * yy)), d, 0.f, d, d);
-        }
+        if (hist > 0) axpby((float)gamma[(head - 1 + kScatterHistory) % kScatterHistory], d, 0.f, d, d);
         for (int32_t c = hist - 1; c >= 0; --c) {
             const int32_t i = (head - 1 - c + 2 * kScatterHistory) % kScatterHistory;
-            const double b = rho[i] * dot(hy + (size_t)i * P, d);
-            axpby(1.f, d, (float)(alpha[i] - b), hs + (size_t)i * P, d);
+            dot_to(hy + (size_t)i * P, d, kBeta, i);
+            axpy_dev(d, hs + (size_t)i * P, d);
         }
-        double dg = -dot(g, d);                  // directional derivative along -d
+        dot_to(g, d, kStore0, 0);
+        double h4[4];                            // one read-back per direction: g.d and |g|_inf
+        {
+            cudaError_t e = cudaMemcpyAsync(h4, scal, 32, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) { err = e; break; }
+        }
+        if (h4[3] <= (double)gtol) break;
+        double dg = -h4[0];                      // directional derivative along -d
         if (!(dg < 0.0)) {                       // not a descent direction: steepest descent, empty history
             hist = 0;
             axpby(1.f, g, 0.f, g, d);
@@ -560,9 +602,20 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
         float *s_new = hs + (size_t)head * P, *y_new = hy + (size_t)head * P;
         axpby(1.f, xn, -1.f, x, s_new);
         axpby(1.f, gn, -1.f, g, y_new);
-        const double sy = dot(s_new, y_new), yy = dot(y_new, y_new);
+        dot_to(s_new, y_new, kStore0, 0);
+        dot_to(y_new, y_new, kStore1, 0);
+        double h2[2];
+        {
+            cudaError_t e = cudaMemcpyAsync(h2, scal, 16, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) { err = e; break; }
+        }
+        const double sy = h2[0], yy = h2[1];
         if (sy > 1e-10 * yy && yy > 0.0) {
-            rho[head] = 1.0 / sy;
+            const double r = 1.0 / sy;           // rho of the new pair, to the device scalars
+            cudaMemcpyAsync(scal + 8 + head, &r, 8, cudaMemcpyHostToDevice, st);
+            cudaStreamSynchronize(st);           // r is a local
+            gamma[head] = sy / yy;
             head = (head + 1) % kScatterHistory;
             hist = std::min(hist + 1, kScatterHistory);
         }
