@@ -284,31 +284,42 @@ k_scatter_gs(const float *__restrict__ psi, int32_t T, int32_t N, int32_t n, con
 __global__ void __launch_bounds__(1024)
 k_scatter_gs_cols(const float *__restrict__ psi, int32_t N, int32_t n, const int32_t *__restrict__ bi0,
                   const float *__restrict__ bw, const int32_t *__restrict__ blo, const int32_t *__restrict__ bhi,
-                  float *__restrict__ g_S) {
-    extern __shared__ float C[];                 // [N]
-    const int32_t t = blockIdx.x, j = threadIdx.x;
-    const bool active = j < N;
+                  int32_t strip_b, int32_t max_sup, float *__restrict__ g_S) {
+    // blockIdx.y: a strip of strip_b input columns b and the image columns under them (strips overlap by the width of
+    // a stencil; more, smaller blocks keep more loads in flight than one block per frame)
+    extern __shared__ float C[];                 // [blockDim.x] column sums, then [strip_b][max_sup] weights
+    float *Wt = C + blockDim.x;
+    const int32_t t = blockIdx.x, tid = threadIdx.x;
+    const int32_t b0 = blockIdx.y * strip_b, b1 = min(n, b0 + strip_b);
+    const int32_t c_lo = blo[b0], c_hi = bhi[b1 - 1];
+    const int32_t j = c_lo + tid;
+    const bool active = j <= c_hi;
     const float *P = psi + (int64_t)t * N * N;
     float *out = g_S + (int64_t)t * n * n;
-    const int32_t my_lo = j < n ? blo[j] : 0, my_hi = j < n ? bhi[j] : -1;
+    const int32_t b = b0 + tid;
+    const int32_t my_lo = b < b1 ? blo[b] : 0, my_hi = b < b1 ? min(bhi[b], blo[b] + max_sup - 1) : -1;
+    // the weights of input column b over its support, once (the support is at most max_sup image columns wide)
+    if (b < b1)
+        for (int32_t c = my_lo; c <= my_hi; ++c) {
+            const int32_t c0 = __ldg(bi0 + c), c1 = min(c0 + 1, n - 1);
+            const float v = __ldg(bw + c);
+            Wt[tid * max_sup + (c - my_lo)] = (c0 == b ? 1.f - v : 0.f) + (c1 == b ? v : 0.f);
+        }
+    const float *myW = Wt + tid * max_sup, *myC = C + (my_lo - c_lo);
+    const int32_t my_n = my_hi - my_lo + 1;
     auto flush = [&](int32_t a, float acc) {
-        if (active) C[j] = acc;
+        if (active) C[tid] = acc;
         __syncthreads();
-        if (j < n) {
+        if (b < b1) {
             float sum = 0.f;
-            for (int32_t c = my_lo; c <= my_hi; ++c) {
-                const int32_t c0 = __ldg(bi0 + c), c1 = min(c0 + 1, n - 1);
-                const float v = __ldg(bw + c);
-                const float wx = (c0 == j ? 1.f - v : 0.f) + (c1 == j ? v : 0.f);
-                sum = fmaf(wx, C[c], sum);
-            }
-            out[a * n + j] = -sum;
+            for (int32_t c = 0; c < my_n; ++c) sum = fmaf(myW[c], myC[c], sum);
+            out[a * n + b] = -sum;
         }
         __syncthreads();
     };
     float acc0 = 0.f, acc1 = 0.f;
     int32_t cur = __ldg(bi0);
-    constexpr int kAhead = 8;                    // rows loaded before they are used: 8 loads in flight per thread
+    constexpr int kAhead = 16;                    // rows loaded before they are used: 8 loads in flight per thread
     for (int32_t ib = 0; ib < N; ib += kAhead) {
         float vv[kAhead];
 #pragma unroll
@@ -488,9 +499,14 @@ int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float 
     }
     k_sum_partials<<<1, 256, 0, st>>>(partials, blocks, 0, loss_dev);
     if (pb.N <= 1024) {
-        const int32_t threads = ((std::max(pb.N, pb.n) + 31) / 32) * 32;
-        k_scatter_gs_cols<<<(unsigned)pb.T, threads, (size_t)pb.N * 4, st>>>(psi, pb.N, pb.n, pb.bi0, pb.bw, pb.blo, pb.bhi,
-                                                                           g_S);
+        // strips of input columns: 4 for the paper's n = 64; image columns of a strip <= N / strips + two stencils
+        const int32_t n_strip = pb.n >= 16 ? 4 : 1, strip_b = (pb.n + n_strip - 1) / n_strip;
+        const int32_t cols = std::min(pb.N, (pb.N + n_strip - 1) / n_strip + 2 * ((pb.N + pb.n - 1) / pb.n) + 4);
+        const int32_t threads = ((std::max(cols, strip_b) + 31) / 32) * 32;
+        const int32_t max_sup = 2 * ((pb.N + pb.n - 1) / pb.n) + 4;          // image columns under one input column
+        dim3 grid((unsigned)pb.T, (unsigned)((pb.n + strip_b - 1) / strip_b));
+        k_scatter_gs_cols<<<grid, threads, ((size_t)threads + (size_t)strip_b * max_sup) * 4, st>>>(
+            psi, pb.N, pb.n, pb.bi0, pb.bw, pb.blo, pb.bhi, strip_b, max_sup, g_S);
     } else {
         const int64_t ns = (int64_t)pb.T * pb.n * pb.n;
         k_scatter_gs<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(psi, pb.T, pb.N, pb.n, pb.bi0, pb.bw, g_S);
