@@ -194,7 +194,7 @@ def run_ours(args, cfg):
         step()
     torch.cuda.synchronize()
     launches_per_step, used_kernel = mf.stats()
-    fma_x, fma_y = mf.work()
+    fma_x, fma_y, add_y = mf.work()
 
     # ---- timed region: K steps, device-timed, max over ranks
     sampler = ClockSampler(local)
@@ -244,11 +244,19 @@ def run_ours(args, cfg):
         e1.record()
         torch.cuda.synchronize()
         e2e_ms = multi.max_over_ranks(e0.elapsed_time(e1) / e2e_steps, dev)
+        # outside the timed region: the host-buffer call must return, bit for bit, what the timed device search
+        # left in out_snr / out_topk (same stack, same bank)
+        step()
+        torch.cuda.synchronize()
+        same = bool(torch.equal(host_topk, out_topk.cpu()))
+        if cfg.want_maps:
+            for k0 in range(0, cfg.n_traj, 16):           # by slices: no second 1.7 GB host copy
+                same = same and bool(torch.equal(host_snr[k0:k0 + 16], out_snr[k0:k0 + 16].cpu()))
         h2d = frames.numel() * 4
         d2h = out_topk.numel() * 4 + (out_snr.numel() * 4 if cfg.want_maps else 0)
         e2e = {"value": multi.aggregate_value(cfg.evals, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
                "steps": e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "host_memory": "pinned" if pinned else "pageable",
+               "host_memory": "pinned" if pinned else "pageable", "equals_device_search": same,
                "api": "tno_mf_search_host (upload in bands of frame rows, overlapped with the search)"}
         del host_frames, host_snr
     except RuntimeError as ex:            # e.g. not enough host memory for the stack
@@ -261,20 +269,26 @@ def run_ours(args, cfg):
     clk_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * clk_hz / 1e12
     k_s = float(np.mean(kernel_ms)) * 1e-3
-    flops = 2.0 * (fma_x + fma_y)
+    flops = 2.0 * (fma_x + fma_y) + add_y        # an addition occupies a lane of the FP32 pipe like a multiply-add, counts 1
     achieved = flops / k_s / 1e12
-    traffic = None
+    # dram__bytes_read + write of one launch, from the committed ncu --set full capture (a stored figure: the
+    # source file names the commit and the profile it was measured at, printed beside it so a stale one shows)
+    traffic, traffic_src = None, None
     tp = os.path.join(ROOT, "profiles", "dram_traffic.json")
     if os.path.exists(tp):
         with open(tp) as f:
-            traffic = json.load(f).get("cfg%d" % cfg.idx)
+            tj = json.load(f)
+        traffic = tj.get("cfg%d" % cfg.idx)
+        traffic_src = {"file": "profiles/dram_traffic.json", "measured_at_commit": tj.get("measured_at_commit"),
+                       "profile": tj.get("profile")}
     roofline = {"bound": "alu", "kernel": "k_search_sep" if used_kernel == 1 else "k_search_generic",
                 "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                "traffic": traffic,
+                "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz, %s)" % (
                     n_sm, clk_hz / 1e6, peaks_src),
                 "kernel_ms": k_s * 1e3, "kernel_share_of_step": k_s * 1e3 / ms_per_step,
-                "fma_per_eval_executed": (fma_x + fma_y) / cfg.evals,
+                "fma_per_eval_executed": (fma_x + fma_y) / cfg.evals, "add_per_eval_executed": add_y / cfg.evals,
+                "pipe_frac": (fma_x + fma_y + add_y) / k_s / (n_sm * FP32_LANES_PER_SM * clk_hz),
                 "frac_vs_25fma_definition": (2.0 * 25.0 * cfg.evals / k_s / 1e12) / peak_tflops,
                 "hbm_compulsory_gbs": (frames.numel() * 4 + (out_snr.numel() * 4 if cfg.want_maps else 0)) / k_s / 1e9,
                 "hbm_peak_gbs": peaks.get("hbm_gbs")}

@@ -27,7 +27,8 @@
  *     synchronises that stream.  Host arrays are consumed before return.
  *   - Every function returns 0 on success or a negative TNO_MF_E* code; no exceptions, no
  *     exit().  After a failure tno_mf_last_error(ctx) describes it; outputs are unspecified.
- *   - A context is not thread-safe; distinct contexts are independent.  No global state.
+ *   - A context is not thread-safe; distinct contexts are independent.  The only state outside a context is
+ *     the thread-local text of the last tno_mf_create failure (tno_mf_last_error(NULL)).
  *   - There is no CPU fallback: without a CUDA device of compute capability 10.x,
  *     tno_mf_create fails with TNO_MF_EUNSUPPORTED / TNO_MF_ECUDA.
  *   - Behaviour for non-finite PIXELS is unspecified (pixels are not scanned).
@@ -99,7 +100,8 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
  *   out_topk      DEVICE  [n_traj][topk] records, or NULL (or topk == 0) = no lists.
  * Errors: EINVAL (NULL frames/sigma_t/trajectories, T/H/W/n_traj < 1, bad prf_sigma, sigma_t,
  * trajectory or t0 values, both outputs absent, shapes whose shifts do not fit 32-bit pixel
- * arithmetic), ENOMEM, ECUDA.
+ * arithmetic, n_traj > 65535, H * W > 2^31, H > 262140 rows -- the same row limit holds for every call
+ * that takes frames or maps), ENOMEM, ECUDA.
  * Any H, W >= 1 is computed correctly; the TMA kernel needs W % 4 == 0 and 16-byte aligned
  * frames (and y-shift ranges below 63 tile heights of 60 px), other inputs take the generic kernel.
  * The TMA kernel accumulates into a context-owned partial-sum workspace of (1 + ceil(y-shift range /
@@ -167,6 +169,24 @@ int tno_mf_search_host(tno_mf_ctx *ctx,
                        float prf_sigma, float t0,
                        float *out_snr_host,
                        tno_mf_cand *out_topk_host);
+
+/* tno_mf_search_host for the paper's real chain: clipped bright pixels (PAPER.md:L106 -> `valid_host`, as in
+ * tno_mf_search_masked) and the maximum over the filter bank (L112 -> `out_max_host`, `out_argk_host`, as in
+ * tno_mf_search_max), with the same banded overlap of upload, search, finish and download.  The validity
+ * weights travel with the frames, band by band (twice the upload); the two max maps are copied back at the end.
+ *   valid_host     HOST float32 [T][H][W] or NULL (= unmasked).
+ *   out_max_host   HOST float32 [H][W] or NULL.   out_argk_host  HOST int32 [H][W] or NULL (needs out_max_host).
+ *   out_snr_host, out_topk_host as in tno_mf_search_host; at least one of the three outputs must be given.
+ * Results are bit for bit those of tno_mf_search_max on the uploaded stacks.  tno_mf_search_host is this call
+ * with valid_host, out_max_host and out_argk_host NULL.  Errors: as tno_mf_search_max. */
+int tno_mf_search_host_max(tno_mf_ctx *ctx,
+                           const float *frames_host, const float *valid_host, int32_t T, int32_t H, int32_t W,
+                           const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                           const tno_mf_traj *trajectories, int32_t n_traj,
+                           float prf_sigma, float t0,
+                           float *out_max_host, int32_t *out_argk_host,
+                           float *out_snr_host,
+                           tno_mf_cand *out_topk_host);
 
 /* Tabulated separable PRF for filter 3: `table` is HOST float32
  * [n_phase][5], row r = the fractions of the flux that fall into the pixels -2 .. +2 around the rounded
@@ -309,11 +329,25 @@ int tno_mf_scatter_subtract(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H
  * within the batch to out_batch[n_traj] / out_slot[n_traj] (either may be NULL) and returns the
  * number of batches (>= 1), or a negative error.  max_entries: slots per batch (1..16);
  * max_spread: largest allowed difference of integer y-shifts inside a batch at any frame; a value
- * >= 2^30 means no limit and an even split of each x-motion into the fewest batches -- that is how
- * tno_mf_search itself batches (with max_entries = 8 or 10, whichever costs less). */
+ * >= 2^30 means no limit and an even split of each x-motion into the fewest batches.  (The search
+ * itself batches SLOTS, tno_mf_plan_slots; this query is the single-trajectory packing.) */
 int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, float t0,
                 int32_t max_entries, int32_t max_spread,
                 int32_t *out_batch, int32_t *out_slot);
+
+/* Host-only planning query (no device work): how the separable kernel groups `trajectories` into batches of
+ * SLOTS.  A batch shares one x-motion; a slot holds a y-motion (vy, ay) and, if it is in the bank, its mirror
+ * image (-vy, -ay), which the kernel scores together at the cost of one (exact
+ * algebra on the five y-taps).  Two trajectories share a slot only if the filter is symmetric under y -> -y
+ * (`symmetric_filter` != 0: cfg.filter 0 and 1), no frame rounds an exact half-pixel tie, and there is no
+ * pointing jitter in y; otherwise each sits alone.  Writes per trajectory its batch, its slot within the batch
+ * and its member (0: the slot's own orientation, vy > 0 or (vy = 0, ay >= 0) for a pairable motion; 1: the
+ * mirror image) to out_batch / out_slot / out_member [n_traj] (each may be NULL); returns the number of batches
+ * or a negative error.  frame_times / jitter_xy as in tno_mf_search_ex (NULL = none).  max_slots in 1 .. 16
+ * (the search uses 5). */
+int tno_mf_plan_slots(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, float t0,
+                      const float *frame_times, const float *jitter_xy, int32_t max_slots,
+                      int32_t symmetric_filter, int32_t *out_batch, int32_t *out_slot, int32_t *out_member);
 
 /* Counters of the last tno_mf_search on this context (host values, valid after the call
  * returns): number of kernel launches enqueued, and which search kernel was used
@@ -325,11 +359,13 @@ int tno_mf_last_stats(const tno_mf_ctx *ctx, int32_t *out_launches, int32_t *out
  * cfg.record_events != 0 (else EINVAL).  Blocks the host until the kernel has finished. */
 int tno_mf_last_kernel_ms(tno_mf_ctx *ctx, float *out_ms);
 
-/* Work of the last tno_mf_search in FP32 multiply-adds of the formulation it executed
- * (DESIGN.md "roofline"): the shared x-pass (5 per staged pixel and batch, halo rows included) and
- * the per-trajectory y-pass (5 per trajectory x frame x pixel).  The generic kernel reports
- * x = 0, y = 25 per evaluation.  NULL pointers are skipped. */
-int tno_mf_last_work(const tno_mf_ctx *ctx, double *out_fma_xpass, double *out_fma_ypass);
+/* Work of the last tno_mf_search in FP32 operations of the formulation it executed (DESIGN.md
+ * "roofline"): multiply-adds of the shared x-pass (5 per staged pixel and batch, halo rows included),
+ * multiply-adds of the y-pass (5 per SLOT x frame x pixel; a slot is one trajectory or a trajectory and
+ * its mirror image (-vy, -ay)), and the additions of the y-pass (4 per batch x
+ * frame x pixel: the sums and differences of the window rows that all slots of a batch share).  The
+ * generic kernel reports x = 0, y = 25 per evaluation, no additions.  NULL pointers are skipped. */
+int tno_mf_last_work(const tno_mf_ctx *ctx, double *out_fma_xpass, double *out_fma_ypass, double *out_add_ypass);
 
 /* Release the context and its workspace.  The caller must have synchronised the stream.
  * NULL is accepted. */

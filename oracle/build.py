@@ -11,8 +11,10 @@ def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB
-    cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-std=c11",
-           "-shared", "-fPIC", "-o", LIB + ".tmp", SRC, "-lm"]
+    # TNO_ORACLE_FLAGS="-fsanitize=address,undefined -g": instrumented build (profiles/r2_sanitizers.md)
+    extra = os.environ.get("TNO_ORACLE_FLAGS", "").split()
+    cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-std=c11"] + extra + \
+          ["-shared", "-fPIC", "-o", LIB + ".tmp", SRC, "-lm"]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB

@@ -58,6 +58,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_search_max.restype = i32
     lib.tno_mf_search_max.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp, vp, vp]
     lib.tno_mf_search_host.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp]
+    lib.tno_mf_search_host_max.restype = i32
+    lib.tno_mf_search_host_max.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i32, f32, f32, vp, vp, vp, vp]
     lib.tno_mf_background.restype = ctypes.c_int
     lib.tno_mf_background.argtypes = [vp, vp, i32, i32, i32, vp, f32, i32, vp, vp]
     lib.tno_mf_flux.restype = ctypes.c_int
@@ -82,12 +84,15 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_set_prf_table.argtypes = [vp, vp, i32]
     lib.tno_mf_plan.restype = ctypes.c_int
     lib.tno_mf_plan.argtypes = [vp, i32, i32, f32, i32, i32, vp, vp]
+    lib.tno_mf_plan_slots.restype = ctypes.c_int
+    lib.tno_mf_plan_slots.argtypes = [vp, i32, i32, f32, vp, vp, i32, i32, vp, vp, vp]
     lib.tno_mf_last_stats.restype = ctypes.c_int
     lib.tno_mf_last_stats.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32)]
     lib.tno_mf_last_kernel_ms.restype = ctypes.c_int
     lib.tno_mf_last_kernel_ms.argtypes = [vp, ctypes.POINTER(f32)]
     lib.tno_mf_last_work.restype = ctypes.c_int
-    lib.tno_mf_last_work.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    lib.tno_mf_last_work.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                     ctypes.POINTER(ctypes.c_double)]
     lib.tno_mf_destroy.restype = ctypes.c_int
     lib.tno_mf_destroy.argtypes = [vp]
     lib.tno_mf_last_error.restype = ctypes.c_char_p
@@ -98,6 +103,7 @@ def _load() -> ctypes.CDLL:
 
 
 _lib = _load()
+_CTX_TOPK = {}          # context handle -> its topk (create-time config), for the size checks of out_topk buffers
 
 
 def _check(rc: int, ctx) -> None:
@@ -124,10 +130,12 @@ def tno_mf_create(device: int = 0, stream: Optional[int] = None, topk: int = 0,
                         filter=int(filter) if filter else int(bool(shift_stack)))
     ctx = ctypes.c_void_p()
     _check(_lib.tno_mf_create(ctypes.byref(cfg), ctypes.byref(ctx)), None)
+    _CTX_TOPK[ctx.value] = int(topk)            # the binding checks the size of out_topk buffers against it
     return ctx
 
 
 def tno_mf_destroy(ctx) -> None:
+    _CTX_TOPK.pop(ctx.value, None)
     _check(_lib.tno_mf_destroy(ctx), None)
 
 
@@ -195,6 +203,8 @@ def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories,
     p_top = None
     if out_topk is not None:
         assert out_topk.is_cuda and out_topk.is_contiguous()
+        assert out_topk.numel() * out_topk.element_size() >= n * _CTX_TOPK.get(ctx.value, 0) * 16, \
+            "out_topk is smaller than [n][topk] records of 16 bytes"
         p_top = out_topk.data_ptr()
     if _valid is not None:
         assert _valid.is_cuda and _valid.is_contiguous() and _valid.shape == frames.shape
@@ -221,26 +231,63 @@ def tno_mf_search_ex(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories,
     _check(rc, ctx)
 
 
-def tno_mf_search_host(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
-                       out_snr=None, out_topk=None) -> None:
-    """frames: HOST float32 tensor or ndarray [T, H, W] (contiguous; pinned for overlap); out_snr: HOST float32
-    [n, H, W] or None; out_topk: HOST buffer of n*topk*16 bytes or None.  Returns when the results are in."""
-    def _ptr(a):
-        return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+def _host_ptr(a, shape, dtype_size, what):
+    """Address of a HOST buffer (torch CPU tensor or ndarray) after checking contiguity, placement and size."""
+    if a is None:
+        return None
+    if hasattr(a, "data_ptr"):
+        assert not a.is_cuda, what + " must be in host memory"
+        assert a.is_contiguous(), what + " must be contiguous"
+        nbytes, ptr = a.numel() * a.element_size(), a.data_ptr()
+    else:
+        assert a.flags.c_contiguous, what + " must be contiguous"
+        nbytes, ptr = a.nbytes, a.ctypes.data
+    need = int(np.prod(shape)) * dtype_size
+    assert nbytes >= need, "%s holds %d bytes, %d needed" % (what, nbytes, need)
+    return ptr
+
+
+def tno_mf_search_host_max(ctx, frames, valid, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float,
+                           t0: float, out_max=None, out_argk=None, out_snr=None, out_topk=None) -> None:
+    """frames (and valid or None): HOST float32 tensors or ndarrays [T, H, W] (contiguous; pinned for overlap);
+    out_max float32 / out_argk int32: HOST [H, W] or None; out_snr: HOST float32 [n, H, W] or None; out_topk: HOST
+    buffer of n*topk*16 bytes or None.  Returns when the results are in the host buffers."""
     T, H, W = frames.shape
-    assert (frames.is_contiguous() if hasattr(frames, "is_contiguous") else frames.flags.c_contiguous)
-    assert (not hasattr(frames, "is_cuda")) or (not frames.is_cuda)
     sig = np.ascontiguousarray(sigma_t, dtype=np.float32)
     tm = None if frame_times is None else np.ascontiguousarray(frame_times, dtype=np.float32)
     jt = None if jitter_xy is None else np.ascontiguousarray(jitter_xy, dtype=np.float32)
     assert sig.shape == (T,) and (tm is None or tm.shape == (T,)) and (jt is None or jt.shape == (T, 2))
     tr = _traj_array(trajectories)
-    _check(_lib.tno_mf_search_host(ctx, _ptr(frames), T, H, W, sig.ctypes.data,
+    n = tr.shape[0]
+    assert valid is None or tuple(valid.shape) == (T, H, W)
+    for a in (frames, valid, out_max, out_snr):
+        assert a is None or (a.element_size() if hasattr(a, "element_size") else a.itemsize) == 4
+    _check(_lib.tno_mf_search_host_max(
+        ctx, _host_ptr(frames, (T, H, W), 4, "frames"), _host_ptr(valid, (T, H, W), 4, "valid"), T, H, W,
+        sig.ctypes.data, tm.ctypes.data if tm is not None else None, jt.ctypes.data if jt is not None else None,
+        tr.ctypes.data, n, float(prf_sigma), float(t0),
+        _host_ptr(out_max, (H, W), 4, "out_max"), _host_ptr(out_argk, (H, W), 4, "out_argk"),
+        _host_ptr(out_snr, (n, H, W), 4, "out_snr"),
+        _host_ptr(out_topk, (n, _CTX_TOPK.get(ctx.value, 0)), 16, "out_topk")), ctx)
+
+
+def tno_mf_search_host(ctx, frames, sigma_t, frame_times, jitter_xy, trajectories, prf_sigma: float, t0: float,
+                       out_snr=None, out_topk=None) -> None:
+    """frames: HOST float32 tensor or ndarray [T, H, W] (contiguous; pinned for overlap); out_snr: HOST float32
+    [n, H, W] or None; out_topk: HOST buffer of n*topk*16 bytes or None.  Returns when the results are in."""
+    T, H, W = frames.shape
+    sig = np.ascontiguousarray(sigma_t, dtype=np.float32)
+    tm = None if frame_times is None else np.ascontiguousarray(frame_times, dtype=np.float32)
+    jt = None if jitter_xy is None else np.ascontiguousarray(jitter_xy, dtype=np.float32)
+    assert sig.shape == (T,) and (tm is None or tm.shape == (T,)) and (jt is None or jt.shape == (T, 2))
+    tr = _traj_array(trajectories)
+    n = tr.shape[0]
+    assert (frames.element_size() if hasattr(frames, "element_size") else frames.itemsize) == 4
+    _check(_lib.tno_mf_search_host(ctx, _host_ptr(frames, (T, H, W), 4, "frames"), T, H, W, sig.ctypes.data,
                                    tm.ctypes.data if tm is not None else None,
-                                   jt.ctypes.data if jt is not None else None, tr.ctypes.data, tr.shape[0],
-                                   float(prf_sigma), float(t0),
-                                   _ptr(out_snr) if out_snr is not None else None,
-                                   _ptr(out_topk) if out_topk is not None else None), ctx)
+                                   jt.ctypes.data if jt is not None else None, tr.ctypes.data, n,
+                                   float(prf_sigma), float(t0), _host_ptr(out_snr, (n, H, W), 4, "out_snr"),
+                                   _host_ptr(out_topk, (n, _CTX_TOPK.get(ctx.value, 0)), 16, "out_topk")), ctx)
 
 
 def tno_mf_background(ctx, frames, jitter_xy, delta: float, n_iter: int, out_coef=None, out_resid=None) -> None:
@@ -280,6 +327,8 @@ def tno_mf_best(ctx, snr, box: int, out_max, out_argk=None, out_z=None, out_topk
     p_top = None
     if out_topk is not None:
         assert out_topk.is_cuda and out_topk.is_contiguous()
+        assert out_topk.numel() * out_topk.element_size() >= 1 * _CTX_TOPK.get(ctx.value, 0) * 16, \
+            "out_topk is smaller than [n][topk] records of 16 bytes"
         p_top = out_topk.data_ptr()
     _check(_lib.tno_mf_best(ctx, snr.data_ptr(), n, H, W, int(box), ptrs[0], ptrs[1], ptrs[2], p_top), ctx)
 
@@ -349,7 +398,8 @@ def tno_mf_peaks(ctx, score, argk, radius: int, out_peaks, out_topk) -> None:
     H, W = score.shape
     for t in (argk, out_peaks):
         assert t is None or (t.is_cuda and t.is_contiguous() and tuple(t.shape) == (H, W) and t.element_size() == 4)
-    assert out_topk is None or (out_topk.is_cuda and out_topk.is_contiguous())
+    assert out_topk is None or (out_topk.is_cuda and out_topk.is_contiguous() and
+                                out_topk.numel() * out_topk.element_size() >= _CTX_TOPK.get(ctx.value, 0) * 16)
     _check(_lib.tno_mf_peaks(ctx, score.data_ptr(), argk.data_ptr() if argk is not None else None, H, W, int(radius),
                              out_peaks.data_ptr() if out_peaks is not None else None,
                              out_topk.data_ptr() if out_topk is not None else None), ctx)
@@ -380,6 +430,23 @@ def tno_mf_plan(trajectories, T: int, t0: float, max_entries: int, max_spread: i
     return rc, ob, os_
 
 
+def tno_mf_plan_slots(trajectories, T: int, t0: float, max_slots: int = 5, symmetric_filter: bool = True,
+                      frame_times=None, jitter_xy=None) -> Tuple[int, np.ndarray, np.ndarray, np.ndarray]:
+    """(number of batches, batch [n], slot [n], member [n]) of the separable kernel's slot packing (host only)."""
+    tr = _traj_array(trajectories)
+    n = tr.shape[0]
+    tm = None if frame_times is None else np.ascontiguousarray(frame_times, dtype=np.float32)
+    jt = None if jitter_xy is None else np.ascontiguousarray(jitter_xy, dtype=np.float32)
+    assert (tm is None or tm.shape == (T,)) and (jt is None or jt.shape == (T, 2))
+    batch, slot, member = (np.full(n, -1, dtype=np.int32) for _ in range(3))
+    rc = _lib.tno_mf_plan_slots(tr.ctypes.data, n, int(T), float(t0), tm.ctypes.data if tm is not None else None,
+                                jt.ctypes.data if jt is not None else None, int(max_slots),
+                                int(bool(symmetric_filter)), batch.ctypes.data, slot.ctypes.data, member.ctypes.data)
+    if rc < 0:
+        raise TnoMfError(rc, "tno_mf_plan_slots: invalid arguments")
+    return rc, batch, slot, member
+
+
 def tno_mf_last_stats(ctx) -> Tuple[int, int]:
     """(kernel launches of the last search, 1 if the separable TMA kernel was used else 0)."""
     a, b = ctypes.c_int32(), ctypes.c_int32()
@@ -394,11 +461,11 @@ def tno_mf_last_kernel_ms(ctx) -> float:
     return ms.value
 
 
-def tno_mf_last_work(ctx) -> Tuple[float, float]:
-    """(x-pass, y-pass) FP32 multiply-adds of the formulation the last search executed."""
-    a, b = ctypes.c_double(), ctypes.c_double()
-    _check(_lib.tno_mf_last_work(ctx, ctypes.byref(a), ctypes.byref(b)), None)
-    return a.value, b.value
+def tno_mf_last_work(ctx) -> Tuple[float, float, float]:
+    """(x-pass multiply-adds, y-pass multiply-adds, y-pass additions) of the formulation the last search executed."""
+    a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(_lib.tno_mf_last_work(ctx, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), None)
+    return a.value, b.value, c.value
 
 
 def make_sources(trajs, xs, ys, amps) -> np.ndarray:

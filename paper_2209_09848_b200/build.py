@@ -25,6 +25,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _newer(LIB, deps):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    # sanitizer / debug builds: TNO_MF_HOST_FLAGS="-fsanitize=address -fsanitize=undefined" (no commas inside a flag: -Xcompiler splits on them) instruments the host code
+    # (planner, ABI), TNO_MF_NVCC_FLAGS="-DTNO_DEBUG_CHECKS" adds flags for nvcc itself (profiles/r2_sanitizers.md)
+    host_extra = os.environ.get("TNO_MF_HOST_FLAGS", "")
+    nvcc_extra = os.environ.get("TNO_MF_NVCC_FLAGS", "").split()
+    flags = list(NVCC_FLAGS) + nvcc_extra
+    if host_extra:
+        flags[flags.index("-fPIC,-O2,-ffp-contract=off")] += "," + ",".join(host_extra.split())
     objs = []
     bdir = os.path.join(HERE, "build")
     os.makedirs(bdir, exist_ok=True)
@@ -35,13 +42,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
         objs.append(obj)
         if not force and not _newer(obj, deps):
             continue
-        cmd = [nvcc] + NVCC_FLAGS + ["-c", src, "-o", obj]
+        cmd = [nvcc] + flags + ["-c", src, "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         logs.append(r.stderr)
         if r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)
             raise RuntimeError("nvcc failed on " + f)
     cmd = [nvcc, "-shared", "-o", LIB + ".tmp"] + objs + ["-lcudart_static", "-lpthread", "-ldl", "-lrt"]
+    if host_extra:
+        cmd += ["-Xcompiler", ",".join(host_extra.split())]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     with open(os.path.join(bdir, "ptxas.log"), "a") as fh:

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -31,21 +32,22 @@ struct tno_mf_ctx {
     void *encode_fn = nullptr;
     std::string err;
     int32_t last_launches = 0, last_kernel = 0;
+    int32_t sep_variant = 0;          // kernel shape of the separable search (search_sep.cu)
     // host-fed search (tno_mf_search_host): rows [0, fed_rows) of every frame are on the device
-    const float *feed_host = nullptr;
-    float *feed_dev = nullptr;
+    const float *feed_host = nullptr, *feed_host2 = nullptr;      // feed_host2: the validity weights of a masked search
+    float *feed_dev = nullptr, *feed_dev2 = nullptr;
     int32_t fed_rows = 0, feed_T = 0, feed_H = 0, feed_W = 0;
     cudaStream_t copy_stream = nullptr, down_stream = nullptr;
     cudaEvent_t copy_ev = nullptr, start_ev = nullptr, fin_ev = nullptr;
     float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
     const float *down_dev = nullptr;
     int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
-    DevBuf stack, hmaps, htopk, bgq, prf_tab, maxkeys, scat;
+    DevBuf stack, stack2, hmaps, htopk, hmax, bgq, prf_tab, maxkeys, scat;
     int32_t prf_phases = 0;          // rows of prf_tab (tno_mf_set_prf_table), 0 = none
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
     const TrajInfo *s_ti = nullptr;
-    double last_fma_x = 0.0, last_fma_y = 0.0;
+    double last_fma_x = 0.0, last_fma_y = 0.0, last_add_y = 0.0;
     std::vector<cudaEvent_t> ev;      // pairs (before, after) around each main search kernel launch
     int32_t ev_used = 0;              // events recorded by the last search
     // grow-only device workspace
@@ -153,6 +155,10 @@ int feed_rows(tno_mf_ctx *ctx, int32_t r_end) {
     CU_TRY(ctx, cudaMemcpy2DAsync(ctx->feed_dev + off, pitch, ctx->feed_host + off, pitch,
                                   (size_t)(r_end - ctx->fed_rows) * ctx->feed_W * 4, (size_t)ctx->feed_T,
                                   cudaMemcpyHostToDevice, ctx->copy_stream));
+    if (ctx->feed_host2)
+        CU_TRY(ctx, cudaMemcpy2DAsync(ctx->feed_dev2 + off, pitch, ctx->feed_host2 + off, pitch,
+                                      (size_t)(r_end - ctx->fed_rows) * ctx->feed_W * 4, (size_t)ctx->feed_T,
+                                      cudaMemcpyHostToDevice, ctx->copy_stream));
     CU_TRY(ctx, cudaEventRecord(ctx->copy_ev, ctx->copy_stream));
     CU_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->copy_ev, 0));
     ctx->fed_rows = r_end;
@@ -215,6 +221,7 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
     ctx->cfg = *cfg;
     ctx->stream = reinterpret_cast<cudaStream_t>(cfg->stream);
     ctx->n_sm = prop.multiProcessorCount;
+    if (const char *ev = getenv("TNO_MF_SEP_VARIANT")) ctx->sep_variant = atoi(ev) ? 1 : 0;   // EXPERIMENT ONLY
     cudaDriverEntryPointQueryResult qres;
     e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_fn, cudaEnableDefault, &qres);
     if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !ctx->encode_fn) {
@@ -241,10 +248,11 @@ int tno_mf_last_kernel_ms(tno_mf_ctx *ctx, float *out_ms) {
     return TNO_MF_OK;
 }
 
-int tno_mf_last_work(const tno_mf_ctx *ctx, double *out_fma_xpass, double *out_fma_ypass) {
+int tno_mf_last_work(const tno_mf_ctx *ctx, double *out_fma_xpass, double *out_fma_ypass, double *out_add_ypass) {
     if (!ctx) return TNO_MF_EINVAL;
     if (out_fma_xpass) *out_fma_xpass = ctx->last_fma_x;
     if (out_fma_ypass) *out_fma_ypass = ctx->last_fma_y;
+    if (out_add_ypass) *out_add_ypass = ctx->last_add_y;
     return TNO_MF_OK;
 }
 
@@ -253,7 +261,8 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     cudaSetDevice(ctx->cfg.device);
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
                       &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
-                      &ctx->stack, &ctx->hmaps, &ctx->htopk, &ctx->bgq, &ctx->prf_tab, &ctx->maxkeys, &ctx->scat};
+                      &ctx->stack, &ctx->stack2, &ctx->hmaps, &ctx->htopk, &ctx->hmax, &ctx->bgq, &ctx->prf_tab,
+                      &ctx->maxkeys, &ctx->scat};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -292,6 +301,35 @@ int tno_mf_plan(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, floa
             if (out_slot) out_slot[plan.batches[b].traj[s]] = (int32_t)s;
         }
     return (int)plan.batches.size();
+}
+
+int tno_mf_plan_slots(const tno_mf_traj *trajectories, int32_t n_traj, int32_t T, float t0, const float *frame_times,
+                      const float *jitter_xy, int32_t max_slots, int32_t symmetric_filter, int32_t *out_batch,
+                      int32_t *out_slot, int32_t *out_member) {
+    if (!trajectories || n_traj < 1 || T < 1 || max_slots < 1 || max_slots > 16 || !finite_f(t0))
+        return TNO_MF_EINVAL;
+    for (int32_t k = 0; k < n_traj; ++k)
+        if (!finite_f(trajectories[k].vx) || !finite_f(trajectories[k].vy) ||
+            !finite_f(trajectories[k].ax) || !finite_f(trajectories[k].ay))
+            return TNO_MF_EINVAL;
+    for (int32_t t = 0; t < T; ++t)
+        if ((frame_times && !finite_f(frame_times[t])) ||
+            (jitter_xy && (!finite_f(jitter_xy[2 * t]) || !finite_f(jitter_xy[2 * t + 1]))))
+            return TNO_MF_EINVAL;
+    Plan plan;
+    const int rc = build_classes(trajectories, n_traj, T, (double)t0, frame_times, jitter_xy, &plan);
+    if (rc != TNO_MF_OK) return rc;
+    build_slot_batches(&plan, max_slots, symmetric_filter != 0);
+    for (size_t b = 0; b < plan.slot_batches.size(); ++b)
+        for (size_t s = 0; s < plan.slot_batches[b].slots.size(); ++s)
+            for (int m = 0; m < 2; ++m) {
+                const int32_t k = plan.slot_batches[b].slots[s].member[m];
+                if (k < 0) continue;
+                if (out_batch) out_batch[k] = (int32_t)b;
+                if (out_slot) out_slot[k] = (int32_t)s;
+                if (out_member) out_member[k] = m;
+            }
+    return (int)plan.slot_batches.size();
 }
 
 // ---- low-resolution scattered-light model (section 3.1) -------------------------------------------------
@@ -387,8 +425,9 @@ int tno_mf_downsample(tno_mf_ctx *ctx, const float *frames, int32_t T, int32_t H
                       float *out) {
     if (!ctx) return TNO_MF_EINVAL;
     if (!frames || !out) return fail(ctx, TNO_MF_EINVAL, "tno_mf_downsample: NULL pointer");
-    if (T < 1 || T > 65535 || H < 1 || W < 1 || factor < 1 || H % factor || W % factor)
-        return fail(ctx, TNO_MF_EINVAL, "tno_mf_downsample: need 1 <= T <= 65535 and factor dividing H and W");
+    if (T < 1 || T > 65535 || H < 1 || W < 1 || factor < 1 || H % factor || W % factor || H / factor > kMaxRows)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_downsample: need 1 <= T <= 65535, factor dividing H and W, and "
+                    "H / factor <= %d", kMaxRows);
     CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
     launch_downsample(ctx->stream, frames, T, H, W, factor, out);
     ctx->last_launches = 1;
@@ -400,8 +439,9 @@ int tno_mf_scatter_subtract(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H
                             int32_t n) {
     if (!ctx) return TNO_MF_EINVAL;
     if (!frames || !S) return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_subtract: NULL pointer");
-    if (T < 1 || T > 65535 || H < 1 || W < 1 || n < 1 || n > H || n > W)
-        return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_subtract: need 1 <= T <= 65535 and 1 <= n <= min(H, W)");
+    if (T < 1 || T > 65535 || H < 1 || H > kMaxRows || W < 1 || n < 1 || n > H || n > W)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_subtract: need 1 <= T <= 65535, H <= %d and 1 <= n <= min(H, W)",
+                    kMaxRows);
     CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
     std::vector<int32_t> tabs(2 * ((size_t)H + W));          // y: first pixel [H], weight [H]; x: the same [W]
     bilinear_table(H, n, tabs.data(), reinterpret_cast<float *>(tabs.data() + H));
@@ -473,8 +513,8 @@ int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
     if (!snr || !out_max) return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: NULL snr or out_max");
-    if (n_traj < 1 || H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 31)
-        return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: n_traj, H, W must be >= 1 and H*W <= 2^31");
+    if (n_traj < 1 || H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 31 || H > kMaxRows)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: n_traj, H, W must be >= 1, H*W <= 2^31 and H <= %d", kMaxRows);
     if (box < 1 || (box & 1) == 0) return fail(ctx, TNO_MF_EINVAL, "tno_mf_best: box must be odd and >= 1");
     CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t st = ctx->stream;
@@ -523,8 +563,8 @@ int tno_mf_peaks(tno_mf_ctx *ctx, const float *score, const int32_t *argk, int32
     if (!ctx) return TNO_MF_EINVAL;
     ctx->last_launches = 0;
     if (!score) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: NULL score map");
-    if (H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 31)
-        return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: H, W must be >= 1 and H*W <= 2^31");
+    if (H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 31 || H > kMaxRows)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: H, W must be >= 1, H*W <= 2^31 and H <= %d", kMaxRows);
     if (radius < 0 || radius > 1024) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: radius must be in [0, 1024]");
     const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
     if (!out_peaks && !want_topk) return fail(ctx, TNO_MF_EINVAL, "tno_mf_peaks: no output requested");
@@ -679,8 +719,8 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
     if (T < 1 || H < 1 || W < 1 || n_traj < 1)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: T, H, W and n_traj must be >= 1");
     if (n_traj > 65535) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: at most 65535 trajectories per call");
-    if ((int64_t)H * W > (int64_t)1 << 31)
-        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: H*W must not exceed 2^31 pixels");
+    if ((int64_t)H * W > (int64_t)1 << 31 || H > kMaxRows)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: H*W must not exceed 2^31 pixels and H %d rows", kMaxRows);
     if (!(prf_sigma > 0.f) || !finite_f(prf_sigma))
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: prf_sigma must be finite and > 0");
     if (ctx->cfg.filter == 3 && ctx->prf_phases == 0)
@@ -723,21 +763,11 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
     const int32_t n_pass = valid ? 2 : 1;             // masked search: a second pass accumulates D
     SepVariant sv = {0, 0};
     if (use_sep) {
-        // variant = batch capacity; cost = x-pass per batch + y-pass per entry (FFMA per pixel), ties
-        // go to the smaller capacity (fewer partially filled batches)
-        double best = 0.0;
-        Plan trial = plan;
-        for (int32_t v = 0; v < sep_num_variants(); ++v) {
-            build_batches(&trial, sep_variant(v).nb, kUnlimitedSpread);
-            double cost = 0.0;
-            for (const Batch &bt : trial.batches) cost += 5.3 + 5.0 * (double)bt.traj.size();
-            if (variant < 0 || cost < best) {
-                best = cost;
-                variant = v;
-                plan.batches = trial.batches;
-            }
-        }
+        // slots (mirror pairs where the filter is symmetric under y -> -y: the Gaussian and the single tap)
+        // packed into batches; both kernel variants take the same batches
+        variant = ctx->sep_variant;
         sv = sep_variant(variant);
+        build_slot_batches(&plan, sv.nb, ctx->cfg.filter == 0 || ctx->cfg.filter == 1);
         int64_t range = 0;
         for (const AxisClass &c : plan.ycls) range = std::max<int64_t>(range, (int64_t)c.smax - c.smin);
         const int64_t np = 1 + (range + sv.tile_h - 1) / sv.tile_h;
@@ -780,26 +810,33 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         rsd_total += cells;
         max_cells = std::max(max_cells, cells);
     }
-    // planned order q: batches in order, entries in order (slots 0 .. n-1 of the batch)
+    // planned order q: batches in order, slots in order, plus member before minus member
     int32_t n_batches = 0;
-    std::vector<int32_t> batch_xc, batch_yc, batch_q, perm, batch_q0;
+    std::vector<int32_t> batch_xc, slot_yc, slot_flip, slot_q, perm, batch_q0;
+    double slot_px = 0.0;                // slots summed over batches (work accounting)
     if (use_sep) {
-        n_batches = (int32_t)plan.batches.size();
+        n_batches = (int32_t)plan.slot_batches.size();
         batch_xc.resize(n_batches);
-        batch_yc.assign((size_t)n_batches * sv.nb, -1);
-        batch_q.assign((size_t)n_batches * sv.nb, -1);
+        slot_yc.assign((size_t)n_batches * sv.nb, -1);
+        slot_flip.assign((size_t)n_batches * sv.nb, 0);
+        slot_q.assign((size_t)n_batches * sv.nb * 2, -1);
         batch_q0.resize(n_batches + 1);
         perm.reserve(n_traj);
         for (int32_t b = 0; b < n_batches; ++b) {
-            const Batch &bt = plan.batches[b];
+            const SlotBatch &bt = plan.slot_batches[b];
             batch_xc[b] = bt.xcls;
             batch_q0[b] = (int32_t)perm.size();
-            for (size_t j = 0; j < bt.traj.size(); ++j) {
-                const size_t slot = j;
-                batch_q[(size_t)b * sv.nb + slot] = (int32_t)perm.size();
-                batch_yc[(size_t)b * sv.nb + slot] = plan.traj_yc[bt.traj[j]];
-                perm.push_back(bt.traj[j]);
+            for (size_t j = 0; j < bt.slots.size(); ++j) {
+                const size_t slot = (size_t)b * sv.nb + j;
+                slot_yc[slot] = bt.slots[j].ycls;
+                slot_flip[slot] = bt.slots[j].flip;
+                for (int m = 0; m < 2; ++m)
+                    if (bt.slots[j].member[m] >= 0) {
+                        slot_q[slot * 2 + m] = (int32_t)perm.size() - batch_q0[b];
+                        perm.push_back(bt.slots[j].member[m]);
+                    }
             }
+            slot_px += (double)bt.slots.size();
         }
         batch_q0[n_batches] = (int32_t)perm.size();
     }
@@ -812,10 +849,12 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
     const size_t o_off = blob.add(ab_off.data(), ab_off.size() * 8);
     const size_t o_ti = blob.add(tinfo.data(), tinfo.size() * sizeof(TrajInfo));
     const size_t o_bx = blob.add(batch_xc.data(), batch_xc.size() * 4);
-    const size_t o_by = blob.add(batch_yc.data(), batch_yc.size() * 4);
+    const size_t o_by = blob.add(slot_yc.data(), slot_yc.size() * 4);
+    const size_t o_fl = blob.add(slot_flip.data(), slot_flip.size() * 4);
+    const size_t o_sq = blob.add(slot_q.data(), slot_q.size() * 4);
     const size_t o_tm = blob.add(frame_times, frame_times ? (size_t)T * 4 : 0);
     const size_t o_jt = blob.add(jitter_xy, jitter_xy ? (size_t)T * 8 : 0);
-    const size_t o_bq = blob.add(batch_q.data(), batch_q.size() * 4);
+    const size_t o_bq = blob.add(batch_q0.data(), batch_q0.size() * 4);
     const size_t o_perm = blob.add(perm.data(), perm.size() * 4);
 
     // ------------------------------------------------------------------ workspace
@@ -851,7 +890,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
             const size_t avail = (size_t)((double)(free_b + ctx->pieces.cap) * 0.8);
             const size_t budget = std::min<size_t>(want, std::min<size_t>(avail, limit));
             // a chunk holds at least one batch
-            const size_t need = std::max<size_t>(budget, per_entry * (size_t)std::min<int64_t>(sv.nb, n_traj));
+            const size_t need = std::max<size_t>(budget, per_entry * (size_t)std::min<int64_t>(2 * sv.nb, n_traj));
             if (need > avail)
                 return fail(ctx, TNO_MF_ENOMEM, "not enough device memory for the partial-sum buffer "
                             "(%zu bytes per trajectory, %zu available)", per_entry, avail);
@@ -909,7 +948,9 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         const size_t tab_floats = (size_t)n_batches * T * sep_table_words(variant);
         for (int32_t pass = 0; pass < n_pass; ++pass) {
             launch_sep_tables(st, variant, tab, reinterpret_cast<const int32_t *>(meta + o_bx),
-                              reinterpret_cast<const int32_t *>(meta + o_by), n_batches, pass,
+                              reinterpret_cast<const int32_t *>(meta + o_by),
+                              reinterpret_cast<const int32_t *>(meta + o_fl),
+                              reinterpret_cast<const int32_t *>(meta + o_sq), n_batches, pass,
                               static_cast<float *>(ctx->stage_tab.p) + pass * tab_floats);
             ctx->last_launches += 1;
         }
@@ -922,7 +963,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
             SepArgs a;
             a.frames = frames; a.T = T; a.H = H; a.W = W;
             a.stage_tab = static_cast<const float *>(ctx->stage_tab.p) + (size_t)b0 * T * tabw;
-            a.batch_q = reinterpret_cast<const int32_t *>(meta + o_bq) + (size_t)b0 * sv.nb;
+            a.batch_q = reinterpret_cast<const int32_t *>(meta + o_bq) + b0;
             a.n_batches = b1 - b0;
             a.q0 = q0;
             a.pieces = static_cast<float *>(ctx->pieces.p);
@@ -933,22 +974,23 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
             CU_TRY(ctx, cudaMemsetAsync(a.pieces, 0, n_pass * pass_floats * 4, st));
             const int32_t nfy = (H + kCollectTile - 1) / kCollectTile;   // rows of 64 x 64 output tiles
             int32_t fin_tiles = 0;                                        // ... already finished (banded)
-            const bool banded_finish = ctx->feed_host && ctx->fed_rows < H && n_pass == 1 && qn == n_traj;
+            const bool banded_finish = ctx->feed_host && ctx->fed_rows < H && qn == n_traj;
             int64_t y_smax = INT32_MIN;                                   // largest y-shift of the bank
             for (const AxisClass &c : plan.ycls) y_smax = std::max<int64_t>(y_smax, c.smax);
-            for (int32_t pass = 0; pass < n_pass; ++pass) {
-                // pass 1 of a masked search: the same kernel over the validity weights with squared taps
-                a.frames = pass ? valid : frames;
-                a.stage_tab = static_cast<const float *>(ctx->stage_tab.p) + pass * tab_floats + (size_t)b0 * T * tabw;
-                a.pieces = static_cast<float *>(ctx->pieces.p) + pass * pass_floats;
-                // a host-fed stack arrives in bands of tile rows: the search of a band starts as soon as
-                // its frame rows are on the device and overlaps the upload of the next bands
-                const int32_t nty = sep_tile_rows(variant, H);
-                const int32_t band = (ctx->feed_host && ctx->fed_rows < H) ? 4 : nty;
-                for (int32_t ty0 = 0; ty0 < nty; ty0 += band) {
-                    a.ty0 = ty0;
-                    a.ty1 = std::min(nty, ty0 + band);
-                    if ((rc = feed_rows(ctx, a.ty1 == nty ? H : a.ty1 * sv.tile_h))) return rc;
+            const float *np_ = static_cast<const float *>(ctx->pieces.p);
+            // a host-fed stack arrives in bands of tile rows: the search of a band starts as soon as
+            // its frame rows are on the device and overlaps the upload of the next bands
+            const int32_t nty = sep_tile_rows(variant, H);
+            const int32_t band = (ctx->feed_host && ctx->fed_rows < H) ? 4 : nty;
+            for (int32_t ty0 = 0; ty0 < nty; ty0 += band) {
+                a.ty0 = ty0;
+                a.ty1 = std::min(nty, ty0 + band);
+                if ((rc = feed_rows(ctx, a.ty1 == nty ? H : a.ty1 * sv.tile_h))) return rc;
+                for (int32_t pass = 0; pass < n_pass; ++pass) {
+                    // pass 1 of a masked search: the same kernel over the validity weights with squared taps
+                    a.frames = pass ? valid : frames;
+                    a.stage_tab = static_cast<const float *>(ctx->stage_tab.p) + pass * tab_floats + (size_t)b0 * T * tabw;
+                    a.pieces = static_cast<float *>(ctx->pieces.p) + pass * pass_floats;
                     int32_t grid = 0;
                     const char *err = "";
                     if ((rc = record_event(ctx))) return rc;
@@ -956,23 +998,23 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
                         return fail(ctx, TNO_MF_ECUDA, "separable search kernel: %s", err);
                     if ((rc = record_event(ctx))) return rc;
                     ctx->last_launches += (ty0 > 0);
-                    // host-fed, one chunk, one pass: the output rows that no later tile row can touch are
-                    // finished and sent to the host while the next bands are still being uploaded
-                    if (banded_finish && a.ty1 < nty) {
-                        const int32_t fy1 = std::min<int64_t>(nfy, std::max<int64_t>(
-                            fin_tiles, ((int64_t)a.ty1 * sv.tile_h - y_smax - 2) / kCollectTile));
-                        if (fy1 > fin_tiles) {
-                            launch_finish(st, static_cast<const float *>(ctx->pieces.p), nullptr, n_pieces, a.piece_stride,
-                                          reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W,
-                                          fin_tiles, fy1, out_snr, mk, slots);
-                            ctx->last_launches += 1;
-                            fin_tiles = fy1;
-                            if ((rc = download_rows(ctx, fy1 * kCollectTile))) return rc;
-                        }
+                }
+                // host-fed, one chunk: the output rows that no later tile row can touch are finished and
+                // sent to the host while the next bands are still being uploaded
+                if (banded_finish && a.ty1 < nty) {
+                    const int32_t fy1 = (int32_t)std::min<int64_t>(nfy, std::max<int64_t>(
+                        fin_tiles, ((int64_t)a.ty1 * sv.tile_h - y_smax - 2) / kCollectTile));
+                    if (fy1 > fin_tiles) {
+                        launch_finish(st, np_, valid ? np_ + pass_floats : nullptr, n_pieces, a.piece_stride,
+                                      reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W,
+                                      fin_tiles, fy1, out_snr, mk, slots);
+                        ctx->last_launches += 1;
+                        fin_tiles = fy1;
+                        if ((rc = download_rows(ctx, fy1 * kCollectTile))) return rc;
                     }
                 }
             }
-            const float *np_ = static_cast<const float *>(ctx->pieces.p);
+            // (all rows may be finished already: a bank whose y-shifts are all negative; launch_finish skips an empty range)
             launch_finish(st, np_, valid ? np_ + pass_floats : nullptr, n_pieces, a.piece_stride,
                           reinterpret_cast<const int32_t *>(meta + o_perm), q0, qn, d_ti, d_rsd, H, W, fin_tiles, nfy,
                           out_snr, mk, slots);
@@ -985,8 +1027,12 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         double rows = 0.0;
         for (int32_t ty = 0; ty < sep_tile_rows(variant, H); ++ty)
             rows += (double)(std::min(sv.tile_h, H + 2 - (ty * sv.tile_h - 2)) + 4);
-        ctx->last_fma_x = n_pass * 5.0 * rows * 64.0 * (double)((W + 63) / 64) * (double)n_batches * T;
-        ctx->last_fma_y = n_pass * 5.0 * (double)n_traj * T * (double)H * W;
+        const double cols = 64.0 * (double)((W + 63) / 64);
+        ctx->last_fma_x = n_pass * 5.0 * rows * cols * (double)n_batches * T;
+        // y-pass: 5 multiply-adds per slot (one or two trajectories), position and frame; the sums and
+        // differences of the window rows, 4 additions per position and frame, are shared by the batch
+        ctx->last_fma_y = n_pass * 5.0 * slot_px * T * (double)H * W;
+        ctx->last_add_y = n_pass * 4.0 * (rows - 4.0 * sep_tile_rows(variant, H)) * cols * (double)n_batches * T;
     } else {
         // generic path: maps are always materialised (caller's buffer, or a workspace chunk)
         if ((rc = feed_rows(ctx, H))) return rc;
@@ -999,6 +1045,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
             maps = static_cast<float *>(ctx->tmp_maps.p);
         }
         ctx->last_fma_x = 0.0;
+        ctx->last_add_y = 0.0;
         ctx->last_fma_y = n_pass * 25.0 * (double)n_traj * T * (double)H * W;
         if ((rc = record_event(ctx))) return rc;
         for (int32_t k0 = 0; k0 < n_traj; k0 += chunk) {
@@ -1055,19 +1102,32 @@ int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int
                        const float *sigma_t, const float *frame_times, const float *jitter_xy,
                        const tno_mf_traj *trajectories, int32_t n_traj, float prf_sigma, float t0,
                        float *out_snr_host, tno_mf_cand *out_topk_host) {
+    return tno_mf_search_host_max(ctx, frames_host, nullptr, T, H, W, sigma_t, frame_times, jitter_xy, trajectories,
+                                  n_traj, prf_sigma, t0, nullptr, nullptr, out_snr_host, out_topk_host);
+}
+
+int tno_mf_search_host_max(tno_mf_ctx *ctx, const float *frames_host, const float *valid_host, int32_t T, int32_t H,
+                           int32_t W, const float *sigma_t, const float *frame_times, const float *jitter_xy,
+                           const tno_mf_traj *trajectories, int32_t n_traj, float prf_sigma, float t0,
+                           float *out_max_host, int32_t *out_argk_host, float *out_snr_host,
+                           tno_mf_cand *out_topk_host) {
     if (!ctx) return TNO_MF_EINVAL;
     if (!frames_host) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host: NULL frames");
     if (T < 1 || H < 1 || W < 1 || n_traj < 1)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host: T, H, W and n_traj must be >= 1");
     const bool want_topk = out_topk_host != nullptr && ctx->cfg.topk > 0;
-    if (!out_snr_host && !want_topk)
+    if (!out_snr_host && !want_topk && !out_max_host)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host: no output requested");
+    if (out_argk_host && !out_max_host)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search_host_max: out_argk needs out_max");
     CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
     int rc;
     const size_t px = (size_t)H * W;
     if ((rc = reserve(ctx, ctx->stack, (size_t)T * px * 4))) return rc;
+    if (valid_host && (rc = reserve(ctx, ctx->stack2, (size_t)T * px * 4))) return rc;
     if (out_snr_host && (rc = reserve(ctx, ctx->hmaps, (size_t)n_traj * px * 4))) return rc;
     if (want_topk && (rc = reserve(ctx, ctx->htopk, (size_t)n_traj * ctx->cfg.topk * sizeof(tno_mf_cand)))) return rc;
+    if (out_max_host && (rc = reserve(ctx, ctx->hmax, px * 8))) return rc;
     if (!ctx->copy_stream) {
         CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
         CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->copy_ev, cudaEventDisableTiming));
@@ -1080,6 +1140,8 @@ int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int
     CU_TRY(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->start_ev, 0));
     ctx->feed_host = frames_host;
     ctx->feed_dev = static_cast<float *>(ctx->stack.p);
+    ctx->feed_host2 = valid_host;
+    ctx->feed_dev2 = valid_host ? static_cast<float *>(ctx->stack2.p) : nullptr;
     ctx->fed_rows = 0;
     ctx->feed_T = T; ctx->feed_H = H; ctx->feed_W = W;
     float *d_maps = out_snr_host ? static_cast<float *>(ctx->hmaps.p) : nullptr;
@@ -1088,9 +1150,11 @@ int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int
     ctx->down_rows = 0;
     ctx->down_K = n_traj;
     tno_mf_cand *d_topk = want_topk ? static_cast<tno_mf_cand *>(ctx->htopk.p) : nullptr;
-    rc = tno_mf_search_masked(ctx, ctx->feed_dev, nullptr, T, H, W, sigma_t, frame_times, jitter_xy, trajectories,
-                              n_traj, prf_sigma, t0, d_maps, d_topk);
-    ctx->feed_host = nullptr;
+    float *d_max = out_max_host ? static_cast<float *>(ctx->hmax.p) : nullptr;
+    int32_t *d_argk = out_argk_host ? reinterpret_cast<int32_t *>(d_max + px) : nullptr;
+    rc = search_core(ctx, ctx->feed_dev, ctx->feed_dev2, T, H, W, sigma_t, frame_times, jitter_xy, trajectories,
+                     n_traj, prf_sigma, t0, d_maps, d_topk, d_max, d_argk);
+    ctx->feed_host = ctx->feed_host2 = nullptr;
     if (rc == TNO_MF_OK) rc = download_rows(ctx, H);       // the rows no band could finish early
     ctx->down_host = nullptr;
     if (rc != TNO_MF_OK) {
@@ -1101,6 +1165,8 @@ int tno_mf_search_host(tno_mf_ctx *ctx, const float *frames_host, int32_t T, int
     if (d_topk)
         CU_TRY(ctx, cudaMemcpyAsync(out_topk_host, d_topk, (size_t)n_traj * ctx->cfg.topk * sizeof(tno_mf_cand),
                                     cudaMemcpyDeviceToHost, ctx->stream));
+    if (d_max) CU_TRY(ctx, cudaMemcpyAsync(out_max_host, d_max, px * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    if (d_argk) CU_TRY(ctx, cudaMemcpyAsync(out_argk_host, d_argk, px * 4, cudaMemcpyDeviceToHost, ctx->stream));
     CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
     CU_TRY(ctx, cudaStreamSynchronize(ctx->down_stream));
     return TNO_MF_OK;

@@ -17,7 +17,9 @@ __global__ void __launch_bounds__(256)
 k_max_map(const float *__restrict__ snr, int32_t K, int64_t n_px, float *__restrict__ out_max,
           int32_t *__restrict__ out_argk) {
     const int64_t n4 = n_px / 4;
-    const bool vec = (reinterpret_cast<uintptr_t>(snr) & 15u) == 0 && (n_px % 4) == 0;
+    // (out_argk == NULL has address 0: aligned)
+    const bool vec = ((reinterpret_cast<uintptr_t>(snr) | reinterpret_cast<uintptr_t>(out_max) |
+                       reinterpret_cast<uintptr_t>(out_argk)) & 15u) == 0 && (n_px % 4) == 0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x, id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (vec) {
         for (int64_t i = id; i < n4; i += stride) {

@@ -29,6 +29,7 @@ void launch_search_generic(cudaStream_t st, const float *frames, const float *va
 // ---- topk.cu ----
 constexpr int32_t kCollectTile = 64;        // k_collect_from_map tiles are 64 x 64 pixels
 constexpr int32_t kMaxTopk = 1024;
+constexpr int32_t kMaxRows = 65535 * 4;     // frame rows: several kernels put rows / 4 into gridDim.y (DESIGN d2)
 // candidates of maps [k_count][H][W] (trajectories k_first..) into tile slots
 void launch_collect_from_map(cudaStream_t st, const float *maps, int32_t H, int32_t W,
                              int32_t k_first, int32_t k_count, const TopkSlots &slots);
@@ -87,7 +88,7 @@ void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t
 
 // ---- search_sep.cu ----
 struct SepVariant {
-    int32_t nb;           // entries per batch
+    int32_t nb;           // slots per batch (a slot = a y-motion and its mirror image, plan.h)
     int32_t tile_h;       // positions (frame rows) per tile; the tile width is 64 columns
 };
 int32_t sep_num_variants();
@@ -97,13 +98,17 @@ int32_t sep_table_words(int32_t v);
 // tile rows of the position space [-2, H + 2)
 int32_t sep_tile_rows(int32_t v, int32_t H);
 void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
-                       const int32_t *batch_yc /* [n_batches][nb], -1 = empty */, int32_t n_batches,
-                       int32_t squared /* 1: taps g^2 (D pass of the masked search) */, float *stage_tab);
+                       const int32_t *slot_yc /* [n_batches][nb] y-class of the slot's tables, -1 = empty */,
+                       const int32_t *slot_flip /* [n_batches][nb] 1: that class is the slot's mirror image */,
+                       const int32_t *slot_q /* [n_batches][nb][2] planned index of the plus / minus member
+                                                relative to the batch's first, -1 = absent */,
+                       int32_t n_batches, int32_t squared /* 1: taps g^2 (D pass of the masked search) */,
+                       float *stage_tab);
 struct SepArgs {
     const float *frames;
     int32_t T, H, W;
     const float *stage_tab;       // [n_batches][T][table_words], first batch of the chunk
-    const int32_t *batch_q;       // [n_batches][nb] planned-order index q of each slot, or -1
+    const int32_t *batch_q;       // [n_batches] planned-order index q of the first member of each batch
     int32_t n_batches;            // batches of the chunk
     int32_t q0;                   // first planned-order index of the chunk
     float *pieces;                // [n_pieces][chunk entries][H][W] partial sums, zero on entry

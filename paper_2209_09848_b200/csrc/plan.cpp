@@ -4,13 +4,14 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdint>
 #include <cstring>
 #include <map>
 #include <utility>
 
 namespace tno {
 
-bool axis_shift(double v, double a, double dt, double j, int32_t *shift) {
+bool axis_shift(double v, double a, double dt, double j, int32_t *shift, bool *tie) {
     volatile double p1 = v * dt;          // volatile: keep the operations separately rounded, in the
     volatile double adt = a * dt;         // order the device (tables.cu) and the oracle use
     volatile double p2 = adt * dt;
@@ -18,6 +19,8 @@ bool axis_shift(double v, double a, double dt, double j, int32_t *shift) {
     const double d = d0 + j;
     const double f = std::floor(d + 0.5);
     if (!(std::fabs(f) < 1.0e9)) return false;
+    // d + 1/2 is exact for |d| < 2^51, so this is the exact tie test (floor(-d + 1/2) != -floor(d + 1/2))
+    if (tie) *tie = (d + 0.5 == f);
     *shift = (int32_t)f;
     return true;
 }
@@ -43,7 +46,10 @@ static int class_of(std::map<uint64_t, int32_t> &index, std::vector<AxisClass> &
         int32_t s = 0;
         const double dt = (times ? (double)times[t] : (double)t) - t0;
         const double j = jitter ? (double)jitter[2 * t + axis] : 0.0;
-        if (!axis_shift((double)v, (double)a, dt, j, &s)) { *ok = false; s = 0; }
+        bool tie = false;
+        if (!axis_shift((double)v, (double)a, dt, j, &s, &tie)) { *ok = false; s = 0; }
+        c.tie = c.tie || tie;
+        c.jittered = c.jittered || j != 0.0;
         c.shift[t] = s;
         c.smin = std::min(c.smin, s);
         c.smax = std::max(c.smax, s);
@@ -136,6 +142,61 @@ void build_batches(Plan *plan, int32_t max_entries, int32_t max_spread) {
             cur.traj.push_back(k);
         }
         if (!cur.traj.empty()) plan->batches.push_back(cur);
+    }
+}
+
+void build_slot_batches(Plan *plan, int32_t max_slots, bool symmetric_filter) {
+    plan->slot_batches.clear();
+    const int32_t n_traj = (int32_t)plan->traj_xc.size();
+    std::vector<std::vector<int32_t>> by_x(plan->xcls.size());
+    for (int32_t k = 0; k < n_traj; ++k) by_x[plan->traj_xc[k]].push_back(k);
+    struct Keyed { float v, a; int32_t pairable; Slot slot; };
+    for (size_t xc = 0; xc < by_x.size(); ++xc) {
+        std::vector<Keyed> slots;
+        // orientation key (pairable, v, a) -> the slots that carry it, in order of creation
+        std::map<std::pair<int32_t, uint64_t>, std::vector<size_t>> index;
+        for (int32_t k : by_x[xc]) {
+            const int32_t yc = plan->traj_yc[k];
+            const AxisClass &c = plan->ycls[yc];
+            const bool pairable = symmetric_filter && !c.tie && !c.jittered;
+            float v = c.v + 0.0f, a = c.a + 0.0f;
+            int32_t m = 0;
+            if (pairable && (v < 0.0f || (v == 0.0f && a < 0.0f))) { v = -v; a = -a; m = 1; }
+            std::vector<size_t> &list = index[std::make_pair((int32_t)pairable, key_of(v, a))];
+            size_t found = SIZE_MAX;
+            for (size_t i : list)
+                if (slots[i].slot.member[m] < 0) { found = i; break; }
+            if (found == SIZE_MAX) {
+                Keyed ks;
+                ks.v = v + 0.0f; ks.a = a + 0.0f; ks.pairable = pairable;
+                ks.slot.member[0] = ks.slot.member[1] = -1;
+                ks.slot.ycls = yc;
+                ks.slot.flip = m;
+                found = slots.size();
+                slots.push_back(ks);
+                list.push_back(found);
+            }
+            Slot &sl = slots[found].slot;
+            sl.member[m] = k;
+            // tables from the member in the slot's own orientation when there is one (the other one gives the
+            // same numbers bit for bit: the class tables are odd in (v, a) when there is no tie)
+            if (m == 0) { sl.ycls = yc; sl.flip = 0; }
+        }
+        std::stable_sort(slots.begin(), slots.end(), [](const Keyed &p, const Keyed &q) {
+            if (p.v != q.v) return p.v < q.v;
+            return p.a < q.a;
+        });
+        const int32_t n = (int32_t)slots.size();
+        const int32_t nbt = (n + max_slots - 1) / max_slots;
+        int32_t pos = 0;
+        for (int32_t j = 0; j < nbt; ++j) {
+            const int32_t len = n / nbt + (j < n % nbt ? 1 : 0);
+            SlotBatch sb;
+            sb.xcls = (int32_t)xc;
+            for (int32_t i = 0; i < len; ++i) sb.slots.push_back(slots[pos + i].slot);
+            pos += len;
+            plan->slot_batches.push_back(std::move(sb));
+        }
     }
 }
 

@@ -16,12 +16,14 @@ namespace tno {
 // floor(d + 1/2) of d = (v*dt + (a*dt)*dt) + j, all in IEEE double without contraction
 // (BASELINE.json:north_star "5x5 window at round(c_t)"; reading c1 in DESIGN.md: ties go up).
 // Returns false if the shift does not fit comfortably in 32 bits.
-bool axis_shift(double v, double a, double dt, double j, int32_t *shift);
+bool axis_shift(double v, double a, double dt, double j, int32_t *shift, bool *tie = nullptr);
 
 struct AxisClass {
     float v, a;                  // px/frame, px/frame^2 (exact float32 values of the ABI)
     int32_t smin, smax;          // extreme integer shifts over t = 0..T-1
     std::vector<int32_t> shift;  // [T]
+    bool tie = false;            // some frame has d + 1/2 exactly integer (the rounding is then not odd in d)
+    bool jittered = false;       // a non-zero jitter enters the displacement of this class
 };
 
 struct Batch {
@@ -30,12 +32,33 @@ struct Batch {
     int32_t max_spread;          // max over t of (max_e sy - min_e sy)
 };
 
+// A SLOT of the separable kernel holds the y-motion (v, a) and, when the filter is symmetric under the
+// reflection y -> -y, also its mirror image (-v, -a): shift_t and phase_t change sign, the 5 taps reverse,
+// so that with the even and odd parts of the taps
+//     N_plus  = E + O,   N_minus = E - O,    E = w2 X0 + s1 (X+1 + X-1) + s2 (X+2 + X-2),
+//                                            O =         d1 (X+1 - X-1) + d2 (X+2 - X-2)
+// both members are accumulated with 5 multiply-adds per pixel and frame instead of 10 (exact algebra;
+// DESIGN.md "mirror pairs").  member[0] moves as (v, a) with v > 0 or (v == 0, a >= 0) when the class is
+// pairable, member[1] as (-v, -a); either may be absent (-1).  A class that is not pairable (exact rounding
+// ties, jitter on the y axis, a filter without the symmetry) sits alone in member[0] in its own orientation.
+struct Slot {
+    int32_t member[2];           // trajectory indices or -1
+    int32_t ycls;                // y-class the tables are built from (index into Plan::ycls)
+    int32_t flip;                // 1: that class is the mirror image of the slot's orientation
+};
+
+struct SlotBatch {
+    int32_t xcls;
+    std::vector<Slot> slots;     // size <= max_slots
+};
+
 struct Plan {
     int32_t T = 0;
     double t0 = 0.0;
     std::vector<AxisClass> xcls, ycls;
     std::vector<int32_t> traj_xc, traj_yc;   // [n_traj]
     std::vector<Batch> batches;
+    std::vector<SlotBatch> slot_batches;
 };
 
 // Group trajectories into axis classes.  Returns TNO_MF_OK or TNO_MF_EINVAL (shift overflow).
@@ -51,5 +74,10 @@ int build_classes(const tno_mf_traj *traj, int32_t n_traj, int32_t T, double t0,
 // is split into the fewest batches, of sizes that differ by at most one.
 constexpr int32_t kUnlimitedSpread = 1 << 30;
 void build_batches(Plan *plan, int32_t max_entries, int32_t max_spread);
+
+// Pack the trajectories of each x-class into slots (mirror pairs where `symmetric_filter` and the class
+// allow it) and the slots, ordered by (|v|-orientation v, a), into the fewest batches of at most max_slots
+// slots, of sizes that differ by at most one.  Duplicate trajectories get slots of their own.
+void build_slot_batches(Plan *plan, int32_t max_slots, bool symmetric_filter);
 
 }  // namespace tno

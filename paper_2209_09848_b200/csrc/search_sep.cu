@@ -7,6 +7,17 @@
 //     N_e(x, y)  += sum_j (gy_{e,t}[j] / sigma_t^2) X_t(x, y + d_{e,t} + j - 2)        (y-pass, per entry)
 // for all frames t, where d_{e,t} is the integer y-shift of entry e at frame t.
 //
+// MIRROR PAIRS.  The entries of a batch are grouped into SLOTS (plan.h): a slot holds a y-motion (v, a) and its
+// mirror image (-v, -a).  The mirror's shift is -d and its five taps are the reversed taps, so with the even and
+// odd parts of the taps, s_j = (w[2+j] + w[2-j]) / 2 and d_j = (w[2+j] - w[2-j]) / 2,
+//     E += w[2] X(P) + s_1 (X(P+1) + X(P-1)) + s_2 (X(P+2) + X(P-2))
+//     O +=             d_1 (X(P+1) - X(P-1)) + d_2 (X(P+2) - X(P-2))
+//     N_plus(x, P - d) = E + O,     N_minus(x, P + d) = E - O
+// both members cost 5 multiply-adds per position and frame instead of 10 (the sums and differences of the
+// window rows are shared by all slots of the batch).  Exact algebra: results differ from the tap-by-tap sum
+// only by rounding.  A slot without a mirror in the bank is evaluated the same way (E + O only), so the map of
+// a trajectory does not depend on the rest of the bank.
+//
 // The y-pass is indexed by the POSITION P = y + d_{e,t} of the track in frame t, not by the start
 // pixel y: a CTA owns the frame-space rows P in [Y0, Y0 + HT) of a 64-column strip, so every entry
 // reads the SAME rows P-2..P+2 of X_t.  A thread loads its R+4 window rows of X_t once per frame
@@ -98,15 +109,17 @@ constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per
 // stage table entry (32-bit words), one per (batch, frame t):
 //   [0] xo = 4*floor((sx - 2)/4), the 16-byte aligned x offset of the staged box relative to the tile
 //   [1] o = sx - 2 - xo in 0..3, the column of the box at which the 5-tap window of output 0 starts
-//   [2] number of entries of the batch (they occupy slots 0 .. n-1)
-//   [3] flush mask: bit e set if entry e must be flushed after this frame
+//   [2] number of slots of the batch (they occupy slots 0 .. n-1)
+//   [3] flush mask: bit s set if slot s must be flushed after this frame
 //   [4..8] gx[0..4]
-//   [10] wait mask: bit e set if the previous flush of entry e is at most XR frames back
-//   [16 + 8e + 0..4] gy_e[0..4] / sigma_t^2   [16 + 8e + 5] d_{e,t}          (entry e; zeros if empty)
+//   [10] wait mask: bit s set if the previous flush of slot s is at most XR frames back
+//   [16 + 8s + 0..4] (w[2], s_1, s_2, d_1, d_2) / sigma_t^2 of slot s (zeros if empty)
+//   [16 + 8s + 5] d_{s,t}    [16 + 8s + 6], [.. + 7] planned-order index of the plus / minus member relative
+//                            to the first one of the batch, -1 = absent
 
 template <int R_, int NB_, int CW_, int SB_, int XR_>
 struct SepCfg {
-    static constexpr int R = R_, NB = NB_, CW = CW_, SB = SB_, XR = XR_;
+    static constexpr int R = R_, NB = NB_, CW = CW_, SB = SB_, XR = XR_;      // NB = slots per batch
     static constexpr int NT = 32 * (CW + kPW);     // consumer warps 0 .. CW-1, then the producer warpgroup
     static constexpr int HT = R * CW;              // positions (rows) per tile: consumer warp w owns w*R ..
     static constexpr int XROWS = HT + 4;
@@ -120,7 +133,9 @@ struct SepCfg {
     // register split: setmaxnreg moves registers between the warpgroups of the CTA, the total stays
     // what the launch allocated (NT x the per-thread count ptxas derives from __launch_bounds__)
     static constexpr int LREGS = 65536 / NT / 8 * 8;
-    static constexpr int PREGS = 56, CREGS = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
+    static constexpr int PREGS = 56;
+    static constexpr int CREGS_RAW = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
+    static constexpr int CREGS = CREGS_RAW > 232 ? 232 : CREGS_RAW;
     static_assert(CW % 4 == 0 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * LREGS, "register budget");
     static_assert((SB & (SB - 1)) == 0 && (XR & (XR - 1)) == 0 && (TS & (TS - 1)) == 0 && TS >= SB + XR + 2,
                   "ring sizes are powers of two");
@@ -138,14 +153,15 @@ __device__ __forceinline__ int32_t seg_phase(float v, float a) {
 // ------------------------------------------------------------------------------------ table kernel
 template <class C>
 __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_xc,
-                             const int32_t *__restrict__ batch_yc, int32_t n_batches, int32_t squared,
+                             const int32_t *__restrict__ slot_yc, const int32_t *__restrict__ slot_flip,
+                             const int32_t *__restrict__ slot_q, int32_t n_batches, int32_t squared,
                              float *__restrict__ stage_tab) {
     const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int32_t T = tab.T;
     if (id >= (int64_t)n_batches * T) return;
     const int32_t b = (int32_t)(id / T), t = (int32_t)(id % T);
     const int32_t xc = batch_xc[b];
-    const int32_t *yc = batch_yc + (int64_t)b * C::NB;
+    const int32_t *yc = slot_yc + (int64_t)b * C::NB;
     float *out = stage_tab + id * C::TABW;
     int32_t *outi = reinterpret_cast<int32_t *>(out);
     auto align4 = [](int32_t v) { return v & ~3; };          // floor to a multiple of 4 (two's complement)
@@ -163,24 +179,35 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
         float *oe = out + kHdr + 8 * e;
         int32_t *oi = reinterpret_cast<int32_t *>(oe);
         for (int j = 0; j < 8; ++j) oi[j] = 0;
+        oi[6] = oi[7] = -1;
         if (yc[e] < 0) continue;
         n = e + 1;
+        const int32_t flip = slot_flip[(int64_t)b * C::NB + e];
         const int32_t c = tab.n_x + yc[e];
         const int64_t ci = (int64_t)c * T + t;
+        // taps of the slot's orientation: those of the class, reversed if the class is the mirror image
+        double w[5];
         for (int j = 0; j < 5; ++j) {
-            const double gv = tab.gd[ci * 5 + j];
-            oe[j] = (float)((squared ? gv * gv : gv) * tab.qd[t]);
+            const double gv = tab.gd[ci * 5 + (flip ? 4 - j : j)];
+            w[j] = (squared ? gv * gv : gv) * tab.qd[t];
         }
-        oi[5] = tab.shift[ci];
+        oe[0] = (float)w[2];
+        oe[1] = (float)(0.5 * (w[3] + w[1]));
+        oe[2] = (float)(0.5 * (w[4] + w[0]));
+        oe[3] = (float)(0.5 * (w[3] - w[1]));
+        oe[4] = (float)(0.5 * (w[4] - w[0]));
+        oi[5] = flip ? -tab.shift[ci] : tab.shift[ci];
+        oi[6] = slot_q[((int64_t)b * C::NB + e) * 2];
+        oi[7] = slot_q[((int64_t)b * C::NB + e) * 2 + 1];
         // flush before the mapping position -> output row changes, once per kSeg frames, and after
-        // the last frame
-        const bool fl = (t == T - 1) || (tab.shift[ci + 1] != tab.shift[ci]) ||
-                        ((t + 1 + seg_phase(tab.cls_v[c], tab.cls_a[c])) % kSeg == 0);
+        // the last frame.  The phase of the periodic flush is that of the slot's orientation.
+        const float ov = (flip ? -tab.cls_v[c] : tab.cls_v[c]) + 0.0f, oa = (flip ? -tab.cls_a[c] : tab.cls_a[c]) + 0.0f;
+        const int32_t ph = seg_phase(ov, oa);
+        const bool fl = (t == T - 1) || (tab.shift[ci + 1] != tab.shift[ci]) || ((t + 1 + ph) % kSeg == 0);
         if (fl) {
             fmask |= 1 << e;
-            // was the entry also flushed after one of the frames t - XR .. t - 1 ?  (t < XR: the
-            // last frame of the CTA's previous work item, where every entry is flushed, is that close)
-            const int32_t ph = seg_phase(tab.cls_v[c], tab.cls_a[c]);
+            // was the slot also flushed after one of the frames t - XR .. t - 1 ?  (t < XR: the
+            // last frame of the CTA's previous work item, where every slot is flushed, is that close)
             if (t < C::XR) fwait |= 1 << e;
             for (int32_t u = max(t - C::XR, 0); u < t; ++u)
                 if (tab.shift[ci - t + u + 1] != tab.shift[ci - t + u] || (u + 1 + ph) % kSeg == 0) fwait |= 1 << e;
@@ -329,54 +356,65 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::CREGS));
         const int32_t r0 = warp * R;
         int32_t n = 0;
-        uint32_t fpar = 0;        // bit e = parity of the number of flushes of entry e so far
+        uint32_t fpar = 0;        // bit s = parity of the number of flushes of slot s so far
         for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-            // flush coordinates of the item: entry s of the batch has planned index q_first + s, its
-            // piece map starts at ebase + s*H*W (this lane's two columns), and the accumulator row r
-            // of this warp holds output row yr0 + r - d
+            // flush coordinates of the item: the members of the batch have planned indices q_first + (the
+            // offsets in the table), a member's piece map starts at ebase + offset*H*W (this lane's two
+            // columns), and the accumulator row r of this warp holds output row yr0 + r - d (plus member) or
+            // yr0 + r + d (minus member)
             const int32_t b = item % a.n_batches, tile = a.ty0 * ntx + item / a.n_batches;
             const int32_t ty = tile / ntx;
             const int32_t x = (tile % ntx) * kTileW + 2 * lane;
             float *ebase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride +
-                           (int64_t)(__ldg(a.batch_q + (int64_t)b * NB) - a.q0) * H * W + x;
+                           (int64_t)(__ldg(a.batch_q + b) - a.q0) * H * W + x;
             // columns past the frame: make every row test fail
             const int32_t yr0 = (x < W) ? ty * HT - 2 + r0 : INT32_MIN / 2;
             // else: positions without any tap in the frame
             const bool y_active = r0 < min(HT, H + 4 - ty * HT);
 
-            float2 acc[NB][R];
+            float2 accE[NB][R], accO[NB][R];
 #pragma unroll
             for (int s = 0; s < NB; ++s)
 #pragma unroll
-                for (int i = 0; i < R; ++i) acc[s][i] = make_float2(0.f, 0.f);
+                for (int i = 0; i < R; ++i) accE[s][i] = accO[s][i] = make_float2(0.f, 0.f);
 
             for (int32_t t = 0; t < T; ++t) {
                 const int32_t xr = n & (XR - 1);
                 mbar_wait(x_full + 8 * (xr), (n / XR) & 1);
                 const float *th = Tab + (n & (TS - 1)) * TABW;
                 const float *tb = th + kHdr;
-                // number of entries and flush mask of the frame, read together ahead of the FFMAs
+                // number of slots and flush mask of the frame, read together ahead of the FFMAs
                 const int2 hdr23 = *reinterpret_cast<const int2 *>(th + 2);
                 if (y_active) {
-                    // ---------------- y-pass: one register window of X for all entries of the batch
+                    // ---------------- y-pass: one register window of X for all slots of the batch, and the
+                    // sums and differences of its rows about each of this thread's R positions
                     const float2 *xp = reinterpret_cast<const float2 *>(Xbuf + xr * C::XBUF + r0 * kXP) + lane;
                     float2 win[R + 4];
 #pragma unroll
                     for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
+                    float2 A1[R], B1[R], A2[R], B2[R];
+                    const float2 neg1 = make_float2(-1.f, -1.f);
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        A1[r] = __fadd2_rn(win[r + 3], win[r + 1]);
+                        B1[r] = __ffma2_rn(neg1, win[r + 1], win[r + 3]);       // exact difference
+                        A2[r] = __fadd2_rn(win[r + 4], win[r]);
+                        B2[r] = __ffma2_rn(neg1, win[r], win[r + 4]);
+                    }
                     const int32_t nfill = hdr23.x;
-#define TNO_FMAS(s)                                                                                   \
-    {                                                                                                 \
-        const float2 w0 = make_float2(wa.x, wa.x), w1 = make_float2(wa.y, wa.y),                      \
+#define TNO_FMAS(s)                                                                                      \
+    {                                                                                                    \
+        const float2 w0 = make_float2(wa.x, wa.x), w1 = make_float2(wa.y, wa.y),                         \
                      w2 = make_float2(wa.z, wa.z), w3 = make_float2(wa.w, wa.w), w5 = make_float2(w4, w4); \
-        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w0, win[r], acc[s][r]);     \
-        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w1, win[r + 1], acc[s][r]); \
-        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w2, win[r + 2], acc[s][r]); \
-        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w3, win[r + 3], acc[s][r]); \
-        _Pragma("unroll") for (int r = 0; r < R; ++r) acc[s][r] = __ffma2_rn(w5, win[r + 4], acc[s][r]); \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) accE[s][r] = __ffma2_rn(w0, win[r + 2], accE[s][r]); \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) accO[s][r] = __ffma2_rn(w3, B1[r], accO[s][r]);      \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) accE[s][r] = __ffma2_rn(w1, A1[r], accE[s][r]);      \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) accO[s][r] = __ffma2_rn(w5, B2[r], accO[s][r]);      \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) accE[s][r] = __ffma2_rn(w2, A2[r], accE[s][r]);      \
     }
                     if (nfill == NB) {
-                        // full batch: straight-line code, the weights of entry s + 1 are loaded
-                        // before the FFMAs of entry s (the empty asm keeps ptxas from hoisting more
+                        // full batch: straight-line code, the weights of slot s + 1 are loaded
+                        // before the FFMAs of slot s (the empty asm keeps ptxas from hoisting more
                         // loads than the register budget holds)
                         float4 wa = *reinterpret_cast<const float4 *>(tb);
                         float w4 = tb[4];
@@ -409,13 +447,13 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 if (lane == 0) mbar_arrive(x_empty + 8 * (xr));      // this warp no longer reads X[xr]
                 if (fmask != 0) {
                     const int32_t fwait = reinterpret_cast<const int32_t *>(th)[10];
-                    // ---------------- flush: piece[ty mod NP][entry][P - d][x] += acc, acc = 0
+                    // ---------------- flush: piece[ty mod NP][member][P -+ d][x] += E +- O, E = O = 0
 #pragma unroll
                     for (int s = 0; s < NB; ++s) {
                         if (fmask & (1 << s)) {
-                            // The output rows a warp holds change with d, so successive flushes of an
-                            // entry touch the same addresses from different warps: flush k starts only
-                            // after every consumer warp has finished flush k - 1 of that entry, which
+                            // The output rows a warp holds change with d, so successive flushes of a
+                            // slot touch the same addresses from different warps: flush k starts only
+                            // after every consumer warp has finished flush k - 1 of that slot, which
                             // fixes the order of the float adds per address.  If flush k - 1 is more
                             // than XR frames back that is already implied by X[n] being there (the
                             // producers waited for every consumer to release frame n - XR, which each
@@ -424,15 +462,22 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                             if (fwait & (1 << s)) mbar_wait(f_done + 8 * (s), ((fpar >> s) & 1u) ^ 1u);
                             fpar ^= 1u << s;
                             if (y_active) {
-                                const int32_t yb = yr0 - reinterpret_cast<const int32_t *>(tb)[8 * s + 5];
-                                float *p = ebase + (int64_t)(s * H + yb) * W;
-                                asm volatile("" : "+l"(p));      // one address, then p += W per row
+                                const int4 dq = *reinterpret_cast<const int4 *>(tb + 8 * s + 4);   // (d_2, d, q+, q-)
+                                const int32_t yp = yr0 - dq.y, ym = yr0 + dq.y;
+                                float *pp = ebase + ((int64_t)dq.z * H + yp) * W;
+                                float *pm = ebase + ((int64_t)dq.w * H + ym) * W;
+                                asm volatile("" : "+l"(pp), "+l"(pm));      // one address each, then += W per row
+                                const bool hp = dq.z >= 0, hm = dq.w >= 0;
 #pragma unroll
-                                for (int r = 0; r < R; ++r, p += W) {
-                                    // the piece address is owned by this CTA, and f_done orders the adds
+                                for (int r = 0; r < R; ++r, pp += W, pm += W) {
+                                    // the piece addresses are owned by this CTA, and f_done orders the adds
                                     // of successive flushes; rows outside the frame are predicated off
-                                    red_add_v2_if((uint32_t)(yb + r) < (uint32_t)H, p, acc[s][r]);
-                                    acc[s][r] = make_float2(0.f, 0.f);
+                                    const float2 e = accE[s][r], o = accO[s][r];
+                                    red_add_v2_if(hp && (uint32_t)(yp + r) < (uint32_t)H, pp,
+                                                  make_float2(e.x + o.x, e.y + o.y));
+                                    red_add_v2_if(hm && (uint32_t)(ym + r) < (uint32_t)H, pm,
+                                                  make_float2(e.x - o.x, e.y - o.y));
+                                    accE[s][r] = accO[s][r] = make_float2(0.f, 0.f);
                                 }
                             }
                             __syncwarp();
@@ -530,12 +575,11 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
 }
 
 // ------------------------------------------------------------------------------------ host side
-// (rows per thread, entries per batch, consumer warps, box stages, X buffers): tiles of 12 R positions x
-// 64 columns, 384 consumer + 128 producer threads.  Both variants fill the consumers' 152 registers with
-// accumulators: 7 rows x 8 entries (112 + 22 window registers, 280 FFMA2 per frame and warp) and 5 rows x 10
-// entries (100 + 18, 250 FFMA2); 6 x 10 spills and is slower, 5 x 8 leaves registers idle (measured: DESIGN.md)
-using V0 = SepCfg<7, 8, 12, 4, 4>;
-using V1 = SepCfg<5, 10, 12, 4, 4>;
+// (rows per thread, slots per batch, consumer warps, box stages, X buffers): tiles of CW x R positions x 64
+// columns.  A slot costs 4 R accumulator registers (E and O, two columns), the window and its sums and
+// differences 2 (R + 4) + 8 R.
+using V0 = SepCfg<4, 5, 12, 4, 4>;
+using V1 = SepCfg<6, 5, 8, 4, 4>;
 
 int32_t sep_num_variants() { return 2; }
 SepVariant sep_variant(int32_t v) { return v == 0 ? SepVariant{V0::NB, V0::HT} : SepVariant{V1::NB, V1::HT}; }
@@ -546,11 +590,14 @@ int32_t sep_tile_rows(int32_t v, int32_t H) {
 }
 
 void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
-                       const int32_t *batch_yc, int32_t n_batches, int32_t squared, float *stage_tab) {
+                       const int32_t *slot_yc, const int32_t *slot_flip, const int32_t *slot_q, int32_t n_batches,
+                       int32_t squared, float *stage_tab) {
     const int64_t n = (int64_t)n_batches * tab.T;
     const unsigned grid = (unsigned)((n + 127) / 128);
-    if (v == 0) k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, batch_yc, n_batches, squared, stage_tab);
-    else k_sep_tables<V1><<<grid, 128, 0, st>>>(tab, batch_xc, batch_yc, n_batches, squared, stage_tab);
+    if (v == 0)
+        k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
+    else
+        k_sep_tables<V1><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
@@ -610,6 +657,7 @@ void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, i
                    const int32_t *perm, int32_t q0, int32_t q_count, const TrajInfo *traj, const float *rsd,
                    int32_t H, int32_t W, int32_t fy0, int32_t fy1, float *out_snr, uint64_t *maxkeys,
                    const TopkSlots &slots) {
+    if (fy1 <= fy0 || q_count <= 0) return;      // nothing left to finish (the banded host search may be done early)
     dim3 grid((unsigned)((W + kCollectTile - 1) / kCollectTile), (unsigned)(fy1 - fy0), (unsigned)q_count);
     k_finish<<<grid, 256, 0, st>>>(pieces, dpieces, n_pieces, piece_stride, perm, q0, traj, rsd, H, W, fy0, out_snr,
                                    reinterpret_cast<unsigned long long *>(maxkeys), slots);

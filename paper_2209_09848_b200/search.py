@@ -141,5 +141,5 @@ class MatchedFilter:
     def kernel_ms(self) -> float:
         return B.tno_mf_last_kernel_ms(self.ctx)
 
-    def work(self) -> Tuple[float, float]:
+    def work(self) -> Tuple[float, float, float]:
         return B.tno_mf_last_work(self.ctx)

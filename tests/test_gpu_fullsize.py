@@ -1,6 +1,7 @@
 """GPU parity at BASELINE.json's full sizes (configs 3, 4, 5), in the launch configuration
 bench.py times.  The full oracle would take ~10 min - 1 h per config, so parity is checked on
-(i) full-T oracle maps of 256 x 256 crops (interior, edges, corner) for a spread of trajectories,
+(i) full-T oracle maps of 256 x 256 crops (interior, edges, corner) for a spread of trajectories, and the WHOLE
+2048 x 2048 map of the slowest and the fastest (corner-of-the-grid) trajectories,
 (ii) oracle_point at every sampled GPU candidate, every injected source, hot pixels and random
 (k, x, y), (iii) the GPU candidate lists against a plain sort of the GPU's own maps.
 Needs a B200 with ~100 GB of free HBM and ~100 GB of host RAM (config 4).  `pytest -m gpu`."""
@@ -41,6 +42,15 @@ def _crops(cfg, size=256):
             (W - size, H - size)]                             # bottom-right corner
 
 
+def _whole_map_trajs(p):
+    """The slowest trajectory and the four corners of the velocity grid (the fastest ones, both diagonals)."""
+    vx, vy = p.traj[:, 0].astype(np.float64), p.traj[:, 1].astype(np.float64)
+    picks = [int(np.argmin(np.hypot(vx, vy)))]
+    for sx, sy in ((-1, -1), (1, -1), (-1, 1), (1, 1)):
+        picks.append(int(np.argmax(sx * vx + sy * vy)))
+    return picks
+
+
 def _check_points(host, p, cfg, pts, gpu_vals):
     worst = 0.0
     for (k, x, y), g in zip(pts, gpu_vals):
@@ -50,7 +60,7 @@ def _check_points(host, p, cfg, pts, gpu_vals):
     return worst
 
 
-def _fullsize_with_maps(cfg, n_crop_traj, n_random):
+def _fullsize_with_maps(cfg, n_crop_traj, n_random, n_whole):
     torch, mf, p, frames = _setup(cfg)
     maps, cand = mf.search(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0)
     torch.cuda.synchronize()
@@ -67,6 +77,12 @@ def _fullsize_with_maps(cfg, n_crop_traj, n_random):
         gm = maps[torch.from_numpy(ks).cuda()][:, cy:cy + 256, cx:cx + 256].cpu().numpy()
         err = np.abs(gm.astype(np.float64) - om)
         assert err.max() <= TOL, (cx, cy, err.max(), np.unravel_index(err.argmax(), err.shape))
+    # (i-b) WHOLE maps against the oracle (SURVEY 8(c) "one full-frame oracle run on a few trajectories"): every
+    # tile row, tile column and piece slot of the benchmarked launch is visited; |dSNR| <= 1e-3 at every pixel
+    for k in _whole_map_trajs(p)[:n_whole]:
+        om = oracle.snr_map(host, p.sigma_t, p.traj[k:k + 1], cfg.prf_sigma, cfg.t0)[0]
+        err = np.abs(maps[k].cpu().numpy().astype(np.float64) - om)
+        assert err.max() <= TOL, (k, err.max(), np.unravel_index(err.argmax(), err.shape))
     # (iii) candidate lists = plain sort of the GPU's own maps (all trajectories)
     for k in range(cfg.n_traj):
         check_topk_vs_own_map(c[k], maps[k].cpu().numpy(), k, cfg.topk, cfg.threshold)
@@ -113,11 +129,11 @@ def _fullsize_with_maps(cfg, n_crop_traj, n_random):
 
 
 def test_config3_headline_sampled_parity():
-    _fullsize_with_maps(tno_synth.CONFIGS[3], n_crop_traj=8, n_random=3000)
+    _fullsize_with_maps(tno_synth.CONFIGS[3], n_crop_traj=8, n_random=3000, n_whole=5)
 
 
 def test_config4_long_sector_sampled_parity():
-    _fullsize_with_maps(tno_synth.CONFIGS[4], n_crop_traj=6, n_random=600)
+    _fullsize_with_maps(tno_synth.CONFIGS[4], n_crop_traj=6, n_random=600, n_whole=3)
 
 
 def test_config5_curved_topk_only():

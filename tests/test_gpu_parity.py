@@ -90,6 +90,42 @@ def test_ragged_shapes_and_mixed_trajectories(shape, force_generic):
         check_topk_vs_own_map(gc[k], gm[k], k, 7, 2.5)
 
 
+@pytest.mark.parametrize("offset_floats", [1, 2, 3])
+def test_frames_pointer_not_16_byte_aligned_takes_the_generic_kernel(offset_floats):
+    """SURVEY 8(b) shape rule: the TMA path needs a 16-byte aligned `frames`; a stack that starts 4, 8 or 12 bytes
+    past such a boundary (a view into a larger buffer) must take the generic kernel and give the same answer.  The
+    validity weights of a masked search fall under the same rule."""
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    T, H, W = 9, 72, 64
+    rng = np.random.default_rng(offset_floats)
+    f = rng.standard_normal((T, H, W)).astype(np.float32)
+    sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
+    traj = np.array([[0.3, -0.2, 0, 0], [0.3, 0.45, 0, 0], [-1.25, 0.5, 0, 0.02], [0, 0, 0, 0]], np.float32)
+    om = oracle.snr_map(f, sigma, traj, 1.0, 4.0)
+    buf = torch.zeros(T * H * W + 8, dtype=torch.float32, device="cuda")
+    assert buf.data_ptr() % 16 == 0
+    view = buf[offset_floats:offset_floats + T * H * W].view(T, H, W)
+    view.copy_(torch.from_numpy(f))
+    assert view.data_ptr() % 16 == 4 * offset_floats and view.is_contiguous()
+    gm, gc, stats = run_gpu(view, sigma, traj, 1.0, 4.0, 6, 2.5)
+    assert stats[1] == 0, "an unaligned stack must not go to the TMA kernel"
+    assert np.abs(gm.astype(np.float64) - om).max() <= TOL
+    for k in range(traj.shape[0]):
+        check_topk(gc[k], om[k], k, 6, 2.5)
+    # aligned frames, unaligned validity weights
+    ctx = P.tno_mf_create(0, None, 0, 0.0)
+    fd = torch.from_numpy(f).cuda()
+    vbuf = torch.ones(T * H * W + 8, dtype=torch.float32, device="cuda")
+    valid = vbuf[offset_floats:offset_floats + T * H * W].view(T, H, W)
+    out = torch.empty((4, H, W), device="cuda")
+    P.tno_mf_search_masked(ctx, fd, valid, sigma, None, None, traj, 1.0, 4.0, out, None)
+    torch.cuda.synchronize()
+    assert P.tno_mf_last_stats(ctx)[1] == 0
+    assert np.abs(out.cpu().numpy().astype(np.float64) - om).max() <= TOL
+    P.tno_mf_destroy(ctx)
+
+
 def test_zero_frames_and_threshold_edges():
     torch = _torch()
     T, H, W = 5, 64, 64

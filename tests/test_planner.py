@@ -91,3 +91,84 @@ def test_unlimited_spread_splits_evenly():
     for idx, nb, expect in ((3, 10, 10), (5, 8, 128), (5, 10, 128), (4, 8, 8)):
         cfg = tno_synth.CONFIGS[idx]
         assert tno_mf_plan(tno_synth.trajectories(cfg), cfg.T, cfg.t0, nb, unlimited)[0] == expect
+
+
+# ---- slots: mirror pairs (tno_mf_plan_slots) ------------------------------------------------------
+from paper_2209_09848_b200 import tno_mf_plan_slots  # noqa: E402
+
+
+def _check_slots(traj, T, t0, ns=5, sym=True, **kw):
+    n, batch, slot, member = tno_mf_plan_slots(traj, T, t0, ns, sym, **kw)
+    assert np.all(batch >= 0) and np.all(batch < n) and np.all(slot >= 0) and np.all(slot < ns)
+    assert set(member.tolist()) <= {0, 1}
+    seen = set(zip(batch.tolist(), slot.tolist(), member.tolist()))
+    assert len(seen) == len(traj), "every trajectory owns exactly one (batch, slot, member)"
+    for b in range(n):
+        ks = np.nonzero(batch == b)[0]
+        assert len({(float(traj[k, 0]), float(traj[k, 2])) for k in ks}) == 1, "one x-motion per batch"
+        assert sorted(set(slot[ks].tolist())) == list(range(len(set(slot[ks].tolist())))), "slots 0 .. n-1"
+        for s in set(slot[ks].tolist()):
+            mem = ks[slot[ks] == s]
+            if len(mem) == 2:           # a pair: exact mirror images in y, sharing the x-motion
+                p, q = (mem[0], mem[1]) if member[mem[0]] == 0 else (mem[1], mem[0])
+                assert member[p] == 0 and member[q] == 1
+                assert traj[p, 1] == -traj[q, 1] and traj[p, 3] == -traj[q, 3]
+                assert traj[p, 1] > 0 or (traj[p, 1] == 0 and traj[p, 3] >= 0)
+    return n, batch, slot, member
+
+
+def _n_pairs(batch, slot):
+    _, counts = np.unique(np.stack([batch, slot], 1), axis=0, return_counts=True)
+    assert counts.max() <= 2
+    return int(np.count_nonzero(counts == 2))
+
+
+def test_slots_of_the_config_banks():
+    """The velocity grids of the five configs are symmetric about zero: every vy < 0 pairs with its mirror image."""
+    for idx, batches, pairs in ((1, 3, 3), (2, 5, 10), (3, 10, 50), (4, 8, 32)):
+        cfg = tno_synth.CONFIGS[idx]
+        traj = tno_synth.trajectories(cfg)
+        n, batch, slot, member = _check_slots(traj, cfg.T, cfg.t0)
+        assert n == batches
+        assert _n_pairs(batch, slot) == pairs
+    # config 5: ay = +2e-5 has no mirror image in the bank -> 256 single slots (the 128 with vy < 0 are lone
+    # minus members), (1024 - 256) / 2 pairs
+    cfg = tno_synth.CONFIGS[5]
+    traj = tno_synth.trajectories(cfg)
+    n, batch, slot, member = _check_slots(traj, cfg.T, cfg.t0)
+    assert _n_pairs(batch, slot) == 384 and int(np.count_nonzero(member == 1)) == 384 + 128
+    assert n == 16 * 5 + 32 * 2            # ax = 0: 8 pairs + 16 singles = 24 slots; ax != 0: 8 pairs
+
+
+def test_no_pairs_without_symmetry_with_ties_or_with_y_jitter():
+    traj = np.array([[0.1, v, 0, 0] for v in (-0.3, -0.1, 0.0, 0.1, 0.3)], dtype=np.float32)
+    assert np.count_nonzero(_check_slots(traj, 40, 20.0)[3] == 1) == 2
+    assert np.count_nonzero(_check_slots(traj, 40, 20.0, sym=False)[3] == 1) == 0
+    jit = np.zeros((40, 2), np.float32)
+    jit[:, 0] = 0.3                                             # jitter in x only: still pairs
+    assert np.count_nonzero(_check_slots(traj, 40, 20.0, jitter_xy=jit)[3] == 1) == 2
+    jit[7, 1] = 0.01                                            # any jitter in y breaks the mirror symmetry
+    assert np.count_nonzero(_check_slots(traj, 40, 20.0, jitter_xy=jit)[3] == 1) == 0
+    # exact half-pixel ties (v = +-0.5 at odd dt): floor(-d + 1/2) != -floor(d + 1/2), so +-0.5 must not pair,
+    # while +-0.3 (never exactly on a tie) still do
+    tie = np.array([[0, 0.5, 0, 0], [0, -0.5, 0, 0], [0, 0.3, 0, 0], [0, -0.3, 0, 0]], dtype=np.float32)
+    n, batch, slot, member = _check_slots(tie, 10, 0.0)
+    assert member[0] == 0 and member[1] == 0 and slot[0] != slot[1]
+    assert member[2] == 0 and member[3] == 1 and slot[2] == slot[3]
+    # irregular frame times keep the symmetry (d is odd in (v, a) for any dt)
+    times = np.cumsum(np.random.default_rng(0).uniform(0.5, 1.5, 40)).astype(np.float32)
+    assert np.count_nonzero(_check_slots(traj, 40, 20.0, frame_times=times)[3] == 1) == 2
+
+
+def test_duplicates_and_lonely_mirror_images():
+    traj = np.array([[0.1, 0.2, 0, 0], [0.1, 0.2, 0, 0], [0.1, -0.2, 0, 0], [0.2, -0.4, 0, 1e-4], [0.1, 0.0, 0, 0],
+                     [0.1, 0.0, 0, 0]], dtype=np.float32)
+    n, batch, slot, member = _check_slots(traj, 30, 15.0)
+    assert n == 2
+    assert member.tolist() == [0, 0, 1, 1, 0, 0]                # a lone negative motion is the minus member
+    assert slot[0] != slot[1] and slot[2] in (slot[0], slot[1])  # the duplicate gets a slot of its own
+    assert slot[4] != slot[5]
+    with pytest.raises(TnoMfError):
+        tno_mf_plan_slots(traj, 30, float("nan"))
+    with pytest.raises(TnoMfError):
+        tno_mf_plan_slots(traj, 30, 0.0, 17)
