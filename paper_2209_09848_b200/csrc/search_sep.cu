@@ -234,16 +234,63 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
+// x-pass of one thread and step: 8 outputs X(c .. c+7) = sum_i g[i] R(c + O + i) from the 16 staged values
+// R(c .. c+15) of its row (four 16-byte loads), O = 0..3 the offset of the window in the 16-byte aligned box.
+struct XIn { float4 a, b, c, d; };
+__device__ __forceinline__ XIn xpass_load(const float *p) {
+    const float4 *p4 = reinterpret_cast<const float4 *>(p);
+    return XIn{p4[0], p4[1], p4[2], p4[3]};
+}
+template <int O>
+__device__ __forceinline__ void xpass_step(const XIn &u, float *dst, const float (&g)[5]) {
+    const float r[16] = {u.a.x, u.a.y, u.a.z, u.a.w, u.b.x, u.b.y, u.b.z, u.b.w,
+                         u.c.x, u.c.y, u.c.z, u.c.w, u.d.x, u.d.y, u.d.z, u.d.w};
+    float v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = g[0] * r[O + j];
+#pragma unroll
+    for (int i = 1; i < 5; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v[j] = fmaf(g[i], r[O + j + i], v[j]);
+    reinterpret_cast<float4 *>(dst)[0] = make_float4(v[0], v[1], v[2], v[3]);
+    reinterpret_cast<float4 *>(dst)[1] = make_float4(v[4], v[5], v[6], v[7]);
+}
+// One frame of one producer warp: this lane's rows row_in, row_in + 8, ... of the box, columns 8 oct_in .. + 7
+// and 32 + 8 oct_in .. + 7.  The loads of the next step are issued before the arithmetic of the current one
+// (in program order ahead of its stores, which the compiler must assume may alias them).
+template <int O>
+__device__ __forceinline__ void xpass_frame(const float *src, float *dst, int32_t nfull, bool tail,
+                                            const float (&g)[5]) {
+    const int32_t nstep = 2 * nfull;
+    XIn u = xpass_load(src);
+    for (int32_t i = 0; i < nstep; ++i) {
+        // step i: row group i >> 1, column half i & 1
+        const float *nsrc = src + ((i & 1) ? 8 * kBoxW - 32 : 32);
+        XIn un = u;
+        if (i + 1 < nstep || tail) un = xpass_load(nsrc);
+        xpass_step<O>(u, dst, g);
+        dst += (i & 1) ? 8 * kXP - 32 : 32;
+        src = nsrc;
+        u = un;
+    }
+    if (tail) {
+        const XIn u2 = xpass_load(src + 32);
+        xpass_step<O>(u, dst, g);
+        xpass_step<O>(u2, dst + 32, g);
+    }
+}
+
 // Warp-specialised, persistent.  Per CTA-local frame counter n (frames of all its work items in
 // sequence) three rings connect the roles:
-//   box[n % SB]  TMA -> producers      full_box  (tx bytes; also covers tab[n % TS])
-//   X[n % XR]    producers -> consumers x_full   (kPW arrivals),  x_empty (CW arrivals)
-//   tab[n % TS]  TMA -> producers (gx) and consumers (gy, d, masks)
-// The TMA of frame n + SB is issued by one producer thread once every producer warp has finished
-// frame n (named barrier 1).  Producers start frame n only after all consumers released frame
-// n - XR, so when frame n + SB is issued every consumer has finished frame n - XR - 1 completely:
-// TS >= SB + XR + 2 table stages suffice even though a consumer releases X before it runs the flush
-// of that frame (which still reads d from the table).
+//   box[n % SB]  TMA -> producer       full_box  (tx bytes; also covers tab[n % TS])
+//   X[n % XR]    producer -> consumers x_full   (1 arrival),  x_empty (CW arrivals)
+//   tab[n % TS]  TMA -> producer (gx) and consumers (weights, d, masks)
+// Frame n belongs to producer warp n % kPW (XR = kPW, SB = 2 kPW: the warp's own X buffer and its two
+// box stages).  The warp requests frame n + SB when it has finished frame n, which it started only
+// after all consumers had released frame n - XR, i.e. had finished frame n - XR - 1 completely: the
+// table stage (n + SB) % TS was last used by frame n + SB - TS <= n - XR - 1 for TS >= SB + XR + 1,
+// even though a consumer releases X before it runs the flush of that frame (which still reads d from
+// the table).
 template <class C>
 __global__ void __launch_bounds__(C::NT, 1)
 k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int32_t ntx,
@@ -265,7 +312,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 
     if (tid == 0) {
         for (int s = 0; s < SB; ++s) mbar_init(full_box + 8 * (s), 1);
-        for (int s = 0; s < XR; ++s) { mbar_init(x_full + 8 * (s), kPW); mbar_init(x_empty + 8 * (s), CW); }
+        for (int s = 0; s < XR; ++s) { mbar_init(x_full + 8 * (s), 1); mbar_init(x_empty + 8 * (s), CW); }
         for (int s = 0; s < NB; ++s) mbar_init(f_done + 8 * (s), CW);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -273,83 +320,82 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 
     if (warp >= CW) {
         // =============================================================== producers: TMA + x-pass
+        // Producer warp pw owns the CTA-local frames n = pw, pw + kPW, ...: it requests their boxes (two
+        // stages of its own, so the next box is in flight while it works), runs the whole x-pass of the
+        // frame and hands X[n % XR] = X[pw] to the consumers.  The four warps work on four consecutive
+        // frames at the same time and never synchronise with each other; the per-frame costs (two
+        // mbarrier waits, the table row, the hand-over) are paid once per warp and frame.
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::PREGS));
+        static_assert(XR == kPW && SB == 2 * kPW, "one X buffer and two box stages per producer warp");
         const int32_t pw = warp - CW;
-        const bool issuer = (pw == 0) && (lane == 0);
-        // issue state (issuer thread only): the next frame to request
-        int32_t iss_item = blockIdx.x, iss_t = 0, iss_n = 0, iss_ts = 0, iss_x0 = 0, iss_y = 0, xo_next = 0;
-        const int32_t *iss_ptr = nullptr;
-        auto iss_setup = [&]() {
+        // position of this warp's next frame to REQUEST (iss_*) and to PROCESS (item, t) in the CTA's
+        // sequence of (work item, frame)
+        int32_t iss_item = blockIdx.x, iss_t = pw, iss_k = 0;
+        auto advance = [&](int32_t &it, int32_t &tt) {
+            tt += kPW;
+            while (tt >= T) { tt -= T; it += gridDim.x; }
+        };
+        while (iss_t >= T) { iss_t -= T; iss_item += gridDim.x; }
+        int32_t item = iss_item, t = iss_t;
+        auto iss_one = [&]() {          // lane 0: request frame (iss_item, iss_t) into this warp's stage iss_k & 1
             const int32_t b = iss_item % a.n_batches, tile = a.ty0 * ntx + iss_item / a.n_batches;
-            iss_x0 = (tile % ntx) * kTileW;
-            iss_y = (tile / ntx) * HT - 4;
-            iss_ptr = reinterpret_cast<const int32_t *>(a.stage_tab + (int64_t)b * T * TABW);
-            xo_next = __ldg(iss_ptr);
-        };
-        auto iss_one = [&]() {          // request frame iss_n into box stage iss_n % SB, table stage iss_ts
-            const int32_t sb = iss_n & (SB - 1);
+            const int32_t *row = reinterpret_cast<const int32_t *>(a.stage_tab + ((int64_t)b * T + iss_t) * TABW);
+            const int32_t sb = pw + kPW * (iss_k & 1), n = pw + kPW * iss_k;
             mbar_expect_tx(full_box + 8 * (sb), C::BOX_BYTES + TABW * 4);
-            tma_load_3d(Rbuf + sb * C::RBUF, &map, iss_x0 + xo_next, iss_y, iss_t, full_box + 8 * (sb));
-            bulk_load(Tab + iss_ts * TABW, iss_ptr, TABW * 4, full_box + 8 * (sb));
-            ++iss_n;
-            iss_ts = (iss_ts + 1) & (TS - 1);
-            iss_ptr += TABW;
-            if (++iss_t == T) {
-                iss_t = 0;
-                iss_item += gridDim.x;
-                if (iss_item < n_items) iss_setup();
-            } else {
-                xo_next = __ldg(iss_ptr);
-            }
+            tma_load_3d(Rbuf + sb * C::RBUF, &map, (tile % ntx) * kTileW + __ldg(row), (tile / ntx) * HT - 4, iss_t,
+                        full_box + 8 * (sb));
+            bulk_load(Tab + (n & (TS - 1)) * TABW, row, TABW * 4, full_box + 8 * (sb));
         };
-        if (issuer && iss_item < n_items) {
+        if (lane == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            iss_setup();
-            for (int f = 0; f < SB && iss_item < n_items; ++f) iss_one();
+            for (int f = 0; f < 2 && iss_item < n_items; ++f) {
+                iss_one();
+                ++iss_k;
+                advance(iss_item, iss_t);
+            }
         }
-        // x-pass roles: group g = (block of 8 rows, 4 of the 16 column quads); a quarter-warp takes the
-        // 8 rows of a block at one quad: 32 distinct banks for the 16-byte loads (pitch 76) and for
-        // the 16-byte stores (pitch 68).  Producer warp pw owns quads 4 pw .. 4 pw + 3 of every block.
-        const int32_t row_in = lane & 7, quad = 4 * pw + (lane >> 3);
-        int32_t n = 0;
-        for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+        iss_k = 2;          // (all lanes keep the same counters; only lane 0 issues)
+        {
+            int32_t ii = blockIdx.x, tt = pw;
+            while (tt >= T) { tt -= T; ii += gridDim.x; }
+            advance(ii, tt); advance(ii, tt);
+            iss_item = ii; iss_t = tt;
+        }
+        // x-pass roles: a quarter-warp takes 8 rows at one offset of 8 columns: 32 distinct banks for the
+        // 16-byte loads (pitch 76) and for the 16-byte stores (pitch 68); the warp covers 8 rows x 32 columns
+        // per step (8 outputs per thread from 16 staged values) and walks 2 halves x ceil(rows / 8) row
+        // groups per frame.
+        const int32_t row_in = lane & 7, oct_in = lane >> 3;
+        for (int32_t k = 0; item < n_items; ++k) {
             const int32_t Y0 = (a.ty0 + item / a.n_batches / ntx) * HT - 2;
             // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
             const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
-            for (int32_t t = 0; t < T; ++t) {
-                const int32_t sb = n & (SB - 1), xr = n & (XR - 1);
-                mbar_wait(full_box + 8 * (sb), (n / SB) & 1);
-                if (n >= XR) mbar_wait(x_empty + 8 * (xr), ((n / XR) + 1) & 1);
-                const float *tb = Tab + (n & (TS - 1)) * TABW;
-                const int32_t o = reinterpret_cast<const int32_t *>(tb)[1];
-                const float g0 = tb[4], g1 = tb[5], g2 = tb[6], g3 = tb[7], g4 = tb[8];
-                const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 4 * quad;
-                float *dst = Xbuf + xr * C::XBUF + row_in * kXP + 4 * quad;
-                for (int32_t row = row_in; row < xrows; row += 8, src += 8 * kBoxW, dst += 8 * kXP) {
-                    const float4 *p4 = reinterpret_cast<const float4 *>(src);
-                    const float4 u0 = p4[0], u1 = p4[1], u2 = p4[2];
-                    const float r[12] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w, u2.x, u2.y, u2.z, u2.w};
-                    float4 v;
-#define TNO_TAPS(O)                                                                                        \
-    v.x = fmaf(g4, r[O + 4], fmaf(g3, r[O + 3], fmaf(g2, r[O + 2], fmaf(g1, r[O + 1], g0 * r[O]))));      \
-    v.y = fmaf(g4, r[O + 5], fmaf(g3, r[O + 4], fmaf(g2, r[O + 3], fmaf(g1, r[O + 2], g0 * r[O + 1]))));  \
-    v.z = fmaf(g4, r[O + 6], fmaf(g3, r[O + 5], fmaf(g2, r[O + 4], fmaf(g1, r[O + 3], g0 * r[O + 2]))));  \
-    v.w = fmaf(g4, r[O + 7], fmaf(g3, r[O + 6], fmaf(g2, r[O + 5], fmaf(g1, r[O + 4], g0 * r[O + 3]))));
-                    switch (o) {                       // uniform across the CTA
-                        case 0: TNO_TAPS(0) break;
-                        case 1: TNO_TAPS(1) break;
-                        case 2: TNO_TAPS(2) break;
-                        default: TNO_TAPS(3) break;
-                    }
-#undef TNO_TAPS
-                    *reinterpret_cast<float4 *>(dst) = v;
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(x_full + 8 * (xr));
-                asm volatile("bar.sync 1, %0;" ::"n"(kPW * 32) : "memory");   // all producers are done with box sb
-                if (issuer && iss_item < n_items) iss_one();
-                ++n;
+            const int32_t sb = pw + kPW * (k & 1), n = pw + kPW * k;
+            mbar_wait(full_box + 8 * (sb), (k >> 1) & 1);
+            if (k >= 1) mbar_wait(x_empty + 8 * (pw), (k + 1) & 1);
+            const float *tb = Tab + (n & (TS - 1)) * TABW;
+            const int32_t o = reinterpret_cast<const int32_t *>(tb)[1];
+            float g[5];
+#pragma unroll
+            for (int i = 0; i < 5; ++i) g[i] = tb[4 + i];
+            const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 8 * oct_in;
+            float *dst = Xbuf + pw * C::XBUF + row_in * kXP + 8 * oct_in;
+            const int32_t nfull = xrows >> 3;                       // row groups with all 8 rows
+            const bool tail = row_in < (xrows & 7);                 // this lane's row of the last, partial group
+            switch (o) {                                            // uniform across the CTA
+                case 0: xpass_frame<0>(src, dst, nfull, tail, g); break;
+                case 1: xpass_frame<1>(src, dst, nfull, tail, g); break;
+                case 2: xpass_frame<2>(src, dst, nfull, tail, g); break;
+                default: xpass_frame<3>(src, dst, nfull, tail, g); break;
             }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(x_full + 8 * (pw));
+                // this warp is done with box stage sb: request its frame after next into it
+                if (iss_item < n_items) { iss_k = k + 2; iss_one(); }
+            }
+            advance(iss_item, iss_t);
+            advance(item, t);
         }
     } else {
         // =============================================================== consumers: y-pass + flush
@@ -578,8 +624,8 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
 // (rows per thread, slots per batch, consumer warps, box stages, X buffers): tiles of CW x R positions x 64
 // columns.  A slot costs 4 R accumulator registers (E and O, two columns), the window and its sums and
 // differences 2 (R + 4) + 8 R.
-using V0 = SepCfg<4, 5, 12, 4, 4>;
-using V1 = SepCfg<6, 5, 8, 4, 4>;
+using V0 = SepCfg<4, 5, 12, 8, 4>;
+using V1 = SepCfg<6, 5, 8, 8, 4>;
 
 int32_t sep_num_variants() { return 2; }
 SepVariant sep_variant(int32_t v) { return v == 0 ? SepVariant{V0::NB, V0::HT} : SepVariant{V1::NB, V1::HT}; }
