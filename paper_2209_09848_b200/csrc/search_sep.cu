@@ -113,6 +113,7 @@ constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per
 //   [3] flush mask: bit s set if slot s must be flushed after this frame
 //   [4..8] gx[0..4]
 //   [10] wait mask: bit s set if the previous flush of slot s is at most XR frames back
+//   [12..15], [11] d_2 / sigma_t^2 of slots 0..3 and of slot 4 (one 16-byte load + one word)
 //   [16 + 8s + 0..4] (w[2], s_1, s_2, d_1, d_2) / sigma_t^2 of slot s (zeros if empty)
 //   [16 + 8s + 5] d_{s,t}    [16 + 8s + 6], [.. + 7] planned-order index of the plus / minus member relative
 //                            to the first one of the batch, -1 = absent
@@ -140,6 +141,7 @@ struct SepCfg {
     static_assert((SB & (SB - 1)) == 0 && (XR & (XR - 1)) == 0 && (TS & (TS - 1)) == 0 && TS >= SB + XR + 2,
                   "ring sizes are powers of two");
     static_assert((TABW * 4) % 16 == 0 && (XBUF * 4) % 16 == 0, "16-byte alignment of the sections");
+    static_assert(NB <= 5, "the header holds d_2 of five slots");
 };
 
 // Phase of an entry's periodic flush: a function of its y-motion alone, so that the summation order
@@ -196,6 +198,7 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
         oe[2] = (float)(0.5 * (w[4] + w[0]));
         oe[3] = (float)(0.5 * (w[3] - w[1]));
         oe[4] = (float)(0.5 * (w[4] - w[0]));
+        out[e < 4 ? 12 + e : 11] = oe[4];
         oi[5] = flip ? -tab.shift[ci] : tab.shift[ci];
         oi[6] = slot_q[((int64_t)b * C::NB + e) * 2];
         oi[7] = slot_q[((int64_t)b * C::NB + e) * 2 + 1];
@@ -261,22 +264,19 @@ __device__ __forceinline__ void xpass_step(const XIn &u, float *dst, const float
 template <int O>
 __device__ __forceinline__ void xpass_frame(const float *src, float *dst, int32_t nfull, bool tail,
                                             const float (&g)[5]) {
-    const int32_t nstep = 2 * nfull;
-    XIn u = xpass_load(src);
-    for (int32_t i = 0; i < nstep; ++i) {
-        // step i: row group i >> 1, column half i & 1
-        const float *nsrc = src + ((i & 1) ? 8 * kBoxW - 32 : 32);
-        XIn un = u;
-        if (i + 1 < nstep || tail) un = xpass_load(nsrc);
+    XIn u = xpass_load(src);                    // left half of the current row group
+    for (int32_t i = 0; i < nfull; ++i) {
+        const XIn w = xpass_load(src + 32);     // right half
         xpass_step<O>(u, dst, g);
-        dst += (i & 1) ? 8 * kXP - 32 : 32;
-        src = nsrc;
-        u = un;
+        src += 8 * kBoxW;
+        if (i + 1 < nfull || tail) u = xpass_load(src);
+        xpass_step<O>(w, dst + 32, g);
+        dst += 8 * kXP;
     }
     if (tail) {
-        const XIn u2 = xpass_load(src + 32);
+        const XIn w = xpass_load(src + 32);
         xpass_step<O>(u, dst, g);
-        xpass_step<O>(u2, dst + 32, g);
+        xpass_step<O>(w, dst + 32, g);
     }
 }
 
@@ -403,6 +403,8 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         const int32_t r0 = warp * R;
         int32_t n = 0;
         uint32_t fpar = 0;        // bit s = parity of the number of flushes of slot s so far
+        const float2 *xp0 = reinterpret_cast<const float2 *>(Xbuf + r0 * kXP) + lane;     // this thread's window in X[0]
+        asm volatile("" : "+l"(xp0));      // kept in a register: not recomputed from the thread index every frame
         for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
             // flush coordinates of the item: the members of the batch have planned indices q_first + (the
             // offsets in the table), a member's piece map starts at ebase + offset*H*W (this lane's two
@@ -434,7 +436,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 if (y_active) {
                     // ---------------- y-pass: one register window of X for all slots of the batch, and the
                     // sums and differences of its rows about each of this thread's R positions
-                    const float2 *xp = reinterpret_cast<const float2 *>(Xbuf + xr * C::XBUF + r0 * kXP) + lane;
+                    const float2 *xp = xp0 + xr * (C::XBUF / 2);
                     float2 win[R + 4];
 #pragma unroll
                     for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
@@ -458,31 +460,29 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         _Pragma("unroll") for (int r = 0; r < R; ++r) accO[s][r] = __ffma2_rn(w5, B2[r], accO[s][r]);      \
         _Pragma("unroll") for (int r = 0; r < R; ++r) accE[s][r] = __ffma2_rn(w2, A2[r], accE[s][r]);      \
     }
+                    // d_2 of all slots: one 16-byte load and one word
+                    const float4 d2q = *reinterpret_cast<const float4 *>(th + 12);
+                    const float d2v[5] = {d2q.x, d2q.y, d2q.z, d2q.w, th[11]};
                     if (nfill == NB) {
                         // full batch: straight-line code, the weights of slot s + 1 are loaded
                         // before the FFMAs of slot s (the empty asm keeps ptxas from hoisting more
                         // loads than the register budget holds)
                         float4 wa = *reinterpret_cast<const float4 *>(tb);
-                        float w4 = tb[4];
 #pragma unroll
                         for (int s = 0; s < NB; ++s) {
                             float4 wan = wa;
-                            float w4n = w4;
-                            if (s + 1 < NB) {
-                                wan = *reinterpret_cast<const float4 *>(tb + 8 * (s + 1));
-                                w4n = tb[8 * (s + 1) + 4];
-                            }
+                            if (s + 1 < NB) wan = *reinterpret_cast<const float4 *>(tb + 8 * (s + 1));
+                            const float w4 = d2v[s];
                             TNO_FMAS(s)
                             asm volatile("" ::: "memory");
                             wa = wan;
-                            w4 = w4n;
                         }
                     } else {
 #pragma unroll
                         for (int s = 0; s < NB; ++s)
                             if (s < nfill) {
                                 const float4 wa = *reinterpret_cast<const float4 *>(tb + 8 * s);
-                                const float w4 = tb[8 * s + 4];
+                                const float w4 = d2v[s];
                                 TNO_FMAS(s)
                             }
                     }
