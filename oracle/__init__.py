@@ -55,6 +55,8 @@ _lib.tno_oracle_inject_mode.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctype
                                         _f32p, _i32p, _i32p, _f32p, ctypes.c_int, ctypes.c_float, ctypes.c_float]
 _lib.tno_oracle_set_prf_table.restype = ctypes.c_int
 _lib.tno_oracle_set_prf_table.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+_lib.tno_oracle_set_prf_table2d.restype = ctypes.c_int
+_lib.tno_oracle_set_prf_table2d.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_int]
 
 
 def _opt(a, shape):
@@ -77,14 +79,21 @@ _f64c = ctypes.POINTER(ctypes.c_double)
 
 
 def _mode(shift_stack, filter, prf_table) -> int:
-    """Filter mode of tap1 in tno_oracle.c (0 point-sampled Gaussian, 1 shift-stack, 2 pixel-integrated
-    Gaussian, 3 tabulated); mode 3 installs `prf_table` ([n_phase, 5] fractions) first."""
+    """Filter mode of tap1 / tap2 in tno_oracle.c (0 point-sampled Gaussian, 1 shift-stack, 2 pixel-integrated
+    Gaussian, 3 tabulated separable, 4 tabulated non-separable); mode 3 installs `prf_table` ([n_phase, 5]
+    fractions) first, mode 4 the 2-D table ([n_phase_y, n_phase_x, 5, 5])."""
     mode = int(filter) if filter else int(bool(shift_stack))
-    assert mode in (0, 1, 2, 3)
+    assert mode in (0, 1, 2, 3, 4)
     if mode == 3:
         tab = np.ascontiguousarray(prf_table, dtype=np.float64)
         assert tab.ndim == 2 and tab.shape[1] == 5 and tab.shape[0] >= 1
         rc = _lib.tno_oracle_set_prf_table(tab.ctypes.data_as(_f64c), int(tab.shape[0]))
+        assert rc == 0
+    if mode == 4:
+        # non-separable tabulated PRF: [n_phase_y, n_phase_x, 5, 5], entry [ry, rx, j + 2, i + 2]
+        tab = np.ascontiguousarray(prf_table, dtype=np.float64)
+        assert tab.ndim == 4 and tab.shape[2:] == (5, 5) and tab.shape[0] >= 1 and tab.shape[1] >= 1
+        rc = _lib.tno_oracle_set_prf_table2d(tab.ctypes.data_as(_f64c), int(tab.shape[0]), int(tab.shape[1]))
         assert rc == 0
     return mode
 

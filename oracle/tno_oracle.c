@@ -108,6 +108,41 @@ static inline double tap1(int mode, int i, double ph, double s) {
     }
     return exp(-(u * u) / (2.0 * s * s));
 }
+/*   mode 4  a tabulated NON-separable PRF (the real TESS PRF, "50 % of the flux in the peak pixel
+ *           and 90 % in 2 x 2", is a 2-D table per 2-D sub-pixel phase, not an outer product): the table installed
+ *           with tno_oracle_set_prf_table2d is [n_phase_y][n_phase_x][5][5]; a source at phases (phx, phy) takes
+ *           the 5 x 5 block of row floor((phy + 1/2) n_phase_y), column floor((phx + 1/2) n_phase_x) (clamped),
+ *           whose entry [j + 2][i + 2] is the response of the pixel at offset (i, j) from the rounded position.
+ *           No interpolation.  Second piece of global state of this file. */
+static double *g_prf_table2d = NULL;
+static int g_prf_phases_y = 0, g_prf_phases_x = 0;
+int tno_oracle_set_prf_table2d(const double *table, int n_phase_y, int n_phase_x) {
+    free(g_prf_table2d);
+    g_prf_table2d = NULL;
+    g_prf_phases_y = g_prf_phases_x = 0;
+    if (!table || n_phase_y <= 0 || n_phase_x <= 0) return 0;
+    const size_t n = (size_t)25 * (size_t)n_phase_y * (size_t)n_phase_x;
+    g_prf_table2d = (double *)malloc(sizeof(double) * n);
+    if (!g_prf_table2d) return -2;
+    memcpy(g_prf_table2d, table, sizeof(double) * n);
+    g_prf_phases_y = n_phase_y;
+    g_prf_phases_x = n_phase_x;
+    return 0;
+}
+static inline int phase_row(double ph, int n) {
+    int row = (int)floor((ph + 0.5) * (double)n);
+    if (row < 0) row = 0;
+    if (row > n - 1) row = n - 1;
+    return row;
+}
+/* the filter value at tap (i, j) for any mode: per-axis products for the separable modes 1-3 */
+static inline double tap2(int mode, int i, int j, double phx, double phy, double s) {
+    if (mode == 4) {
+        const int ry = phase_row(phy, g_prf_phases_y), rx = phase_row(phx, g_prf_phases_x);
+        return g_prf_table2d[((size_t)(ry * g_prf_phases_x + rx) * 5 + (size_t)(j + 2)) * 5 + (size_t)(i + 2)];
+    }
+    return tap1(mode, i, phx, s) * tap1(mode, j, phy, s);
+}
 static inline double frame_dt(const float *times, int t, double t0) {
     return (times ? (double)times[t] : (double)t) - t0;
 }
@@ -153,7 +188,7 @@ int tno_oracle_point_ex(const float *frames, int T, int H, int W,
                 if (px < 0 || px >= W || py < 0 || py >= H) continue;
                 if (px < wx0 || px >= wx0 + ww || py < wy0 || py >= wy0 + wh) return -1;
                 const double ux = (double)i - phx, uy = (double)j - phy;
-                const double g = mode != 0 ? tap1(mode, i, phx, s) * tap1(mode, j, phy, s)
+                const double g = mode != 0 ? tap2(mode, i, j, phx, phy, s)
                                            : exp(-(ux * ux + uy * uy) / (2.0 * s * s));
                 const size_t idx = ((size_t)t * wh + (size_t)(py - wy0)) * ww + (size_t)(px - wx0);
                 const double R = frames[idx];
@@ -193,7 +228,8 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
     if (rw <= 0 || rh <= 0 || K <= 0 || T <= 0) return -2;
     int *SX = (int *)malloc(sizeof(int) * (size_t)T * 2);
     double *G = (double *)malloc(sizeof(double) * (size_t)T * 11);
-    if (!SX || !G) { free(SX); free(G); return -3; }
+    double *G2 = mode == 4 ? (double *)malloc(sizeof(double) * (size_t)T * 25) : NULL;   /* mode 4: [t][j][i] */
+    if (!SX || !G || (mode == 4 && !G2)) { free(SX); free(G); free(G2); return -3; }
     int err = 0;
     for (int k = 0; k < K; ++k) {
         const double vx = traj[4 * k + 0], vy = traj[4 * k + 1];
@@ -205,9 +241,12 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
             split(disp(vy, ay, dt) + jit(jitter, t, 1), &sy, &phy);
             SX[2 * t] = sx; SX[2 * t + 1] = sy;
             for (int i = -2; i <= 2; ++i) {
-                G[11 * t + (i + 2)] = tap1(mode, i, phx, s);
-                G[11 * t + 5 + (i + 2)] = tap1(mode, i, phy, s);
+                G[11 * t + (i + 2)] = mode == 4 ? 0.0 : tap1(mode, i, phx, s);
+                G[11 * t + 5 + (i + 2)] = mode == 4 ? 0.0 : tap1(mode, i, phy, s);
             }
+            if (mode == 4)
+                for (int j = -2; j <= 2; ++j)
+                    for (int i = -2; i <= 2; ++i) G2[25 * t + 5 * (j + 2) + (i + 2)] = tap2(4, i, j, phx, phy, s);
             const double sig = sigma_t[t];
             G[11 * t + 10] = 1.0 / (sig * sig);
         }
@@ -229,7 +268,7 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
                     const float *row = frames + ((size_t)t * wh + (size_t)(py - wy0)) * ww;
                     const float *vrow = valid ? valid + ((size_t)t * wh + (size_t)(py - wy0)) * ww : NULL;
                     for (int i = -2; i <= 2; ++i) {
-                        const double g = gx[i + 2] * gy[j + 2];
+                        const double g = G2 ? G2[25 * t + 5 * (j + 2) + (i + 2)] : gx[i + 2] * gy[j + 2];
                         const double wN = g * q, wD = g * g * q;
                         int xa = x_lo, xb = x_hi;           /* start pixels with px inside the frame */
                         if (xa + sx + i < 0) xa = -(sx + i);
@@ -255,7 +294,7 @@ int tno_oracle_map_ex(const float *frames, int T, int H, int W,
         free(Nk); free(Dk);
         if (err) break;
     }
-    free(SX); free(G);
+    free(SX); free(G); free(G2);
     return err;
 }
 
@@ -303,7 +342,7 @@ int tno_oracle_inject_ex(float *frames, int T, int H, int W, const float *times,
     return 0;
 }
 
-/* The same with the per-axis filter of `mode` (tap1): the source as modes 1-3 see it. */
+/* The same with the filter of `mode` (tap2): the source as modes 1-4 see it. */
 int tno_oracle_inject_mode(float *frames, int T, int H, int W, const float *times, const float *jitter, int mode,
                          const float *traj, const int *xs, const int *ys, const float *amp, int n,
                          float prf_sigma_f, float t0_f)
@@ -322,7 +361,7 @@ int tno_oracle_inject_mode(float *frames, int T, int H, int W, const float *time
                 for (int i = -2; i <= 2; ++i) {
                     const int px = xs[m] + sx + i, py = ys[m] + sy + j;
                     if (px < 0 || px >= W || py < 0 || py >= H) continue;
-                    const double g = tap1(mode, i, phx, s) * tap1(mode, j, phy, s);
+                    const double g = tap2(mode, i, j, phx, phy, s);
                     float *p = frames + ((size_t)t * H + (size_t)py) * W + (size_t)px;
                     *p = (float)((double)*p + A * g);
                 }

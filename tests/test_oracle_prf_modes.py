@@ -95,3 +95,91 @@ def test_map_and_point_agree_and_injected_source_is_recovered_in_every_mode():
         oracle.inject(clean, trajs[:1], [11], [10], [37.5], 0.9, 5.0, filter=mode, prf_table=table)
         _, N, D = oracle.point(clean, sigma_t, trajs[0], 0.9, 5.0, 11, 10, filter=mode, prf_table=table)
         assert abs(N / D - 37.5) < 1e-4
+
+
+# ---- filter 4: tabulated NON-separable PRF ------------------------------------------
+def _table2d(rng, ny, nx):
+    """A random non-negative [ny, nx, 5, 5] table that is NOT an outer product (rank > 1 blocks)."""
+    tab = rng.uniform(0.0, 1.0, (ny, nx, 5, 5))
+    tab[..., 2, 2] += 2.0
+    assert np.linalg.matrix_rank(tab[0, 0]) > 1
+    return tab
+
+
+def test_nonseparable_table_reads_the_block_of_both_phases():
+    """An explicit 25-tap lookup: the frame's filter is the 5 x 5 block at (row of the y-phase, column of the
+    x-phase), entry [j + 2][i + 2] at pixel offset (i, j) -- transposing the block, swapping the phase axes or
+    mirroring a tap index fails (the table is random, with ny != nx)."""
+    rng = np.random.default_rng(7)
+    ny, nx = 6, 4
+    tab = _table2d(rng, ny, nx)
+    for phx, phy in ((-0.5, 0.49), (0.0, 0.124), (0.126, -0.3), (0.3, 0.3)):
+        g = _one_frame_taps(4, 1.0, phx, phy, prf_table=tab)
+        rx = min(nx - 1, int(np.floor((float(np.float32(phx)) + 0.5) * nx)))
+        ry = min(ny - 1, int(np.floor((float(np.float32(phy)) + 0.5) * ny)))
+        assert np.array_equal(g[2:7, 2:7], tab[ry, rx])           # g[row = y offset + 2, column = x offset + 2]
+        mask = np.ones_like(g, bool)
+        mask[2:7, 2:7] = False
+        assert np.all(g[mask] == 0)
+
+
+def test_nonseparable_table_of_outer_products_is_the_separable_mode():
+    """Reduction to mode 3: with table2d[ry, rx] = outer(tab[ry], tab[rx]) maps, N and D are those of the separable
+    tabulated filter (same products, so equal to rounding of one multiplication)."""
+    rng = np.random.default_rng(5)
+    n_phase = 8
+    tab = rng.uniform(0.1, 1.0, (n_phase, 5))
+    tab2 = np.einsum("yj,xi->yxji", tab, tab)
+    T, H, W = 9, 14, 17
+    frames = rng.standard_normal((T, H, W)).astype(np.float32)
+    sigma_t = rng.uniform(0.8, 1.3, T).astype(np.float32)
+    trajs = np.array([[0.31, -0.22, 0.004, 0.002], [-0.4, 0.15, 0.0, -0.003], [0.5, 0.25, 0, 0]], np.float32)
+    m3, N3, D3 = oracle.snr_map(frames, sigma_t, trajs, 1.0, 4.0, filter=3, prf_table=tab, return_ND=True)
+    m4, N4, D4 = oracle.snr_map(frames, sigma_t, trajs, 1.0, 4.0, filter=4, prf_table=tab2, return_ND=True)
+    assert np.allclose(N4, N3, rtol=1e-13, atol=1e-13) and np.allclose(D4, D3, rtol=1e-13, atol=0)
+    assert np.allclose(m4, m3, rtol=1e-12, atol=1e-12)
+
+
+def test_nonseparable_map_point_brute_force_and_injection():
+    """snr_map (hoisted) equals point (literal) in mode 4; both equal a Python evaluation of the definition written
+    out here (exact-rational displacement, explicit table lookup, off-frame taps dropped from N and D); a noiseless
+    source injected with the same table gives N / D = its amplitude."""
+    from fractions import Fraction
+    import math
+    rng = np.random.default_rng(13)
+    ny, nx = 5, 7
+    tab = _table2d(rng, ny, nx)
+    T, H, W = 6, 9, 11
+    frames = rng.standard_normal((T, H, W)).astype(np.float32)
+    sigma_t = rng.uniform(0.8, 1.3, T).astype(np.float32)
+    trajs = np.array([[0.31, -0.22, 0.01, 0.02], [-0.9, 0.55, 0.0, -0.03]], np.float32)
+    t0 = 2.0
+    m = oracle.snr_map(frames, sigma_t, trajs, 1.0, t0, filter=4, prf_table=tab)
+
+    def brute(k, x, y):
+        N = D = 0.0
+        for t in range(T):
+            dt = Fraction(t) - Fraction(t0)
+            d = [Fraction(float(trajs[k, a])) * dt + Fraction(float(trajs[k, a + 2])) * dt * dt for a in (0, 1)]
+            s = [math.floor(v + Fraction(1, 2)) for v in d]
+            ph = [float(v - sv) for v, sv in zip(d, s)]
+            rx = min(nx - 1, max(0, math.floor((ph[0] + 0.5) * nx)))
+            ry = min(ny - 1, max(0, math.floor((ph[1] + 0.5) * ny)))
+            q = 1.0 / float(sigma_t[t]) ** 2
+            for j in range(-2, 3):
+                for i in range(-2, 3):
+                    px, py = x + s[0] + i, y + s[1] + j
+                    if 0 <= px < W and 0 <= py < H:
+                        g = tab[ry, rx, j + 2, i + 2]
+                        N += g * float(frames[t, py, px]) * q
+                        D += g * g * q
+        return N / math.sqrt(D) if D > 0 else 0.0
+
+    for k, x, y in ((0, 3, 4), (1, 7, 2), (0, 10, 8), (1, 0, 0), (0, 0, 8)):
+        s, _, _ = oracle.point(frames, sigma_t, trajs[k], 1.0, t0, x, y, filter=4, prf_table=tab)
+        assert abs(m[k, y, x] - s) < 1e-11
+        assert abs(s - brute(k, x, y)) < 1e-11
+    clean = np.zeros((T, H, W), np.float32)
+    oracle.inject(clean, trajs[:1], [5], [4], [21.5], 1.0, t0, filter=4, prf_table=tab)
+    _, N, D = oracle.point(clean, sigma_t, trajs[0], 1.0, t0, 5, 4, filter=4, prf_table=tab)
+    assert abs(N / D - 21.5) < 1e-5
