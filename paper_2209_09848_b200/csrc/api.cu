@@ -221,7 +221,6 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
     ctx->cfg = *cfg;
     ctx->stream = reinterpret_cast<cudaStream_t>(cfg->stream);
     ctx->n_sm = prop.multiProcessorCount;
-    if (const char *ev = getenv("TNO_MF_SEP_VARIANT")) ctx->sep_variant = atoi(ev) ? 1 : 0;   // EXPERIMENT ONLY
     cudaDriverEntryPointQueryResult qres;
     e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_fn, cudaEnableDefault, &qres);
     if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !ctx->encode_fn) {

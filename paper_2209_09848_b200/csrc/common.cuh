@@ -3,6 +3,23 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+// Debug build (nvcc -DTNO_DEBUG_CHECKS, see profiles/r2_sanitizers.md): every shared-memory index, piece address
+// and ring invariant the kernels rely on is checked on the device; a violation prints its place and traps, which
+// the next CUDA call of the host reports as an error.  Compiled out otherwise.
+#ifdef TNO_DEBUG_CHECKS
+#include <cstdio>
+#define TNO_CHECK(cond)                                                                                   \
+    do {                                                                                                  \
+        if (!(cond)) {                                                                                    \
+            printf("TNO_CHECK failed: %s  at %s:%d (block %d thread %d)\n", #cond, __FILE__, __LINE__,    \
+                   (int)blockIdx.x, (int)threadIdx.x);                                                    \
+            __trap();                                                                                     \
+        }                                                                                                 \
+    } while (0)
+#else
+#define TNO_CHECK(cond) do { } while (0)
+#endif
+
 namespace tno {
 
 // ---- axis classes -----------------------------------------------------------------------------

