@@ -83,12 +83,13 @@ typedef struct {
                                 2 = pixel-integrated Gaussian PRF: the tap of pixel i is the flux fraction a source
                                 at sub-pixel phase ph puts into it, Phi((i-ph+1/2)/prf_sigma) - Phi((i-ph-1/2)/prf_sigma)
                                 per axis (PAPER.md:L41 describes the PRF by such fractions: ~50 % in the peak pixel);
-                                3 = tabulated separable PRF, see tno_mf_set_prf_table; prf_sigma is ignored.
-                                In modes 2 and 3 tno_mf_inject renders sources with the same taps. */
+                                3 = tabulated separable PRF, see tno_mf_set_prf_table; prf_sigma is ignored;
+                                4 = tabulated non-separable PRF, see tno_mf_set_prf_table2d; prf_sigma is ignored.
+                                In modes 2, 3 and 4 tno_mf_inject renders sources with the same taps. */
 } tno_mf_config;
 
 /* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
- * workspace_limit_mb < 0, filter not 0 .. 3), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
+ * workspace_limit_mb < 0, filter not 0 .. 4), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
 int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
 
 /* The search (formula above).
@@ -196,6 +197,18 @@ int tno_mf_search_host_max(tno_mf_ctx *ctx,
  * n_phase = 0 removes it.  A context with filter 3 and no table fails its searches with EINVAL.
  * Errors: EINVAL, ENOMEM, ECUDA. */
 int tno_mf_set_prf_table(tno_mf_ctx *ctx, const float *table, int32_t n_phase);
+
+/* Tabulated NON-separable PRF for filter 4 (the TESS PRF, "approximately 50 % of
+ * the flux in the peak pixel and 90 % in 2 x 2", is tabulated per 2-D sub-pixel phase and is not an outer product).
+ * `table` is HOST float32 [n_phase_y][n_phase_x][5][5]: block (ry, rx) holds, at [j + 2][i + 2], the response of the
+ * pixel at offset (i, j) from the rounded position for a source whose sub-pixel phases (phx, phy) fall into column
+ * rx = floor((phx + 1/2) n_phase_x) and row ry = floor((phy + 1/2) n_phase_y) (clamped; no interpolation).
+ * Values finite and >= 0; phases 1 .. 4096; both 0 removes the table.  The table is copied.
+ * Searches of a context with filter 4 run the 25-tap formulation (one thread per trajectory and pixel, N and D
+ * accumulated together: D is not separable either), at any H, W and alignment, with or without validity weights;
+ * tno_mf_inject renders with the same blocks; tno_mf_flux does not apply (EINVAL).  A context with filter 4 and no
+ * table fails its searches with EINVAL.  Errors: EINVAL, ENOMEM, ECUDA. */
+int tno_mf_set_prf_table2d(tno_mf_ctx *ctx, const float *table, int32_t n_phase_y, int32_t n_phase_x);
 
 /* Signal injection ("signal injection corresponds to adding a filter times a flux
  * to the raw data"): for each source m in order and every frame t,

@@ -82,6 +82,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_peaks.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     lib.tno_mf_set_prf_table.restype = i32
     lib.tno_mf_set_prf_table.argtypes = [vp, vp, i32]
+    lib.tno_mf_set_prf_table2d.restype = i32
+    lib.tno_mf_set_prf_table2d.argtypes = [vp, vp, i32, i32]
     lib.tno_mf_plan.restype = ctypes.c_int
     lib.tno_mf_plan.argtypes = [vp, i32, i32, f32, i32, i32, vp, vp]
     lib.tno_mf_plan_slots.restype = ctypes.c_int
@@ -414,6 +416,17 @@ def tno_mf_set_prf_table(ctx, table) -> None:
     if tab.ndim != 2 or tab.shape[1] != 5:
         raise ValueError("prf table must have shape [n_phase, 5]")
     _check(_lib.tno_mf_set_prf_table(ctx, tab.ctypes.data, tab.shape[0]), ctx)
+
+
+def tno_mf_set_prf_table2d(ctx, table) -> None:
+    """table: [n_phase_y, n_phase_x, 5, 5] responses (host array) for filter 4; None removes it."""
+    if table is None or len(table) == 0:
+        _check(_lib.tno_mf_set_prf_table2d(ctx, None, 0, 0), ctx)
+        return
+    tab = np.ascontiguousarray(table, dtype=np.float32)
+    if tab.ndim != 4 or tab.shape[2:] != (5, 5):
+        raise ValueError("prf table must have shape [n_phase_y, n_phase_x, 5, 5]")
+    _check(_lib.tno_mf_set_prf_table2d(ctx, tab.ctypes.data, tab.shape[0], tab.shape[1]), ctx)
 
 
 def tno_mf_plan(trajectories, T: int, t0: float, max_entries: int, max_spread: int

@@ -42,8 +42,9 @@ struct tno_mf_ctx {
     float *down_host = nullptr;       // host maps of tno_mf_search_host (NULL: no maps wanted)
     const float *down_dev = nullptr;
     int32_t down_rows = 0, down_K = 0;   // rows [0, down_rows) of every map are on their way to the host
-    DevBuf stack, stack2, hmaps, htopk, hmax, bgq, prf_tab, maxkeys, scat;
+    DevBuf stack, stack2, hmaps, htopk, hmax, bgq, prf_tab, prf_tab2, maxkeys, scat;
     int32_t prf_phases = 0;          // rows of prf_tab (tno_mf_set_prf_table), 0 = none
+    int32_t prf2_py = 0, prf2_px = 0;   // phases of prf_tab2 (tno_mf_set_prf_table2d), 0 = none
     // geometry and tables of the last successful search (for tno_mf_flux)
     int32_t s_traj = 0, s_H = 0, s_W = 0;
     const TrajInfo *s_ti = nullptr;
@@ -198,8 +199,8 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
     if (std::isnan(cfg->snr_threshold))
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
-    if (cfg->filter < 0 || cfg->filter > 3 || cfg->workspace_limit_mb < 0)
-        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 .. 3 and workspace_limit_mb >= 0");
+    if (cfg->filter < 0 || cfg->filter > 4 || cfg->workspace_limit_mb < 0)
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 .. 4 and workspace_limit_mb >= 0");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess || n_dev == 0) {
@@ -261,7 +262,7 @@ int tno_mf_destroy(tno_mf_ctx *ctx) {
     DevBuf *bufs[] = {&ctx->meta, &ctx->shift, &ctx->g, &ctx->gd, &ctx->ab, &ctx->rsd, &ctx->stage_tab,
                       &ctx->pieces, &ctx->keys, &ctx->counts, &ctx->tmp_maps, &ctx->src, &ctx->sat, &ctx->ztmp,
                       &ctx->stack, &ctx->stack2, &ctx->hmaps, &ctx->htopk, &ctx->hmax, &ctx->bgq, &ctx->prf_tab,
-                      &ctx->maxkeys, &ctx->scat};
+                      &ctx->prf_tab2, &ctx->maxkeys, &ctx->scat};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -477,6 +478,29 @@ int tno_mf_set_prf_table(tno_mf_ctx *ctx, const float *table, int32_t n_phase) {
     return TNO_MF_OK;
 }
 
+int tno_mf_set_prf_table2d(tno_mf_ctx *ctx, const float *table, int32_t n_phase_y, int32_t n_phase_x) {
+    if (!ctx) return TNO_MF_EINVAL;
+    if (n_phase_y < 0 || n_phase_x < 0 || n_phase_y > 4096 || n_phase_x > 4096 || (n_phase_y == 0) != (n_phase_x == 0) ||
+        (n_phase_y > 0 && !table))
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_set_prf_table2d: phases must be in [0, 4096], both zero or both "
+                    "positive, and table non-NULL");
+    const int64_t n = (int64_t)n_phase_y * n_phase_x * 25;
+    for (int64_t i = 0; i < n; ++i)
+        if (!finite_f(table[i]) || table[i] < 0.f)
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_set_prf_table2d: table[%lld] is negative or not finite", (long long)i);
+    CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
+    ctx->prf2_py = ctx->prf2_px = 0;
+    if (n == 0) return TNO_MF_OK;
+    int rc = reserve(ctx, ctx->prf_tab2, (size_t)n * sizeof(float));
+    if (rc) return rc;
+    // the caller's buffer may go away after the call
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->prf_tab2.p, table, (size_t)n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->prf2_py = n_phase_y;
+    ctx->prf2_px = n_phase_x;
+    return TNO_MF_OK;
+}
+
 int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W,
                   const tno_mf_source *sources, int32_t n_sources, float prf_sigma, float t0) {
     if (!ctx) return TNO_MF_EINVAL;
@@ -486,6 +510,8 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: prf_sigma must be finite and > 0, t0 finite");
     if (ctx->cfg.filter == 3 && ctx->prf_phases == 0)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: filter 3 needs a table (tno_mf_set_prf_table)");
+    if (ctx->cfg.filter == 4 && ctx->prf2_py == 0)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: filter 4 needs a table (tno_mf_set_prf_table2d)");
     if (n_sources == 0) return TNO_MF_OK;
     std::vector<SourceDev> host(n_sources);
     for (int32_t m = 0; m < n_sources; ++m) {
@@ -501,8 +527,9 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
     CU_TRY(ctx, cudaMemcpyAsync(ctx->src.p, host.data(), host.size() * sizeof(SourceDev),
                                 cudaMemcpyHostToDevice, ctx->stream));
     launch_inject(ctx->stream, frames, T, H, W, static_cast<const SourceDev *>(ctx->src.p), n_sources,
-                  (double)prf_sigma, (double)t0, ctx->cfg.filter, static_cast<const float *>(ctx->prf_tab.p),
-                  ctx->prf_phases);
+                  (double)prf_sigma, (double)t0, ctx->cfg.filter,
+                  static_cast<const float *>(ctx->cfg.filter == 4 ? ctx->prf_tab2.p : ctx->prf_tab.p),
+                  ctx->cfg.filter == 4 ? (ctx->prf2_py << 16 | ctx->prf2_px) : ctx->prf_phases);
     CU_TRY(ctx, cudaGetLastError());
     return TNO_MF_OK;
 }
@@ -724,6 +751,9 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: prf_sigma must be finite and > 0");
     if (ctx->cfg.filter == 3 && ctx->prf_phases == 0)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: filter 3 needs a table (tno_mf_set_prf_table)");
+    if (ctx->cfg.filter == 4 && ctx->prf2_py == 0)
+        return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: filter 4 needs a table (tno_mf_set_prf_table2d)");
+    const bool nonsep = ctx->cfg.filter == 4;      // 25-tap formulation of the generic kernel only
     if (!finite_f(t0)) return fail(ctx, TNO_MF_EINVAL, "tno_mf_search: t0 must be finite");
     const bool want_topk = out_topk != nullptr && ctx->cfg.topk > 0;
     if (!out_snr && !want_topk && !out_max)
@@ -755,7 +785,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
 
     // The separable kernel needs TMA-compatible frames (W % 4 == 0, 16-byte aligned) and a piece
     // count (1 + ceil(y-shift range / tile height)) that stays small.
-    bool use_sep = !ctx->cfg.force_generic && (W % 4 == 0) &&
+    bool use_sep = !ctx->cfg.force_generic && !nonsep && (W % 4 == 0) &&
                    ((reinterpret_cast<uintptr_t>(frames) & 15u) == 0) &&
                    ((reinterpret_cast<uintptr_t>(valid) & 15u) == 0) && W >= 4;
     int32_t variant = -1, n_pieces = 1;
@@ -920,7 +950,8 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
                         frame_times ? reinterpret_cast<const float *>(meta + o_tm) : nullptr,
                         jitter_xy ? reinterpret_cast<const float *>(meta + o_jt) : nullptr,
                         n_cls, n_x, T, (double)t0, (double)prf_sigma, ctx->cfg.filter,
-                        static_cast<const float *>(ctx->prf_tab.p), ctx->prf_phases, static_cast<int32_t *>(ctx->shift.p),
+                        static_cast<const float *>(ctx->prf_tab.p),
+                        nonsep ? (ctx->prf2_py << 16 | ctx->prf2_px) : ctx->prf_phases, static_cast<int32_t *>(ctx->shift.p),
                         static_cast<float *>(ctx->g.p), static_cast<double *>(ctx->gd.p));
     launch_border_tables(st, tab.shift, tab.gd, tab.qd, reinterpret_cast<const AxisBorder *>(meta + o_bd), d_off,
                          n_cls, n_x, max_n, T, W, H, static_cast<double *>(ctx->ab.p));
@@ -1050,7 +1081,11 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         for (int32_t k0 = 0; k0 < n_traj; k0 += chunk) {
             const int32_t kc = std::min(chunk, n_traj - k0);
             float *dst = out_snr ? out_snr + (int64_t)k0 * map_px : maps;
-            launch_search_generic(st, frames, valid, T, H, W, tab, d_ti, d_rsd, k0, kc, dst);
+            if (nonsep)
+                launch_search_generic25(st, frames, valid, T, H, W, tab, d_ti, static_cast<const float *>(ctx->prf_tab2.p),
+                                        ctx->prf2_px, k0, kc, dst);
+            else
+                launch_search_generic(st, frames, valid, T, H, W, tab, d_ti, d_rsd, k0, kc, dst);
             ctx->last_launches += 1;
             if (want_topk) {
                 launch_collect_from_map(st, dst, H, W, k0, kc, slots);
@@ -1075,7 +1110,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         CU_TRY(ctx, cudaGetLastError());
     }
     ctx->s_traj = n_traj; ctx->s_H = H; ctx->s_W = W;
-    ctx->s_ti = valid ? nullptr : d_ti;                // tno_mf_flux needs the analytic D tables
+    ctx->s_ti = (valid || nonsep) ? nullptr : d_ti;    // tno_mf_flux needs the analytic (separable) D tables
     return TNO_MF_OK;
 }
 

@@ -33,11 +33,21 @@ __global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32
                 const int32_t px = s.x + sx + i;
                 if (px < 0 || px >= W) continue;
                 const double ux = (double)i - phx, uy = (double)j - phy;
-                // filters 2 and 3 render the source with their own (separable) PRF; 0 and 1 with the
-                // point-sampled Gaussian (shift-stack is a way to search, not a PRF)
-                const double g = filter >= 2 ? prf_tap(filter, i + 2, phx, prf_sigma, prf_tab, n_phase) *
-                                                   prf_tap(filter, j + 2, phy, prf_sigma, prf_tab, n_phase)
-                                             : exp(-(ux * ux + uy * uy) * inv);
+                // filters 2, 3 and 4 render the source with their own PRF; 0 and 1 with the point-sampled
+                // Gaussian (shift-stack is a way to search, not a PRF)
+                double g;
+                if (filter == 4) {
+                    // non-separable table [n_py][n_px][5][5], n_phase = n_py << 16 | n_px
+                    const int32_t npx = n_phase & 0xffff, npy = n_phase >> 16;
+                    int32_t rx = (int32_t)floor((phx + 0.5) * (double)npx), ry = (int32_t)floor((phy + 0.5) * (double)npy);
+                    rx = rx < 0 ? 0 : (rx > npx - 1 ? npx - 1 : rx);
+                    ry = ry < 0 ? 0 : (ry > npy - 1 ? npy - 1 : ry);
+                    g = (double)prf_tab[((int64_t)ry * npx + rx) * 25 + 5 * (j + 2) + (i + 2)];
+                } else {
+                    g = filter >= 2 ? prf_tap(filter, i + 2, phx, prf_sigma, prf_tab, n_phase) *
+                                          prf_tap(filter, j + 2, phy, prf_sigma, prf_tab, n_phase)
+                                    : exp(-(ux * ux + uy * uy) * inv);
+                }
                 float *p = f + (int64_t)py * W + px;
                 *p = (float)((double)*p + (double)s.amp * g);
             }

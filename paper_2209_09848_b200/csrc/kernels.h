@@ -26,6 +26,12 @@ void launch_search_generic(cudaStream_t st, const float *frames, const float *va
                            const ClassTables &tab, const TrajInfo *traj, const float *rsd,
                            int32_t k_first, int32_t k_count, float *out_snr /* [k_count][H][W] */);
 
+// filter 4: the 25 taps of (trajectory, frame) from the non-separable table tab2 [n_py][n_px][5][5]; tab.gd holds
+// the phase rows / columns (tables.cu); N and D are accumulated together
+void launch_search_generic25(cudaStream_t st, const float *frames, const float *valid, int32_t T, int32_t H, int32_t W,
+                             const ClassTables &tab, const TrajInfo *traj, const float *tab2, int32_t n_px,
+                             int32_t k_first, int32_t k_count, float *out_snr);
+
 // ---- topk.cu ----
 constexpr int32_t kCollectTile = 64;        // k_collect_from_map tiles are 64 x 64 pixels
 constexpr int32_t kMaxTopk = 1024;

@@ -33,9 +33,18 @@ __global__ void k_class_tables(const float *__restrict__ cls_v, const float *__r
         const double u = (double)(i - 2) - ph;
         // filter 0: the expression the first version of this kernel had (bit-compatible tables);
         // 1 shift-stack, 2 pixel-integrated Gaussian, 3 tabulated: prf_tap (common.cuh)
-        const double w = filter == 0 ? exp(-(u * u) * inv) : prf_tap(filter, i, ph, prf_sigma, prf_tab, n_phase);
+        const double w = filter == 0 ? exp(-(u * u) * inv)
+                       : filter == 4 ? 0.0 : prf_tap(filter, i, ph, prf_sigma, prf_tab, n_phase);
         g[id * 5 + i] = (float)w;
         gd[id * 5 + i] = w;
+    }
+    if (filter == 4) {
+        // non-separable tabulated PRF: the class contributes the row (y) or column (x) of its phase in the 2-D
+        // table; n_phase packs (n_phase_y << 16 | n_phase_x).  The 25 taps are looked up per trajectory and frame.
+        const int32_t np = c < n_x ? (n_phase & 0xffff) : (n_phase >> 16);
+        int32_t row = (int32_t)floor((ph + 0.5) * (double)np);
+        row = row < 0 ? 0 : (row > np - 1 ? np - 1 : row);
+        gd[id * 5] = (double)row;
     }
 }
 

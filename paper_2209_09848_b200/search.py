@@ -15,7 +15,7 @@ class MatchedFilter:
                  force_generic: bool = False, record_events: bool = False, workspace_limit_mb: int = 0,
                  shift_stack: bool = False, filter: int = 0, prf_table=None):
         """filter: tno_mf_config::filter (0 Gaussian PRF, 1 shift-stack, 2 pixel-integrated Gaussian, 3 tabulated:
-        prf_table [n_phase, 5])."""
+        prf_table [n_phase, 5], 4 tabulated non-separable: prf_table [n_phase_y, n_phase_x, 5, 5])."""
         import torch
         self._torch = torch
         self.device = torch.device("cuda", device)
@@ -24,7 +24,10 @@ class MatchedFilter:
         self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events,
                                    workspace_limit_mb, shift_stack, filter)
         if prf_table is not None:
-            B.tno_mf_set_prf_table(self.ctx, prf_table)
+            if int(filter) == 4:
+                B.tno_mf_set_prf_table2d(self.ctx, prf_table)
+            else:
+                B.tno_mf_set_prf_table(self.ctx, prf_table)
 
     def close(self) -> None:
         if self.ctx is not None:
