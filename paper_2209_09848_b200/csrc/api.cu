@@ -385,7 +385,7 @@ int tno_mf_scatter_lossgrad(tno_mf_ctx *ctx, const float *D, int32_t T, int32_t 
     if (!out_loss || !g_beta || !g_S) return fail(ctx, TNO_MF_EINVAL, "tno_mf_scatter_lossgrad: NULL output");
     ScatterProblem pb;
     unsigned char *ws = nullptr;
-    const size_t blocks = std::max<size_t>(1024, ((size_t)N * N + 255) / 256);
+    const size_t blocks = std::max<size_t>(8192, ((size_t)N * N + 255) / 256);       // kLossPartials of scatter.cu
     const size_t psi_bytes = ((size_t)T * N * N * 4 + 255) & ~(size_t)255;
     int rc = scatter_setup(ctx, "tno_mf_scatter_lossgrad", D, T, N, n, jitter_xy, delta, beta, S,
                            psi_bytes + (blocks + 8) * 8, &pb, &ws);

@@ -45,6 +45,7 @@ k_downsample(const float *__restrict__ frames, int32_t H, int32_t W, int32_t f, 
 }
 
 constexpr int kRedBlocks = 1024;       // partial sums of every reduction
+constexpr int kLossPartials = 8192;    // capacity of the loss partials (blocks of the evaluation kernels)
 
 // block-wide sum in a fixed order -> partials[blockIdx.x]
 __device__ __forceinline__ void block_sum_to(double v, double *__restrict__ partials) {
@@ -248,6 +249,201 @@ k_scatter_resid_bulk(const float *__restrict__ D, int32_t T, int32_t N, int32_t 
     }
 }
 
+// ---- fused evaluation (N = 2 NT: one block per image row) -----------------------------------------------------------
+// k_scatter_resid_bulk, but psi never goes to global memory: dL/dS_t = -A^T psi_t A is separable, and the column
+// half of it, C[i][t][b] = sum_j wx(j, b) psi[t][i][j], only needs the row i the block owns.  The consumers put the
+// clipped residuals of a stage (FS frames x N pixels) into a padded shared buffer, then thread (f, b) sums the <= max_sup
+// columns under input column b -- pitch N + 1 makes the 8 frames x 4 columns of a warp hit 32 distinct banks -- and
+// the block writes FS x n partial sums, coalesced, to cpart[i][t][b].  k_scatter_gs_rows finishes the row half.  One
+// evaluation then reads the data once (T N^2 floats) and moves 2 T N n floats of partial sums: 1.3 GB instead of 3 GB at
+// the paper's size.  Every sum has a fixed order: the gradient is reproducible bit for bit.
+template <int NT, int NS, int FS, int SF>
+__global__ void __launch_bounds__(NT + 32, 3)
+k_scatter_fused(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, const float *__restrict__ phi,
+                const int32_t *__restrict__ bi0, const float *__restrict__ bw, const int32_t *__restrict__ blo,
+                const int32_t *__restrict__ bhi, int32_t max_sup, float delta,
+                const float *__restrict__ beta, const float *__restrict__ S, float *__restrict__ cpart,
+                float *__restrict__ g_beta, double *__restrict__ partials, int32_t t_chunk) {
+    // blockIdx.y: the chunk of frames [ta, tb) of this block; g_beta is then the block's partial sum, written to
+    // g_beta + blockIdx.y * 6 N^2 (k_scatter_gbeta_sum adds the chunks in order).  Chunks exist to balance the blocks
+    // over the SMs: N rows alone leave a second, nearly empty wave.
+    constexpr int PX = 2;
+    constexpr int PXF = NT * PX, STAGE = FS * (PXF + 8 + SF), PP = PXF + 1;
+    const int32_t ta = blockIdx.y * t_chunk, tb = min(T, ta + t_chunk);
+    extern __shared__ __align__(128) float ring[];               // [NS][STAGE], then psi rows [FS][PP], then weights
+    __shared__ __align__(8) uint64_t bars[2 * NS];
+    __shared__ double wsum[NT / 32];
+    float *prow = ring + NS * STAGE;                             // clipped residuals of the current stage
+    float *Wt = prow + FS * PP;                                  // [n][max_sup] column weights wx(blo[b] + c, b)
+    const uint32_t full = sc_smem(bars), empty = full + 8 * NS;
+    const int32_t tid = threadIdx.x, lane = tid & 31;
+    const int64_t n_px = (int64_t)N * N;
+    const int32_t i = blockIdx.x;                                // the image row of this block (N == PXF)
+    const int64_t p0 = (int64_t)i * PXF;
+    const uint32_t bytes = PXF * 4u;
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(full + 8 * s), "r"(1));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty + 8 * s), "r"(NT / 32));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int32_t total = (tb - ta + FS - 1) / FS;
+    const int32_t ra = bi0[i], rb = min(ra + 1, n - 1);          // the rows of S_t under this image row
+    const uint32_t sbytes = (uint32_t)(rb - ra + 1) * n * 4u;
+    if (tid >= NT) {
+        if (lane == 0) {
+            for (int32_t g = 0; g < total; ++g) {
+                const uint32_t s = (uint32_t)g % NS, bar = full + 8 * s, dst = sc_smem(ring + s * STAGE);
+                if (g >= NS) sc_wait(empty + 8 * s, ((uint32_t)(g / NS) - 1u) & 1u);
+                const int32_t t0 = ta + g * FS, nf = min(FS, tb - t0);
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(nf * (bytes + 32u + sbytes))
+                             : "memory");
+                for (int32_t f = 0; f < nf; ++f)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                                     "r"(dst + f * (PXF * 4)), "l"(D + (int64_t)(t0 + f) * n_px + p0), "r"(bytes), "r"(bar)
+                                 : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                                 "r"(dst + FS * (PXF * 4)), "l"(phi + 8 * (int64_t)t0), "r"(nf * 32u), "r"(bar)
+                             : "memory");
+                for (int32_t f = 0; f < nf; ++f)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                                     "r"(dst + (FS * (PXF + 8) + f * SF) * 4), "l"(S + ((int64_t)(t0 + f) * n + ra) * n),
+                                     "r"(sbytes), "r"(bar)
+                                 : "memory");
+            }
+        }
+        return;
+    }
+    // the weights of every input column over its support (at most max_sup image columns), once per block
+    for (int32_t e = tid; e < n * max_sup; e += NT) {
+        const int32_t b = e / max_sup, c = blo[b] + e % max_sup;
+        float w = 0.f;
+        if (c <= bhi[b]) {
+            const int32_t c0 = bi0[c], c1 = min(c0 + 1, n - 1);
+            const float v = bw[c];
+            w = (c0 == b ? 1.f - v : 0.f) + (c1 == b ? v : 0.f);
+        }
+        Wt[e] = w;
+    }
+    const int64_t p = p0 + (int64_t)tid * PX;
+    const int32_t j = tid * PX;
+    const int32_t i1 = rb;
+    const float wy = bw[i];
+    int32_t o0[PX], dj[PX];
+    float wx[PX];
+#pragma unroll
+    for (int k = 0; k < PX; ++k) {
+        const int32_t j0 = bi0[j + k];
+        o0[k] = j0;                                              // row ra of S_t is row 0 of the staged rows
+        dj[k] = min(j0 + 1, n - 1) - j0;
+        wx[k] = bw[j + k];
+    }
+    const int32_t di = (i1 - ra) * n;
+    float b[6][PX], g[6][PX];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float2 v = *reinterpret_cast<const float2 *>(beta + k * n_px + p);
+        b[k][0] = v.x; b[k][1] = v.y;
+        g[k][0] = g[k][1] = 0.f;
+    }
+    double loss = 0.0;
+    uint32_t st = 0, par = 0;
+    for (int32_t t0 = ta; t0 < tb; t0 += FS) {
+        sc_wait(full + 8 * st, par);
+        const float *sp = ring + st * STAGE;
+        float lsum = 0.f;
+#pragma unroll
+        for (int f = 0; f < FS; ++f) {
+            float c4[PX] = {0.f, 0.f};
+            if (t0 + f < tb) {
+                const float2 dv = reinterpret_cast<const float2 *>(sp + f * PXF)[tid];
+                const float4 qa = *reinterpret_cast<const float4 *>(sp + FS * PXF + f * 8);
+                const float2 qb = *reinterpret_cast<const float2 *>(sp + FS * PXF + f * 8 + 4);
+                const float q[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
+                const float d4[PX] = {dv.x, dv.y};
+                const float *St = sp + FS * (PXF + 8) + f * SF;
+#pragma unroll
+                for (int k = 0; k < PX; ++k) {
+                    const float a00 = St[o0[k]], a01 = St[o0[k] + dj[k]];
+                    const float a10 = St[o0[k] + di], a11 = St[o0[k] + di + dj[k]];
+                    // the same expression as k_scatter_resid: four weights times four values
+                    float pred = (1.f - wy) * (1.f - wx[k]) * a00 + (1.f - wy) * wx[k] * a01 + wy * (1.f - wx[k]) * a10 +
+                                 wy * wx[k] * a11;
+#pragma unroll
+                    for (int m = 0; m < 6; ++m) pred = fmaf(q[m], b[m][k], pred);
+                    const float r = d4[k] - pred;
+                    const float a = fabsf(r);
+                    lsum += a <= delta ? 0.5f * r * r : delta * (a - 0.5f * delta);       // Eq. 4
+                    const float c = fminf(fmaxf(r, -delta), delta);
+                    c4[k] = c;
+#pragma unroll
+                    for (int m = 0; m < 6; ++m) g[m][k] = fmaf(q[m], c, g[m][k]);
+                }
+            }
+            prow[f * PP + j] = c4[0];
+            prow[f * PP + j + 1] = c4[1];
+        }
+        loss += (double)lsum;
+        // the stage's data is consumed: hand it back, then reduce the psi rows along the columns
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty + 8 * st) : "memory");
+        asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory");
+        // thread -> (frame f = e % FS, input column b = e / FS): a warp covers FS frames x 32 / FS columns
+        for (int32_t e = tid; e < FS * n; e += NT) {
+            const int32_t f = e % FS, bb = e / FS;
+            if (t0 + f < tb) {
+                const float *pr = prow + f * PP + blo[bb], *w = Wt + bb * max_sup;
+                float sum = 0.f;
+                for (int32_t c = 0; c < max_sup; ++c) sum = fmaf(w[c], pr[c], sum);      // zero weights past the support
+                cpart[((int64_t)i * T + (t0 + f)) * n + bb] = sum;
+            }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory");      // prow is rewritten by the next stage
+        if (++st == NS) { st = 0; par ^= 1u; }
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+        *reinterpret_cast<float2 *>(g_beta + (int64_t)blockIdx.y * 6 * n_px + k * n_px + p) = make_float2(-g[k][0], -g[k][1]);
+    for (int o = 16; o > 0; o >>= 1) loss += __shfl_down_sync(0xffffffffu, loss, o);
+    if (lane == 0) wsum[tid >> 5] = loss;
+    asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory");
+    if (tid == 0) {
+        double s = 0.0;
+        for (int w = 0; w < NT / 32; ++w) s += wsum[w];
+        partials[blockIdx.y * gridDim.x + blockIdx.x] = s;
+    }
+}
+
+// g_beta = sum over the chunks of the partial sums, in order
+__global__ void __launch_bounds__(256)
+k_scatter_gbeta_sum(const float *__restrict__ part, int32_t n_chunk, int64_t n, float *__restrict__ g_beta) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float s = part[i];
+    for (int32_t c = 1; c < n_chunk; ++c) s += part[c * n + i];
+    g_beta[i] = s;
+}
+
+// g_S[t][a][b] = - sum_i wy(i, a) cpart[i][t][b] over the image rows i under input row a (rlo[a] .. rhi[a]), in order
+__global__ void __launch_bounds__(256)
+k_scatter_gs_rows(const float *__restrict__ cpart, int32_t T, int32_t N, int32_t n, const int32_t *__restrict__ bi0,
+                  const float *__restrict__ bw, const int32_t *__restrict__ blo, const int32_t *__restrict__ bhi,
+                  float *__restrict__ g_S) {
+    const int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (int64_t)T * n * n) return;
+    const int32_t b = (int32_t)(id % n), a = (int32_t)((id / n) % n), t = (int32_t)(id / ((int64_t)n * n));
+    float acc = 0.f;
+    for (int32_t i = blo[a]; i <= bhi[a]; ++i) {
+        const int32_t i0 = __ldg(bi0 + i), i1 = min(i0 + 1, n - 1);
+        const float w = __ldg(bw + i);
+        const float wy = (i0 == a ? 1.f - w : 0.f) + (i1 == a ? w : 0.f);
+        acc = fmaf(wy, __ldg(cpart + ((int64_t)i * T + t) * n + b), acc);
+    }
+    g_S[id] = -acc;
+}
+
 // dL/dS[t][a][b] = - sum_{i,j} wy(i, a) wx(j, b) psi[t][i][j]: only pixels within one input pixel of (a, b) count
 __global__ void __launch_bounds__(256)
 k_scatter_gs(const float *__restrict__ psi, int32_t T, int32_t N, int32_t n, const int32_t *__restrict__ bi0,
@@ -414,18 +610,37 @@ k_reduce_op(const double *__restrict__ partials, int32_t n, int32_t op, int32_t 
         else if (op == kBeta) sc[2] = alpha[i] - rho[i] * s;                           // r += (alpha_i - beta) s_i
     }
 }
-// z = x + (float)coef[0] * y   (z may alias x or y)
+// z = x + (float)coef[0] * y   (z may alias x or y); four elements per thread when n4 > 0 (n = 4 n4, aligned)
 __global__ void __launch_bounds__(256)
-k_axpy_dev(const float *x, const double *__restrict__ coef, const float *y, int64_t n, float *z) {
+k_axpy_dev(const float *x, const double *__restrict__ coef, const float *y, int64_t n, int64_t n4, float *z) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const float c = (float)coef[0];
-    if (i < n) z[i] = x[i] + c * y[i];
+    if (n4 > 0) {
+        if (i < n4) {
+            const float4 a = reinterpret_cast<const float4 *>(x)[i], b = reinterpret_cast<const float4 *>(y)[i];
+            reinterpret_cast<float4 *>(z)[i] = make_float4(a.x + c * b.x, a.y + c * b.y, a.z + c * b.z, a.w + c * b.w);
+        }
+    } else if (i < n) {
+        z[i] = x[i] + c * y[i];
+    }
 }
 // z = a x + b y   (z may alias x or y)
 __global__ void __launch_bounds__(256)
-k_axpby(float a, const float *x, float b, const float *y, int64_t n, float *z) {
+k_axpby(float a, const float *x, float b, const float *y, int64_t n, int64_t n4, float *z) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) z[i] = a * x[i] + (b != 0.f ? b * y[i] : 0.f);
+    if (n4 > 0) {
+        if (i < n4) {
+            const float4 u = reinterpret_cast<const float4 *>(x)[i];
+            float4 v = make_float4(a * u.x, a * u.y, a * u.z, a * u.w);
+            if (b != 0.f) {
+                const float4 w = reinterpret_cast<const float4 *>(y)[i];
+                v = make_float4(a * u.x + b * w.x, a * u.y + b * w.y, a * u.z + b * w.z, a * u.w + b * w.w);
+            }
+            reinterpret_cast<float4 *>(z)[i] = v;
+        }
+    } else if (i < n) {
+        z[i] = a * x[i] + (b != 0.f ? b * y[i] : 0.f);
+    }
 }
 
 // VEC: four neighbouring pixels per thread (W % 4 == 0, 16-byte aligned frames)
@@ -482,6 +697,46 @@ int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float 
     const bool aligned = ((reinterpret_cast<uintptr_t>(pb.D) | reinterpret_cast<uintptr_t>(beta) |
                            reinterpret_cast<uintptr_t>(psi) | reinterpret_cast<uintptr_t>(g_beta)) & 15u) == 0;
     constexpr int NT = 256, NS = 2, FS = 8, SF = 192;     // 45.6 KB per CTA: four CTAs per SM, all 512 blocks of N = 512 resident
+    // fused evaluation (one block per image row, psi stays on chip): N = 2 NT, two rows of S_t fit the staging area
+    // image columns under one input column: two stencil widths, plus the half width of clamped columns at the edge
+    // (input column 1 also "sees", with weight 0, the columns clamped to input column 0)
+    const int32_t max_sup_f = 5 * ((pb.N + pb.n - 1) / pb.n) / 2 + 4;
+    if (pb.N == 2 * NT && pb.n % 4 == 0 && 2 * pb.n <= SF && aligned && (reinterpret_cast<uintptr_t>(S) & 15u) == 0 &&
+        (size_t)pb.n * max_sup_f * 4 <= 32 * 1024) {
+        const size_t smem = ((size_t)NS * FS * (NT * 2 + 8 + SF) + (size_t)FS * (NT * 2 + 1) + (size_t)pb.n * max_sup_f) * 4;
+        cudaFuncSetAttribute(k_scatter_fused<NT, NS, FS, SF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        // chunks of frames: the number (<= 16, chunks of at least two stages, partial sums inside the scratch stack)
+        // that wastes the least of the last wave of blocks, three blocks per SM
+        int dev = 0, n_sm = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        const double slots = 3.0 * n_sm;
+        int32_t n_chunk = 1;
+        double best = std::ceil(pb.N / slots);
+        for (int32_t c = 2; c <= 16; ++c) {
+            const int32_t tc = ((pb.T + c - 1) / c + FS - 1) / FS * FS;
+            if (tc < 2 * FS || (int64_t)(c - 1) * tc >= pb.T) continue;
+            if ((int64_t)pb.N * pb.T * pb.n + (int64_t)c * 6 * n_px > (int64_t)pb.T * n_px || (int64_t)c * pb.N > kLossPartials)
+                continue;
+            const double cost = std::ceil(c * pb.N / slots) / c;
+            if (cost < best - 1e-9) { best = cost; n_chunk = c; }
+        }
+        const int32_t t_chunk = n_chunk == 1 ? pb.T : ((pb.T + n_chunk - 1) / n_chunk + FS - 1) / FS * FS;
+        float *gb_part = n_chunk == 1 ? g_beta : psi + (int64_t)pb.N * pb.T * pb.n;
+        dim3 grid((unsigned)pb.N, (unsigned)n_chunk);
+        k_scatter_fused<NT, NS, FS, SF><<<grid, NT + 32, smem, st>>>(
+            pb.D, pb.T, pb.N, pb.n, pb.phi, pb.bi0, pb.bw, pb.blo, pb.bhi, max_sup_f, pb.delta, beta, S, psi, gb_part,
+            partials, t_chunk);
+        int32_t launched = 3;
+        if (n_chunk > 1) {
+            k_scatter_gbeta_sum<<<(unsigned)((6 * n_px + 255) / 256), 256, 0, st>>>(gb_part, n_chunk, 6 * n_px, g_beta);
+            ++launched;
+        }
+        k_sum_partials<<<1, 256, 0, st>>>(partials, pb.N * n_chunk, 0, loss_dev);
+        const int64_t ns = (int64_t)pb.T * pb.n * pb.n;
+        k_scatter_gs_rows<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(psi, pb.T, pb.N, pb.n, pb.bi0, pb.bw, pb.blo, pb.bhi, g_S);
+        return launched;
+    }
     // rows of S a block of NT * 2 pixels can touch: those under its first and last image row, plus one
     const int64_t img_rows = std::min<int64_t>(pb.N, (NT * 2 + pb.N - 2) / pb.N + 1);
     const int64_t s_rows = std::min<int64_t>(pb.n, (img_rows * pb.n + pb.N - 1) / pb.N + 2);
@@ -501,9 +756,9 @@ int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float 
     if (pb.N <= 1024) {
         // strips of input columns: 4 for the paper's n = 64; image columns of a strip <= N / strips + two stencils
         const int32_t n_strip = pb.n >= 16 ? 4 : 1, strip_b = (pb.n + n_strip - 1) / n_strip;
-        const int32_t cols = std::min(pb.N, (pb.N + n_strip - 1) / n_strip + 2 * ((pb.N + pb.n - 1) / pb.n) + 4);
+        const int32_t cols = std::min(pb.N, (pb.N + n_strip - 1) / n_strip + max_sup_f);
         const int32_t threads = ((std::max(cols, strip_b) + 31) / 32) * 32;
-        const int32_t max_sup = 2 * ((pb.N + pb.n - 1) / pb.n) + 4;          // image columns under one input column
+        const int32_t max_sup = max_sup_f;                                   // image columns under one input column
         dim3 grid((unsigned)pb.T, (unsigned)((pb.n + strip_b - 1) / strip_b));
         k_scatter_gs_cols<<<grid, threads, ((size_t)threads + (size_t)strip_b * max_sup) * 4, st>>>(
             psi, pb.N, pb.n, pb.bi0, pb.bw, pb.blo, pb.bhi, strip_b, max_sup, g_S);
@@ -522,14 +777,14 @@ int32_t scatter_lossgrad(cudaStream_t st, const ScatterProblem &pb, const float 
 // line search cannot decrease it at all (float32 resolution reached).
 size_t scatter_ws_bytes(int32_t T, int32_t N, int32_t n) {
     const size_t P = (size_t)6 * N * N + (size_t)T * n * n;
-    const size_t blocks = std::max<size_t>(kRedBlocks, ((size_t)N * N + 255) / 256);
+    const size_t blocks = std::max<size_t>(kLossPartials, ((size_t)N * N + 255) / 256);
     return (5 + 2 * (size_t)kScatterHistory) * P * 4 + (size_t)T * N * N * 4 + (blocks + 8 + 2 * kScatterHistory) * 8 + 256;
 }
 
 int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, float *S, void *ws, int32_t max_iter,
                     float gtol, double *out_loss, int32_t *out_iters, int32_t *out_evals, int32_t *out_launches) {
     const int64_t nb = (int64_t)6 * pb.N * pb.N, ns = (int64_t)pb.T * pb.n * pb.n, P = nb + ns;
-    const size_t blocks = std::max<size_t>(kRedBlocks, ((size_t)pb.N * pb.N + 255) / 256);
+    const size_t blocks = std::max<size_t>(kLossPartials, ((size_t)pb.N * pb.N + 255) / 256);
     float *x = static_cast<float *>(ws), *g = x + P, *xn = g + P, *gn = xn + P, *d = gn + P;
     float *hs = d + P, *hy = hs + (size_t)kScatterHistory * P, *psi = hy + (size_t)kScatterHistory * P;
     double *partials = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(psi + (size_t)pb.T * pb.N * pb.N) + 15) &
@@ -553,12 +808,15 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
         dot_to(a, b, kStore0, 0);
         return fetch(scal);
     };
+    // every vector of the workspace starts a multiple of P floats after the 256-byte aligned base
+    const int64_t P4 = (P % 4 == 0 && (reinterpret_cast<uintptr_t>(ws) & 15u) == 0) ? P / 4 : 0;
+    const unsigned vgrid = (unsigned)(((P4 > 0 ? P4 : P) + 255) / 256);
     auto axpby = [&](float a, const float *xx, float b, const float *yy, float *zz) {
-        k_axpby<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(a, xx, b, yy, P, zz);
+        k_axpby<<<vgrid, 256, 0, st>>>(a, xx, b, yy, P, P4, zz);
         launches += 1;
     };
     auto axpy_dev = [&](const float *xx, const float *yy, float *zz) {                // zz = xx + sc[2] * yy
-        k_axpy_dev<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(xx, scal + 2, yy, P, zz);
+        k_axpy_dev<<<vgrid, 256, 0, st>>>(xx, scal + 2, yy, P, P4, zz);
         launches += 1;
     };
     auto eval = [&](const float *xx, float *gg) -> double {
@@ -634,6 +892,10 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
             gamma[head] = sy / yy;
             head = (head + 1) % kScatterHistory;
             hist = std::min(hist + 1, kScatterHistory);
+        } else if (hist == kScatterHistory) {
+            // the rejected pair was written over the oldest pair of a full history: that slot no longer holds a
+            // valid pair, so it leaves the recursion (which reads slots head - 1 ... head - hist)
+            hist = kScatterHistory - 1;
         }
         std::swap(x, xn);
         std::swap(g, gn);

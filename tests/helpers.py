@@ -65,3 +65,18 @@ def check_topk_vs_own_map(gpu, gmap, k, ktop, thr):
     assert np.array_equal(gpu["x"], ref["x"]) and np.array_equal(gpu["y"], ref["y"])
     assert np.array_equal(gpu["snr"].astype(np.float64), ref["snr"])
     assert np.all(gpu["k"] == k)
+
+
+def scatter_problem(seed, T, N, n, noise=0.3, outliers=0.02):
+    """Smooth scattered light that changes from frame to frame over a static background that moves with the
+    jitter, plus noise and a few outliers (the shape of the paper's problem)."""
+    rng = np.random.default_rng(seed)
+    jit = (0.15 * rng.standard_normal((T, 2))).astype(np.float32)
+    beta = rng.standard_normal((6, N, N)) * np.array([20, 3, 3, 1, 1, 1])[:, None, None]
+    S = 10.0 + 5.0 * rng.standard_normal((T, n, n))
+    D = oracle.upsample(S, N) + np.einsum("tk,kij->tij", oracle.background_basis(jit), beta)
+    D += noise * rng.standard_normal(D.shape)
+    D += (rng.uniform(size=D.shape) < outliers) * rng.laplace(0, 15, size=D.shape)
+    return D.astype(np.float32), jit, beta, S
+
+

@@ -16,22 +16,15 @@ def _torch():
     return torch
 
 
-def _problem(seed, T, N, n, noise=0.3, outliers=0.02):
-    """Smooth scattered light that changes from frame to frame over a static background that moves with the
-    jitter, plus noise and a few outliers (the shape of the paper's problem)."""
-    rng = np.random.default_rng(seed)
-    jit = (0.15 * rng.standard_normal((T, 2))).astype(np.float32)
-    beta = rng.standard_normal((6, N, N)) * np.array([20, 3, 3, 1, 1, 1])[:, None, None]
-    S = 10.0 + 5.0 * rng.standard_normal((T, n, n))
-    D = oracle.upsample(S, N) + np.einsum("tk,kij->tij", oracle.background_basis(jit), beta)
-    D += noise * rng.standard_normal(D.shape)
-    D += (rng.uniform(size=D.shape) < outliers) * rng.laplace(0, 15, size=D.shape)
-    return D.astype(np.float32), jit, beta, S
+from helpers import scatter_problem as _problem  # noqa: E402
 
 
 @pytest.mark.parametrize("T,N,n", [(9, 24, 3), (5, 64, 8), (17, 40, 5), (3, 16, 16), (6, 33, 4),
                                    (2, 1040, 13),           # N > 1024: the gather form of the S gradient
-                                   (11, 36, 4), (3, 512, 64)])    # staged kernel: ragged last block, T % 8 != 0; paper size
+                                   (11, 36, 4), (3, 512, 64),     # staged kernel: ragged last block, T % 8 != 0; paper size
+                                   (19, 512, 64), (9, 512, 32),   # fused kernel (N = 512): several stages, ratio 8 and 16
+                                   (8, 512, 96),                  # ... and a non-integer N / n
+                                   (5, 256, 16), (4, 320, 8)])    # wide stencils (N / n = 16, 40) on the two-kernel path
 def test_loss_and_gradient_match_oracle(T, N, n):
     torch = _torch()
     import paper_2209_09848_b200 as P
@@ -107,6 +100,34 @@ def test_fit_reaches_the_oracles_minimum():
                                                              b.cpu().numpy().astype(np.float64))
     pred_o = oracle.upsample(oS, N) + np.einsum("tk,kij->tij", oracle.background_basis(jit), ob)
     assert np.sqrt(np.mean((pred_g - pred_o) ** 2)) < 0.02           # noise is 0.3: the fits agree far below it
+
+
+def test_fit_parity_on_a_longer_stack():
+    """The fit at 200 frames of 128 x 128 (n = 16): the convex minimum and the prediction of scipy's L-BFGS-B (the
+    oracle; its result is stored by tests/golden/make_scatter_golden.py, which takes the oracle a quarter of an hour)
+    are reached from zeros, and two calls give the same bits."""
+    torch = _torch()
+    import os
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    T, N, n = 200, 128, 16
+    D, jit, beta, S = _problem(21, T, N, n)
+    delta = 1.0
+    gold = np.loadtxt(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "scatter_fit_T200_N128_n16.txt"))
+    oL, samples = gold[0, 3], gold[1:]
+    with MatchedFilter(0) as mf:
+        d = torch.from_numpy(D).cuda()
+        b = torch.zeros((6, N, N), device="cuda")
+        s = torch.zeros((T, n, n), device="cuda")
+        loss, iters, evals = P.tno_mf_scatter_fit(mf.ctx, d, jit, delta, 3000, 0.0, b, s)
+        b2, s2 = torch.zeros_like(b), torch.zeros_like(s)
+        loss2, iters2, _ = P.tno_mf_scatter_fit(mf.ctx, d, jit, delta, 3000, 0.0, b2, s2)
+        assert loss2 == loss and iters2 == iters and torch.equal(b2, b) and torch.equal(s2, s)
+    assert abs(loss - oL) <= 2e-4 * oL, (loss, oL, iters, evals)
+    basis = oracle.background_basis(jit)
+    pred_g = oracle.upsample(s.cpu().numpy(), N) + np.einsum("tk,kij->tij", basis, b.cpu().numpy().astype(np.float64))
+    t, i, j = samples[:, 0].astype(int), samples[:, 1].astype(int), samples[:, 2].astype(int)
+    assert np.sqrt(np.mean((pred_g[t, i, j] - samples[:, 3]) ** 2)) < 0.03      # noise is 0.3
 
 
 def test_fit_on_exact_data_and_errors():
