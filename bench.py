@@ -384,6 +384,35 @@ def run_ours(args, cfg):
             extras["background_n_iter_%d" % n_iter] = {"ms": ms, "algorithmic_gb": gb, "achieved_gbs": gb / ms * 1e3,
                                                        "peak_gbs": hbm, "frac": gb / ms * 1e3 / hbm if hbm else None}
 
+        if cfg.want_maps and cfg.H % 4 == 0 and cfg.W == cfg.H and cfg.H >= 64:
+            # the paper's whole chain on this stack, back to back (README): downsample -> scattered-light fit ->
+            # subtract -> per-pixel background -> search with the max over the bank -> local-sigma scores -> peaks.
+            # Host-timed: the fit reads scalars back, the rest is asynchronous until the final synchronize.
+            import paper_2209_09848_b200 as P
+            N, n = cfg.H // 4, cfg.H // 32
+            low = torch.empty((cfg.T, N, N), device=dev)
+            b = torch.zeros((6, N, N), device=dev)
+            s = torch.zeros((cfg.T, n, n), device=dev)
+            mxf, akf = torch.empty((cfg.H, cfg.W), device=dev), torch.empty((cfg.H, cfg.W), dtype=torch.int32, device=dev)
+            torch.cuda.synchronize()
+            t_chain = time.perf_counter()
+            P.tno_mf_downsample(mf.ctx, frames, 4, low)
+            _, it_c, ev_c = P.tno_mf_scatter_fit(mf.ctx, low, jit, 1.0, 1000, 0.0, b, s)
+            P.tno_mf_scatter_subtract(mf.ctx, frames, s)
+            mf.background(frames, jit, 1.0, 4, in_place=True)
+            P.tno_mf_search_max(mf.ctx, frames, None, p.sigma_t, None, None, p.traj, cfg.prf_sigma, cfg.t0, mxf, akf,
+                                None, out_topk)
+            _, _, zc, _ = mf.best(mxf[None])
+            mf.peaks(zc, 5, akf)
+            torch.cuda.synchronize()
+            extras["chain"] = {"seconds": time.perf_counter() - t_chain, "scatter_fit_iterations": it_c,
+                               "what": "downsample 4x -> L-BFGS scattered-light fit -> subtract -> Huber background "
+                                       "(4 iterations, in place) -> search with fused max over the bank -> local-sigma "
+                                       "Z -> non-maximum suppression, on the resident stack",
+                               "paper": "3-5 min per CCD-sector on an A100 (PAPER.md:L25, L144), 1 min of it the "
+                                        "two background steps"}
+            del low, b, s
+
     mf.close()
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -220,6 +220,17 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
                   const tno_mf_source *sources, int32_t n_sources,
                   float prf_sigma, float t0);
 
+/* tno_mf_inject on the track that tno_mf_search_ex scores: frame times and pointing jitter enter the position of
+ * the source exactly as they enter the filter, c_t = (x, y) + v (tau_t - t0) + a (tau_t - t0)^2 + j_t ("the line of
+ * the trajectory (including the pointing jitter)"; injection = "adding a filter times a flux", L130),
+ * so that injection and recovery are consistent for irregular cadence and jitter.
+ *   frame_times HOST float32 [T] or NULL; jitter_xy HOST float32 [T][2] or NULL (both NULL = tno_mf_inject).
+ * Errors: EINVAL (also: non-finite times / jitter, a displacement beyond 1e9 px), ENOMEM, ECUDA. */
+int tno_mf_inject_ex(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W,
+                     const float *frame_times, const float *jitter_xy,
+                     const tno_mf_source *sources, int32_t n_sources,
+                     float prf_sigma, float t0);
+
 /* Interpreting scores (section 3.3): "We take the maximum score across the filter bank, which
  * then tells us the most likely trajectory, along with the score of that trajectory" (L112), and "we
  * compute the standard deviation sigma of the scores in the 255 x 255 square centered on a pixel. We

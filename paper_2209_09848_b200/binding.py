@@ -68,6 +68,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
+    lib.tno_mf_inject_ex.restype = ctypes.c_int
+    lib.tno_mf_inject_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, i32, f32, f32]
     f64p = ctypes.POINTER(ctypes.c_double)
     i32p = ctypes.POINTER(i32)
     lib.tno_mf_scatter_lossgrad.restype = i32
@@ -342,6 +344,19 @@ def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float)
     src = np.ascontiguousarray(sources, dtype=SOURCE_DTYPE)
     _check(_lib.tno_mf_inject(ctx, frames.data_ptr(), T, H, W, src.ctypes.data, src.shape[0],
                               float(prf_sigma), float(t0)), ctx)
+
+
+def tno_mf_inject_ex(ctx, frames, frame_times, jitter_xy, sources: np.ndarray, prf_sigma: float, t0: float) -> None:
+    """tno_mf_inject with frame times (host [T] or None) and pointing jitter (host [T, 2] or None) in the track."""
+    assert frames.is_cuda and frames.is_contiguous() and frames.dim() == 3 and frames.element_size() == 4
+    T, H, W = frames.shape
+    src = np.ascontiguousarray(sources, dtype=SOURCE_DTYPE)
+    tm = None if frame_times is None else np.ascontiguousarray(frame_times, dtype=np.float32)
+    jt = None if jitter_xy is None else np.ascontiguousarray(jitter_xy, dtype=np.float32)
+    assert (tm is None or tm.shape == (T,)) and (jt is None or jt.shape == (T, 2))
+    _check(_lib.tno_mf_inject_ex(ctx, frames.data_ptr(), T, H, W, tm.ctypes.data if tm is not None else None,
+                                 jt.ctypes.data if jt is not None else None, src.ctypes.data, src.shape[0],
+                                 float(prf_sigma), float(t0)), ctx)
 
 
 def _dev3(t, shape=None):

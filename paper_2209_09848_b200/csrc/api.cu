@@ -503,6 +503,12 @@ int tno_mf_set_prf_table2d(tno_mf_ctx *ctx, const float *table, int32_t n_phase_
 
 int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W,
                   const tno_mf_source *sources, int32_t n_sources, float prf_sigma, float t0) {
+    return tno_mf_inject_ex(ctx, frames, T, H, W, nullptr, nullptr, sources, n_sources, prf_sigma, t0);
+}
+
+int tno_mf_inject_ex(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t W, const float *frame_times,
+                     const float *jitter_xy, const tno_mf_source *sources, int32_t n_sources, float prf_sigma,
+                     float t0) {
     if (!ctx) return TNO_MF_EINVAL;
     if (!frames || !sources || T < 1 || H < 1 || W < 1 || n_sources < 0)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: NULL pointer or non-positive size");
@@ -512,6 +518,12 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: filter 3 needs a table (tno_mf_set_prf_table)");
     if (ctx->cfg.filter == 4 && ctx->prf2_py == 0)
         return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: filter 4 needs a table (tno_mf_set_prf_table2d)");
+    for (int32_t t = 0; t < T; ++t) {
+        if (frame_times && !finite_f(frame_times[t]))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: frame_times[%d] is not finite", t);
+        if (jitter_xy && (!finite_f(jitter_xy[2 * t]) || !finite_f(jitter_xy[2 * t + 1])))
+            return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: jitter_xy[%d] is not finite", t);
+    }
     if (n_sources == 0) return TNO_MF_OK;
     std::vector<SourceDev> host(n_sources);
     for (int32_t m = 0; m < n_sources; ++m) {
@@ -520,16 +532,34 @@ int tno_mf_inject(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32_t 
             !finite_f(s.amplitude))
             return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: source %d has a non-finite value", m);
         host[m] = {s.traj.vx, s.traj.vy, s.traj.ax, s.traj.ay, s.x, s.y, s.amplitude};
+        // the displacement must fit 32-bit pixel arithmetic, as in the search (reading d2)
+        for (int32_t t = 0; t < T; ++t) {
+            const double dt = (frame_times ? (double)frame_times[t] : (double)t) - (double)t0;
+            int32_t sh;
+            if (!axis_shift((double)s.traj.vx, (double)s.traj.ax, dt, jitter_xy ? (double)jitter_xy[2 * t] : 0.0, &sh) ||
+                !axis_shift((double)s.traj.vy, (double)s.traj.ay, dt, jitter_xy ? (double)jitter_xy[2 * t + 1] : 0.0, &sh))
+                return fail(ctx, TNO_MF_EINVAL, "tno_mf_inject: the displacement of source %d exceeds 1e9 px", m);
+        }
     }
     CU_TRY(ctx, cudaSetDevice(ctx->cfg.device));
-    int rc = reserve(ctx, ctx->src, host.size() * sizeof(SourceDev));
+    // one upload: the sources, then frame_times [T] and jitter_xy [T][2] if given
+    const size_t src_bytes = (host.size() * sizeof(SourceDev) + 15) & ~(size_t)15;
+    std::vector<unsigned char> blob(src_bytes + (frame_times ? (size_t)T * 4 : 0) + (jitter_xy ? (size_t)T * 8 : 0) + 16);
+    std::memcpy(blob.data(), host.data(), host.size() * sizeof(SourceDev));
+    size_t o_tm = src_bytes, o_jt = (o_tm + (frame_times ? (size_t)T * 4 : 0) + 7) & ~(size_t)7;
+    if (frame_times) std::memcpy(blob.data() + o_tm, frame_times, (size_t)T * 4);
+    if (jitter_xy) std::memcpy(blob.data() + o_jt, jitter_xy, (size_t)T * 8);
+    int rc = reserve(ctx, ctx->src, blob.size());
     if (rc) return rc;
-    CU_TRY(ctx, cudaMemcpyAsync(ctx->src.p, host.data(), host.size() * sizeof(SourceDev),
-                                cudaMemcpyHostToDevice, ctx->stream));
-    launch_inject(ctx->stream, frames, T, H, W, static_cast<const SourceDev *>(ctx->src.p), n_sources,
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->src.p, blob.data(), blob.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));      // blob is a local buffer
+    const unsigned char *base = static_cast<const unsigned char *>(ctx->src.p);
+    launch_inject(ctx->stream, frames, T, H, W, reinterpret_cast<const SourceDev *>(base), n_sources,
                   (double)prf_sigma, (double)t0, ctx->cfg.filter,
                   static_cast<const float *>(ctx->cfg.filter == 4 ? ctx->prf_tab2.p : ctx->prf_tab.p),
-                  ctx->cfg.filter == 4 ? (ctx->prf2_py << 16 | ctx->prf2_px) : ctx->prf_phases);
+                  ctx->cfg.filter == 4 ? (ctx->prf2_py << 16 | ctx->prf2_px) : ctx->prf_phases,
+                  frame_times ? reinterpret_cast<const float *>(base + o_tm) : nullptr,
+                  jitter_xy ? reinterpret_cast<const float *>(base + o_jt) : nullptr);
     CU_TRY(ctx, cudaGetLastError());
     return TNO_MF_OK;
 }

@@ -5,8 +5,9 @@
 
 namespace tno {
 
-__device__ __forceinline__ void axis_pos(double v, double a, double dt, int32_t *s, double *ph) {
-    const double d = __dadd_rn(__dmul_rn(v, dt), __dmul_rn(__dmul_rn(a, dt), dt));
+// d = (v*dt + (a*dt)*dt) + j, every operation separately rounded: the evaluation of k_class_tables (tables.cu)
+__device__ __forceinline__ void axis_pos(double v, double a, double dt, double j, int32_t *s, double *ph) {
+    const double d = __dadd_rn(__dadd_rn(__dmul_rn(v, dt), __dmul_rn(__dmul_rn(a, dt), dt)), j);
     const double f = floor(__dadd_rn(d, 0.5));
     *s = (int32_t)f;
     *ph = __dsub_rn(d, f);
@@ -14,18 +15,20 @@ __device__ __forceinline__ void axis_pos(double v, double a, double dt, int32_t 
 
 __global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32_t W,
                          const SourceDev *__restrict__ src, int32_t n_src, double prf_sigma,
-                         double t0, int32_t filter, const float *__restrict__ prf_tab, int32_t n_phase) {
+                         double t0, int32_t filter, const float *__restrict__ prf_tab, int32_t n_phase,
+                         const float *__restrict__ times, const float *__restrict__ jitter) {
     const int32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= T) return;
-    const double dt = (double)t - t0;
+    const double dt = __dsub_rn(times ? (double)times[t] : (double)t, t0);
+    const double jx = jitter ? (double)jitter[2 * t] : 0.0, jy = jitter ? (double)jitter[2 * t + 1] : 0.0;
     const double inv = 1.0 / (2.0 * prf_sigma * prf_sigma);
     float *f = frames + (int64_t)t * H * W;
     for (int32_t m = 0; m < n_src; ++m) {
         const SourceDev s = src[m];
         int32_t sx, sy;
         double phx, phy;
-        axis_pos((double)s.vx, (double)s.ax, dt, &sx, &phx);
-        axis_pos((double)s.vy, (double)s.ay, dt, &sy, &phy);
+        axis_pos((double)s.vx, (double)s.ax, dt, jx, &sx, &phx);
+        axis_pos((double)s.vy, (double)s.ay, dt, jy, &sy, &phy);
         for (int j = -2; j <= 2; ++j) {
             const int32_t py = s.y + sy + j;
             if (py < 0 || py >= H) continue;
@@ -57,9 +60,9 @@ __global__ void k_inject(float *__restrict__ frames, int32_t T, int32_t H, int32
 
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,
                    const SourceDev *src, int32_t n_src, double prf_sigma, double t0, int32_t filter,
-                   const float *prf_tab, int32_t n_phase) {
+                   const float *prf_tab, int32_t n_phase, const float *times, const float *jitter) {
     k_inject<<<(unsigned)((T + 63) / 64), 64, 0, st>>>(frames, T, H, W, src, n_src, prf_sigma, t0, filter, prf_tab,
-                                                       n_phase);
+                                                       n_phase, times, jitter);
 }
 
 }  // namespace tno

@@ -90,7 +90,8 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
 struct SourceDev { float vx, vy, ax, ay; int32_t x, y; float amp; };
 void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W,
                    const SourceDev *src, int32_t n_src, double prf_sigma, double t0, int32_t filter,
-                   const float *prf_tab, int32_t n_phase);
+                   const float *prf_tab, int32_t n_phase, const float *times /* DEVICE [T] or NULL */,
+                   const float *jitter /* DEVICE [T][2] or NULL */);
 
 // ---- search_sep.cu ----
 struct SepVariant {

@@ -129,8 +129,9 @@ class MatchedFilter:
         B.tno_mf_peaks(self.ctx, score, argk, radius, out, top)
         return out, top
 
-    def inject(self, frames, trajs, xs, ys, amps, prf_sigma: float, t0: float) -> None:
-        B.tno_mf_inject(self.ctx, frames, B.make_sources(trajs, xs, ys, amps), prf_sigma, t0)
+    def inject(self, frames, trajs, xs, ys, amps, prf_sigma: float, t0: float, frame_times=None,
+               jitter_xy=None) -> None:
+        B.tno_mf_inject_ex(self.ctx, frames, frame_times, jitter_xy, B.make_sources(trajs, xs, ys, amps), prf_sigma, t0)
 
     @staticmethod
     def candidates_to_numpy(out_topk) -> np.ndarray:

@@ -83,3 +83,40 @@ def test_injected_source_is_recovered_at_a_sqrt_d_and_bad_values_are_rejected():
     with pytest.raises(P.TnoMfError):
         P.tno_mf_search_ex(ctx, d, sigma, None, badj, tr, 1.0, t0, out)
     P.tno_mf_destroy(ctx)
+
+
+def test_injection_on_the_jittered_track_is_recovered_by_search_ex():
+    """tno_mf_inject_ex renders the source on the track that tno_mf_search_ex scores (irregular cadence + jitter):
+    it equals the oracle's renderer, and the search finds the source at its start pixel with SNR = A sqrt(D)."""
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    T, H, W = 50, 64, 96
+    rng = np.random.default_rng(4)
+    times = (np.arange(T) + np.where(np.arange(T) >= 20, 7.25, 0.0) + rng.uniform(-0.3, 0.3, T)).astype(np.float32)
+    jitter = (0.7 * rng.standard_normal((T, 2))).astype(np.float32)
+    sigma = rng.uniform(0.8, 1.2, T).astype(np.float32)
+    tr = np.array([[0.21, -0.13, 0.001, 0.0005], [-0.3, 0.3, 0, 0]], np.float32)
+    t0 = float(times[T // 2])
+    ref = np.zeros((T, H, W), np.float32)
+    oracle.inject(ref, tr, [40, 70], [30, 12], [6.0, 9.0], 1.0, t0, times=times, jitter=jitter)
+    with MatchedFilter(0, 3, 5.0) as mf:
+        d = torch.zeros((T, H, W), dtype=torch.float32, device="cuda")
+        mf.inject(d, tr, [40, 70], [30, 12], [6.0, 9.0], 1.0, t0, frame_times=times, jitter_xy=jitter)
+        torch.cuda.synchronize()
+        assert np.array_equal(d.cpu().numpy(), ref)
+        plain = torch.zeros_like(d)
+        mf.inject(plain, tr, [40, 70], [30, 12], [6.0, 9.0], 1.0, t0)           # without times / jitter: another track
+        assert not torch.equal(plain, d)
+        maps, cand = mf.search(d, sigma, tr, 1.0, t0, frame_times=times, jitter_xy=jitter)
+        torch.cuda.synchronize()
+        c = mf.candidates_to_numpy(cand)
+        for k, (x, y, A) in enumerate(((40, 30, 6.0), (70, 12, 9.0))):
+            s, N, D = oracle.point(ref, sigma, tr[k], 1.0, t0, x, y, times=times, jitter=jitter)
+            assert abs(N / D - A) < 1e-4 * A and abs(s - A * np.sqrt(D)) < 1e-4 * s
+            assert (int(c[k]["x"][0]), int(c[k]["y"][0])) == (x, y) and abs(float(c[k]["snr"][0]) - s) <= TOL
+        with pytest.raises(P.TnoMfError):                   # a displacement beyond 32-bit pixel arithmetic
+            mf.inject(d, np.array([[3e8, 0, 0, 0]], np.float32), [1], [1], [1.0], 1.0, 0.0)
+        bad = times.copy(); bad[3] = np.nan
+        with pytest.raises(P.TnoMfError):
+            mf.inject(d, tr, [40, 70], [30, 12], [6.0, 9.0], 1.0, t0, frame_times=bad)
