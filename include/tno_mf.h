@@ -71,7 +71,8 @@ typedef struct {
                                 1 = always use the generic (non-TMA) kernel -- for tests */
     int32_t record_events;   /* != 0: bracket the main search kernel with CUDA events on the stream
                                 so that tno_mf_last_kernel_ms can report its duration */
-    int32_t workspace_limit_mb; /* 0 = default (<= 8 GB and <= 80 % of the free device memory);
+    int32_t workspace_limit_mb; /* 0 = default (<= 8 GB -- 40 GB in tno_mf_search_host, where the first chunk
+                                hides the upload -- and <= 80 % of the free device memory);
                                 > 0: cap, in MiB, of the partial-sum workspace of the separable
                                 kernel -- a bank that needs more is searched in chunks of whole
                                 batches (same results) */

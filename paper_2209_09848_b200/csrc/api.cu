@@ -932,7 +932,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         if ((rc = reserve(ctx, ctx->counts, (size_t)n_tiles * n_traj * 4))) return rc;
     }
     // piece buffer: n_pieces partial-sum maps per entry; the bank is processed in chunks of whole
-    // batches when it does not fit the budget (<= 8 GB and <= 80 % of what the device has free)
+    // batches when it does not fit the budget (<= 8 GB, or 40 GB for a host-fed search whose first chunk hides the upload, and <= 80 % of what the device has free)
     const int64_t map_px = (int64_t)H * W;
     int64_t chunk_cap = n_traj;                            // entries per chunk
     if (use_sep) {
@@ -941,7 +941,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         const size_t per_entry = (size_t)n_pass * n_pieces * map_px * 4;
         const size_t want = per_entry * n_traj;
         const size_t limit = ctx->cfg.workspace_limit_mb > 0 ? (size_t)ctx->cfg.workspace_limit_mb << 20
-                                                             : (size_t)8 << 30;
+                                                             : (size_t)(ctx->feed_host ? 40 : 8) << 30;
         size_t have = std::min(ctx->pieces.cap, limit);
         if (want > have) {
             size_t free_b = 0, total_b = 0;

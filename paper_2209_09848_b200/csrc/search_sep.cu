@@ -408,8 +408,10 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         const int32_t r0 = warp * R;
         int32_t n = 0;
         uint32_t fpar = 0;        // bit s = parity of the number of flushes of slot s so far
-        const float2 *xp0 = reinterpret_cast<const float2 *>(Xbuf + r0 * kXP) + lane;     // this thread's window in X[0]
-        asm volatile("" : "+l"(xp0));      // kept in a register: not recomputed from the thread index every frame
+        // this thread's window in X[0] as a shared-window address, kept in a register (not recomputed from the
+        // thread index every frame); the loads below are explicit ld.shared with immediate row offsets
+        uint32_t xw0 = smem_u32(Xbuf + r0 * kXP) + 8u * (uint32_t)lane;
+        asm volatile("" : "+r"(xw0));
         for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
             // flush coordinates of the item: the members of the batch have planned indices q_first + (the
             // offsets in the table), a member's piece map starts at ebase + offset*H*W (this lane's two
@@ -441,13 +443,14 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 if (y_active) {
                     // ---------------- y-pass: one register window of X for all slots of the batch, and the
                     // sums and differences of its rows about each of this thread's R positions
-                    const float2 *xp = xp0 + xr * (C::XBUF / 2);
-                    TNO_CHECK(reinterpret_cast<const float *>(xp + (R + 3) * (kXP / 2)) + 1 <
-                              Xbuf + (xr + 1) * C::XBUF);                 // the window lies inside X[xr]
+                    const uint32_t xw = xw0 + (uint32_t)xr * (C::XBUF * 4);
+                    TNO_CHECK(xw + (R + 3) * (kXP * 4) + 8 <= smem_u32(Xbuf + (xr + 1) * C::XBUF));   // inside X[xr]
                     TNO_CHECK(hdr23.x >= 1 && hdr23.x <= NB && (hdr23.y >> NB) == 0);
                     float2 win[R + 4];
 #pragma unroll
-                    for (int r = 0; r < R + 4; ++r) win[r] = xp[r * (kXP / 2)];
+                    for (int r = 0; r < R + 4; ++r)
+                        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];"
+                                     : "=f"(win[r].x), "=f"(win[r].y) : "r"(xw + (uint32_t)(r * kXP * 4)));
                     float2 A1[R], B1[R], A2[R], B2[R];
                     const float2 neg1 = make_float2(-1.f, -1.f);
 #pragma unroll
