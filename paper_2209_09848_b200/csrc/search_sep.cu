@@ -134,7 +134,7 @@ struct SepCfg {
     // register split: setmaxnreg moves registers between the warpgroups of the CTA, the total stays
     // what the launch allocated (NT x the per-thread count ptxas derives from __launch_bounds__)
     static constexpr int LREGS = 65536 / NT / 8 * 8;
-    static constexpr int PREGS = 56;
+    static constexpr int PREGS = 80;
     static constexpr int CREGS_RAW = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
     static constexpr int CREGS = CREGS_RAW > 232 ? 232 : CREGS_RAW;
     static_assert(CW % 4 == 0 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * LREGS, "register budget");
@@ -326,7 +326,8 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         // frames at the same time and never synchronise with each other; the per-frame costs (two
         // mbarrier waits, the table row, the hand-over) are paid once per warp and frame.
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::PREGS));
-        static_assert(XR == kPW && SB == 2 * kPW, "one X buffer and two box stages per producer warp");
+        static_assert(XR % kPW == 0 && SB % kPW == 0, "whole X buffers and box stages per producer warp");
+        constexpr int BST = SB / kPW, XST = XR / kPW;       // box stages and X buffers of one producer warp
         const int32_t pw = warp - CW;
         // position of this warp's next frame to REQUEST (iss_*) and to PROCESS (item, t) in the CTA's
         // sequence of (work item, frame)
@@ -340,7 +341,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         auto iss_one = [&]() {          // lane 0: request frame (iss_item, iss_t) into this warp's stage iss_k & 1
             const int32_t b = iss_item % a.n_batches, tile = a.ty0 * ntx + iss_item / a.n_batches;
             const int32_t *row = reinterpret_cast<const int32_t *>(a.stage_tab + ((int64_t)b * T + iss_t) * TABW);
-            const int32_t sb = pw + kPW * (iss_k & 1), n = pw + kPW * iss_k;
+            const int32_t sb = pw + kPW * (iss_k % BST), n = pw + kPW * iss_k;
             TNO_CHECK(iss_item >= 0 && iss_item < n_items && iss_t >= 0 && iss_t < T && b < a.n_batches);
             TNO_CHECK(sb >= 0 && sb < SB && ((__ldg(row) & 3) == 0) && (uint32_t)__ldg(row + 1) < 4u);
             TNO_CHECK(tile / ntx < a.ty0 + nty && tile % ntx < ntx);
@@ -351,17 +352,17 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         };
         if (lane == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            for (int f = 0; f < 2 && iss_item < n_items; ++f) {
+            for (int f = 0; f < BST && iss_item < n_items; ++f) {
                 iss_one();
                 ++iss_k;
                 advance(iss_item, iss_t);
             }
         }
-        iss_k = 2;          // (all lanes keep the same counters; only lane 0 issues)
+        iss_k = BST;        // (all lanes keep the same counters; only lane 0 issues)
         {
             int32_t ii = blockIdx.x, tt = pw;
             while (tt >= T) { tt -= T; ii += gridDim.x; }
-            advance(ii, tt); advance(ii, tt);
+            for (int f = 0; f < BST; ++f) advance(ii, tt);
             iss_item = ii; iss_t = tt;
         }
         // x-pass roles: a quarter-warp takes 8 rows at one offset of 8 columns: 32 distinct banks for the
@@ -373,16 +374,16 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             const int32_t Y0 = (a.ty0 + item / a.n_batches / ntx) * HT - 2;
             // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
             const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
-            const int32_t sb = pw + kPW * (k & 1), n = pw + kPW * k;
-            mbar_wait(full_box + 8 * (sb), (k >> 1) & 1);
-            if (k >= 1) mbar_wait(x_empty + 8 * (pw), (k + 1) & 1);
+            const int32_t sb = pw + kPW * (k % BST), xb = pw + kPW * (k % XST), n = pw + kPW * k;
+            mbar_wait(full_box + 8 * (sb), (k / BST) & 1);
+            if (k >= XST) mbar_wait(x_empty + 8 * (xb), (k / XST + 1) & 1);
             const float *tb = Tab + (n & (TS - 1)) * TABW;
             const int32_t o = reinterpret_cast<const int32_t *>(tb)[1];
             float g[5];
 #pragma unroll
             for (int i = 0; i < 5; ++i) g[i] = tb[4 + i];
             const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 8 * oct_in;
-            float *dst = Xbuf + pw * C::XBUF + row_in * kXP + 8 * oct_in;
+            float *dst = Xbuf + xb * C::XBUF + row_in * kXP + 8 * oct_in;
             TNO_CHECK(xrows >= 4 + R && xrows <= C::XROWS && (uint32_t)o < 4u && sb < SB);
             TNO_CHECK((xrows + 7) / 8 * 8 * kBoxW <= C::RBUF + 8 * kBoxW);      // loads stay inside the staging ring
             const int32_t nfull = xrows >> 3;                       // row groups with all 8 rows
@@ -395,9 +396,9 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             }
             __syncwarp();
             if (lane == 0) {
-                mbar_arrive(x_full + 8 * (pw));
-                // this warp is done with box stage sb: request its frame after next into it
-                if (iss_item < n_items) { iss_k = k + 2; iss_one(); }
+                mbar_arrive(x_full + 8 * (xb));
+                // this warp is done with box stage sb: request the frame that uses it next
+                if (iss_item < n_items) { iss_k = k + BST; iss_one(); }
             }
             advance(iss_item, iss_t);
             advance(item, t);
@@ -650,7 +651,7 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
 // (rows per thread, slots per batch, consumer warps, box stages, X buffers): tiles of CW x R positions x 64
 // columns.  A slot costs 4 R accumulator registers (E and O, two columns), the window and its sums and
 // differences 2 (R + 4) + 8 R.
-using V0 = SepCfg<4, 5, 12, 8, 4>;
+using V0 = SepCfg<4, 5, 12, 4, 8>;
 // (measured alternatives: 8 consumer warps x 6 rows is 4-10 % slower on every config)
 
 int32_t sep_num_variants() { return 1; }
