@@ -338,16 +338,24 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         };
         while (iss_t >= T) { iss_t -= T; iss_item += gridDim.x; }
         int32_t item = iss_item, t = iss_t;
-        auto iss_one = [&]() {          // lane 0: request frame (iss_item, iss_t) into this warp's stage iss_k & 1
-            const int32_t b = iss_item % a.n_batches, tile = a.ty0 * ntx + iss_item / a.n_batches;
+        // (the divisions that split a work item into batch and tile are redone only when the item changes)
+        int32_t iss_cached = -1, iss_b = 0, iss_x0 = 0, iss_y0 = 0;
+        auto iss_one = [&]() {          // lane 0: request frame (iss_item, iss_t) into this warp's next box stage
+            if (iss_item != iss_cached) {
+                iss_cached = iss_item;
+                iss_b = iss_item % a.n_batches;
+                const int32_t tl = a.ty0 * ntx + iss_item / a.n_batches;
+                iss_x0 = (tl % ntx) * kTileW;
+                iss_y0 = (tl / ntx) * HT - 4;
+            }
+            const int32_t b = iss_b;
             const int32_t *row = reinterpret_cast<const int32_t *>(a.stage_tab + ((int64_t)b * T + iss_t) * TABW);
             const int32_t sb = pw + kPW * (iss_k % BST), n = pw + kPW * iss_k;
             TNO_CHECK(iss_item >= 0 && iss_item < n_items && iss_t >= 0 && iss_t < T && b < a.n_batches);
             TNO_CHECK(sb >= 0 && sb < SB && ((__ldg(row) & 3) == 0) && (uint32_t)__ldg(row + 1) < 4u);
-            TNO_CHECK(tile / ntx < a.ty0 + nty && tile % ntx < ntx);
+            TNO_CHECK(iss_y0 + 4 < (a.ty0 + nty) * HT && iss_x0 < ntx * kTileW);
             mbar_expect_tx(full_box + 8 * (sb), C::BOX_BYTES + TABW * 4);
-            tma_load_3d(Rbuf + sb * C::RBUF, &map, (tile % ntx) * kTileW + __ldg(row), (tile / ntx) * HT - 4, iss_t,
-                        full_box + 8 * (sb));
+            tma_load_3d(Rbuf + sb * C::RBUF, &map, iss_x0 + __ldg(row), iss_y0, iss_t, full_box + 8 * (sb));
             bulk_load(Tab + (n & (TS - 1)) * TABW, row, TABW * 4, full_box + 8 * (sb));
         };
         if (lane == 0) {
@@ -370,10 +378,14 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         // per step (8 outputs per thread from 16 staged values) and walks 2 halves x ceil(rows / 8) row
         // groups per frame.
         const int32_t row_in = lane & 7, oct_in = lane >> 3;
+        int32_t cached = -1, xrows = 0;
         for (int32_t k = 0; item < n_items; ++k) {
-            const int32_t Y0 = (a.ty0 + item / a.n_batches / ntx) * HT - 2;
-            // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
-            const int32_t xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
+            if (item != cached) {
+                cached = item;
+                const int32_t Y0 = (a.ty0 + item / a.n_batches / ntx) * HT - 2;
+                // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
+                xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
+            }
             const int32_t sb = pw + kPW * (k % BST), xb = pw + kPW * (k % XST), n = pw + kPW * k;
             mbar_wait(full_box + 8 * (sb), (k / BST) & 1);
             if (k >= XST) mbar_wait(x_empty + 8 * (xb), (k / XST + 1) & 1);
