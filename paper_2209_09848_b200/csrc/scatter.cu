@@ -610,20 +610,6 @@ k_reduce_op(const double *__restrict__ partials, int32_t n, int32_t op, int32_t 
         else if (op == kBeta) sc[2] = alpha[i] - rho[i] * s;                           // r += (alpha_i - beta) s_i
     }
 }
-// z = x + (float)coef[0] * y   (z may alias x or y); four elements per thread when n4 > 0 (n = 4 n4, aligned)
-__global__ void __launch_bounds__(256)
-k_axpy_dev(const float *x, const double *__restrict__ coef, const float *y, int64_t n, int64_t n4, float *z) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const float c = (float)coef[0];
-    if (n4 > 0) {
-        if (i < n4) {
-            const float4 a = reinterpret_cast<const float4 *>(x)[i], b = reinterpret_cast<const float4 *>(y)[i];
-            reinterpret_cast<float4 *>(z)[i] = make_float4(a.x + c * b.x, a.y + c * b.y, a.z + c * b.z, a.w + c * b.w);
-        }
-    } else if (i < n) {
-        z[i] = x[i] + c * y[i];
-    }
-}
 // z = a x + b y   (z may alias x or y)
 __global__ void __launch_bounds__(256)
 k_axpby(float a, const float *x, float b, const float *y, int64_t n, int64_t n4, float *z) {
@@ -641,6 +627,99 @@ k_axpby(float a, const float *x, float b, const float *y, int64_t n, int64_t n4,
     } else if (i < n) {
         z[i] = a * x[i] + (b != 0.f ? b * y[i] : 0.f);
     }
+}
+
+// Reduction tail shared by the fused kernels below: every block leaves its partial sum(s) in partials[block] (and
+// partials[grid + block]), the block that arrives last (a ticket counter, reset for the next launch) adds them up in
+// index order -- the same tree whatever the arrival order, so the result is reproducible -- and applies the recursion's
+// formula like k_reduce_op.
+__device__ __forceinline__ void last_block_reduce(double v0, double v1, int32_t two, double *partials,
+                                                  unsigned int *ticket, int32_t op, int32_t i, double *sc) {
+    __shared__ double sh0[8], sh1[8];
+    __shared__ double tr0[256], tr1[256];
+    __shared__ bool last;
+    for (int o = 16; o > 0; o >>= 1) {
+        v0 += __shfl_down_sync(0xffffffffu, v0, o);
+        v1 += __shfl_down_sync(0xffffffffu, v1, o);
+    }
+    if ((threadIdx.x & 31) == 0) { sh0[threadIdx.x >> 5] = v0; sh1[threadIdx.x >> 5] = v1; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { a += sh0[w]; b += sh1[w]; }
+        partials[blockIdx.x] = a;
+        if (two) partials[gridDim.x + blockIdx.x] = b;
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double a = 0.0, b = 0.0;
+    for (int32_t k = threadIdx.x; k < (int32_t)gridDim.x; k += 256) {
+        a += __ldcg(partials + k);
+        if (two) b += __ldcg(partials + gridDim.x + k);
+    }
+    tr0[threadIdx.x] = a; tr1[threadIdx.x] = b;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) { tr0[threadIdx.x] += tr0[threadIdx.x + o]; tr1[threadIdx.x] += tr1[threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        *ticket = 0;
+        const double s = tr0[0];
+        double *rho = sc + 8, *alpha = sc + 8 + kScatterHistory;
+        if (op == kStore0) { sc[0] = s; if (two) sc[1] = tr1[0]; }
+        else if (op == kAlpha) { alpha[i] = rho[i] * s; sc[2] = -alpha[i]; }          // q -= alpha_i y_i
+        else if (op == kBeta) sc[2] = alpha[i] - rho[i] * s;                           // r += (alpha_i - beta) s_i
+    }
+}
+// One step of the two-loop recursion in one pass: out = scale * (in + (float)sc[2] * v)  (v == NULL: out = scale * in),
+// then the dot product of out with w, reduced and turned into the next coefficient by the last block.
+__global__ void __launch_bounds__(256)
+k_update_dot(const float *in, const float *v, float scale, const float *__restrict__ w, int64_t n, int64_t n4,
+             float *out, double *partials, unsigned int *ticket, int32_t op, int32_t i, double *sc) {
+    const float c = v ? (float)sc[2] : 0.f;
+    double acc = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n4 > 0) {
+        for (int64_t k = id; k < n4; k += stride) {
+            float4 a = reinterpret_cast<const float4 *>(in)[k];
+            if (v) {
+                const float4 b = reinterpret_cast<const float4 *>(v)[k];
+                a = make_float4(a.x + c * b.x, a.y + c * b.y, a.z + c * b.z, a.w + c * b.w);
+            }
+            a = make_float4(scale * a.x, scale * a.y, scale * a.z, scale * a.w);
+            reinterpret_cast<float4 *>(out)[k] = a;
+            const float4 q = reinterpret_cast<const float4 *>(w)[k];
+            acc += (double)a.x * q.x + (double)a.y * q.y + (double)a.z * q.z + (double)a.w * q.w;
+        }
+    } else {
+        for (int64_t k = id; k < n; k += stride) {
+            float a = in[k];
+            if (v) a = a + c * v[k];
+            a = scale * a;
+            out[k] = a;
+            acc += (double)a * (double)w[k];
+        }
+    }
+    last_block_reduce(acc, 0.0, 0, partials, ticket, op, i, sc);
+}
+// The new pair in one pass: s = xn - x, y = gn - g, and both s.y -> sc[0] and y.y -> sc[1]
+__global__ void __launch_bounds__(256)
+k_pair(const float *__restrict__ xn, const float *__restrict__ x, const float *__restrict__ gn, const float *__restrict__ g,
+       int64_t n, float *__restrict__ s_out, float *__restrict__ y_out, double *partials, unsigned int *ticket,
+       double *sc) {
+    double sy = 0.0, yy = 0.0;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        const float sv = xn[k] - x[k], yv = gn[k] - g[k];
+        s_out[k] = sv;
+        y_out[k] = yv;
+        sy += (double)sv * (double)yv;
+        yy += (double)yv * (double)yv;
+    }
+    last_block_reduce(sy, yy, 1, partials, ticket, kStore0, 0, sc);
 }
 
 // VEC: four neighbouring pixels per thread (W % 4 == 0, 16-byte aligned frames)
@@ -790,6 +869,8 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
     double *partials = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(psi + (size_t)pb.T * pb.N * pb.N) + 15) &
                                                   ~(uintptr_t)15);
     double *scal = partials + blocks;            // 8 + 2 * kScatterHistory doubles (k_reduce_op)
+    unsigned int *ticket = reinterpret_cast<unsigned int *>(scal + 6);       // scal[6] is not used as a scalar
+    cudaMemsetAsync(ticket, 0, 8, st);
     int32_t launches = 0, evals = 0;
     cudaError_t err = cudaSuccess;
     auto fetch = [&](double *dev) -> double {
@@ -815,10 +896,6 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
         k_axpby<<<vgrid, 256, 0, st>>>(a, xx, b, yy, P, P4, zz);
         launches += 1;
     };
-    auto axpy_dev = [&](const float *xx, const float *yy, float *zz) {                // zz = xx + sc[2] * yy
-        k_axpy_dev<<<vgrid, 256, 0, st>>>(xx, scal + 2, yy, P, P4, zz);
-        launches += 1;
-    };
     auto eval = [&](const float *xx, float *gg) -> double {
         launches += scatter_lossgrad(st, pb, xx, xx + nb, psi, partials, gg, gg + nb, scal + 1);
         ++evals;
@@ -834,20 +911,26 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
         k_absmax<<<kRedBlocks, 256, 0, st>>>(g, P, partials);
         k_sum_partials<<<1, 256, 0, st>>>(partials, kRedBlocks, 1, scal + 3);
         launches += 2;
-        // d = H g by the two-loop recursion, every scalar of it on the device
-        axpby(1.f, g, 0.f, g, d);
-        for (int32_t c = 0; c < hist; ++c) {
-            const int32_t i = (head - 1 - c + 2 * kScatterHistory) % kScatterHistory;
-            dot_to(hs + (size_t)i * P, d, kAlpha, i);
-            axpy_dev(d, hy + (size_t)i * P, d);
+        // d = H g by the two-loop recursion, every scalar of it on the device.  Each step is ONE launch: the vector
+        // update that the previous coefficient calls for, fused with the dot product that yields the next one.
+        auto slot = [&](int32_t c) { return (head - 1 - c + 2 * kScatterHistory) % kScatterHistory; };
+        auto step_dot = [&](const float *in, const float *v, float scale, const float *w, int32_t op, int32_t i) {
+            k_update_dot<<<kRedBlocks, 256, 0, st>>>(in, v, scale, w, P, P4, d, partials, ticket, op, i, scal);
+            launches += 1;
+        };
+        if (hist == 0) {
+            step_dot(g, nullptr, 1.f, g, kStore0, 0);                                   // d = g, g.d
+        } else {
+            step_dot(g, nullptr, 1.f, hs + (size_t)slot(0) * P, kAlpha, slot(0));      // d = g, alpha of the newest pair
+            for (int32_t c = 1; c < hist; ++c)                                          // d -= alpha y (previous pair)
+                step_dot(d, hy + (size_t)slot(c - 1) * P, 1.f, hs + (size_t)slot(c) * P, kAlpha, slot(c));
+            // d = gamma (d - alpha y) of the oldest pair, then the second loop from the oldest pair up
+            step_dot(d, hy + (size_t)slot(hist - 1) * P, (float)gamma[(head - 1 + kScatterHistory) % kScatterHistory],
+                     hy + (size_t)slot(hist - 1) * P, kBeta, slot(hist - 1));
+            for (int32_t c = hist - 2; c >= 0; --c)                                     // d += (alpha - beta) s (previous pair)
+                step_dot(d, hs + (size_t)slot(c + 1) * P, 1.f, hy + (size_t)slot(c) * P, kBeta, slot(c));
+            step_dot(d, hs + (size_t)slot(0) * P, 1.f, g, kStore0, 0);                  // last update, g.d
         }
-        if (hist > 0) axpby((float)gamma[(head - 1 + kScatterHistory) % kScatterHistory], d, 0.f, d, d);
-        for (int32_t c = hist - 1; c >= 0; --c) {
-            const int32_t i = (head - 1 - c + 2 * kScatterHistory) % kScatterHistory;
-            dot_to(hy + (size_t)i * P, d, kBeta, i);
-            axpy_dev(d, hs + (size_t)i * P, d);
-        }
-        dot_to(g, d, kStore0, 0);
         double h4[4];                            // one read-back per direction: g.d and |g|_inf
         {
             cudaError_t e = cudaMemcpyAsync(h4, scal, 32, cudaMemcpyDeviceToHost, st);
@@ -874,10 +957,8 @@ int32_t scatter_fit(cudaStream_t st, const ScatterProblem &pb, float *beta, floa
         if (!ok) break;
         // s = xn - x, y = gn - g into the history slot
         float *s_new = hs + (size_t)head * P, *y_new = hy + (size_t)head * P;
-        axpby(1.f, xn, -1.f, x, s_new);
-        axpby(1.f, gn, -1.f, g, y_new);
-        dot_to(s_new, y_new, kStore0, 0);
-        dot_to(y_new, y_new, kStore1, 0);
+        k_pair<<<kRedBlocks, 256, 0, st>>>(xn, x, gn, g, P, s_new, y_new, partials, ticket, scal);
+        launches += 1;
         double h2[2];
         {
             cudaError_t e = cudaMemcpyAsync(h2, scal, 16, cudaMemcpyDeviceToHost, st);
