@@ -331,16 +331,21 @@ k_scatter_fused(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, co
     const int32_t j = tid * PX;
     const int32_t i1 = rb;
     const float wy = bw[i];
-    int32_t o0[PX], dj[PX];
-    float wx[PX];
+    // per pixel: the four bilinear weights (the products of k_scatter_resid, formed once) and the places of the four
+    // values of S_t in the staged rows of stage 0, frame 0 (row ra of S_t is row 0 of the staged rows)
+    float w00[PX], w01[PX], w10[PX], w11[PX];
+    const float *s00[PX], *s01[PX], *s10[PX], *s11[PX];
+    const int32_t di = (i1 - ra) * n;
 #pragma unroll
     for (int k = 0; k < PX; ++k) {
-        const int32_t j0 = bi0[j + k];
-        o0[k] = j0;                                              // row ra of S_t is row 0 of the staged rows
-        dj[k] = min(j0 + 1, n - 1) - j0;
-        wx[k] = bw[j + k];
+        const int32_t j0 = bi0[j + k], dj = min(j0 + 1, n - 1) - j0;
+        const float wx = bw[j + k];
+        w00[k] = (1.f - wy) * (1.f - wx); w01[k] = (1.f - wy) * wx; w10[k] = wy * (1.f - wx); w11[k] = wy * wx;
+        s00[k] = ring + FS * (PXF + 8) + j0;
+        s01[k] = s00[k] + dj;
+        s10[k] = s00[k] + di;
+        s11[k] = s10[k] + dj;
     }
-    const int32_t di = (i1 - ra) * n;
     float b[6][PX], g[6][PX];
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
@@ -350,40 +355,49 @@ k_scatter_fused(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, co
     }
     double loss = 0.0;
     uint32_t st = 0, par = 0;
+    // one frame of the stage at offset so (floats) for this thread's two pixels; returns the clipped residuals
+    auto frame = [&](const float *sp, int32_t so, int f, float &lsum, float (&c4)[PX]) {
+        const float2 dv = reinterpret_cast<const float2 *>(sp + f * PXF)[tid];
+        const float4 qa = *reinterpret_cast<const float4 *>(sp + FS * PXF + f * 8);
+        const float2 qb = *reinterpret_cast<const float2 *>(sp + FS * PXF + f * 8 + 4);
+        const float q[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
+        const float d4[PX] = {dv.x, dv.y};
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+            const int32_t o = so + f * SF;
+            // the same expression as k_scatter_resid: four weights times four values
+            float pred = w00[k] * s00[k][o] + w01[k] * s01[k][o] + w10[k] * s10[k][o] + w11[k] * s11[k][o];
+#pragma unroll
+            for (int m = 0; m < 6; ++m) pred = fmaf(q[m], b[m][k], pred);
+            const float r = d4[k] - pred;
+            const float c = fminf(fmaxf(r, -delta), delta);
+            lsum = fmaf(c, r - 0.5f * c, lsum);        // Eq. 4: c (r - c/2) = r^2/2 inside, delta (|r| - delta/2) outside
+            c4[k] = c;
+#pragma unroll
+            for (int m = 0; m < 6; ++m) g[m][k] = fmaf(q[m], c, g[m][k]);
+        }
+    };
     for (int32_t t0 = ta; t0 < tb; t0 += FS) {
         sc_wait(full + 8 * st, par);
         const float *sp = ring + st * STAGE;
+        const int32_t so = (int32_t)st * STAGE;
         float lsum = 0.f;
+        if (t0 + FS <= tb) {                      // a full stage: no per-frame test
 #pragma unroll
-        for (int f = 0; f < FS; ++f) {
-            float c4[PX] = {0.f, 0.f};
-            if (t0 + f < tb) {
-                const float2 dv = reinterpret_cast<const float2 *>(sp + f * PXF)[tid];
-                const float4 qa = *reinterpret_cast<const float4 *>(sp + FS * PXF + f * 8);
-                const float2 qb = *reinterpret_cast<const float2 *>(sp + FS * PXF + f * 8 + 4);
-                const float q[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
-                const float d4[PX] = {dv.x, dv.y};
-                const float *St = sp + FS * (PXF + 8) + f * SF;
-#pragma unroll
-                for (int k = 0; k < PX; ++k) {
-                    const float a00 = St[o0[k]], a01 = St[o0[k] + dj[k]];
-                    const float a10 = St[o0[k] + di], a11 = St[o0[k] + di + dj[k]];
-                    // the same expression as k_scatter_resid: four weights times four values
-                    float pred = (1.f - wy) * (1.f - wx[k]) * a00 + (1.f - wy) * wx[k] * a01 + wy * (1.f - wx[k]) * a10 +
-                                 wy * wx[k] * a11;
-#pragma unroll
-                    for (int m = 0; m < 6; ++m) pred = fmaf(q[m], b[m][k], pred);
-                    const float r = d4[k] - pred;
-                    const float a = fabsf(r);
-                    lsum += a <= delta ? 0.5f * r * r : delta * (a - 0.5f * delta);       // Eq. 4
-                    const float c = fminf(fmaxf(r, -delta), delta);
-                    c4[k] = c;
-#pragma unroll
-                    for (int m = 0; m < 6; ++m) g[m][k] = fmaf(q[m], c, g[m][k]);
-                }
+            for (int f = 0; f < FS; ++f) {
+                float c4[PX];
+                frame(sp, so, f, lsum, c4);
+                prow[f * PP + j] = c4[0];
+                prow[f * PP + j + 1] = c4[1];
             }
-            prow[f * PP + j] = c4[0];
-            prow[f * PP + j + 1] = c4[1];
+        } else {
+#pragma unroll
+            for (int f = 0; f < FS; ++f) {
+                float c4[PX] = {0.f, 0.f};
+                if (t0 + f < tb) frame(sp, so, f, lsum, c4);
+                prow[f * PP + j] = c4[0];
+                prow[f * PP + j + 1] = c4[1];
+            }
         }
         loss += (double)lsum;
         // the stage's data is consumed: hand it back, then reduce the psi rows along the columns
