@@ -273,6 +273,53 @@ def test_results_are_reproducible_and_independent_of_the_bank():
     assert np.array_equal(a[sub], c)
 
 
+def test_mirror_pairs_edge_cases():
+    """Slots of the separable kernel: pairs (+-vy, +-ay), a pair with exact half-pixel ties
+    (must NOT share a slot: floor(-d + 1/2) != -floor(d + 1/2) there), duplicates, a lone negative motion, vy = 0 with
+    and without acceleration, six slots of one x-motion (two batches).  Every map against the oracle, and every
+    trajectory alone gives the same bits as inside the bank -- with or without its mirror image next to it."""
+    torch = _torch()
+    T, H, W = 90, 100, 128
+    f, sigma = _bank_case(T, H, W, 29)
+    traj = np.array([[0.3, 0.2, 0, 0], [0.3, -0.2, 0, 0],            # a pair
+                     [0.3, 0.5, 0, 0], [0.3, -0.5, 0, 0],            # exact ties at odd dt: two single slots
+                     [0.3, 0.2, 0, 0],                               # duplicate of the first
+                     [0.3, 0.11, 0, 0.002], [0.3, -0.11, 0, -0.002],  # a pair with acceleration
+                     [0.3, -0.37, 0, 0.001],                         # lone minus member (its mirror is not in the bank)
+                     [0.3, 0.0, 0, 0], [0.3, 0.0, 0, 0.003], [0.3, 0.0, 0, -0.003],   # vy = 0
+                     [-0.1, -0.45, 0, 0], [-0.1, 0.45, 0, 0]], np.float32)            # a second x-motion
+    t0 = 45.0
+    import paper_2209_09848_b200 as P
+    n, batch, slot, member = P.tno_mf_plan_slots(traj, T, t0)
+    assert slot[0] == slot[1] and member[0] == 0 and member[1] == 1
+    assert (batch[2], slot[2]) != (batch[3], slot[3]) and member[2] == 0 and member[3] == 0      # ties: not paired
+    assert member[7] == 1 and (batch[9], slot[9]) == (batch[10], slot[10])
+    om = oracle.snr_map(f, sigma, traj, 1.0, t0)
+    d = torch.from_numpy(f).cuda()
+    gm, gc, stats = run_gpu(d, sigma, traj, 1.0, t0, 6, 3.0)
+    assert stats[1] == 1
+    err = np.abs(gm.astype(np.float64) - om)
+    assert err.max() <= TOL, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    for k in range(traj.shape[0]):
+        check_topk(gc[k], om[k], k, 6, 3.0)
+        check_topk_vs_own_map(gc[k], gm[k], k, 6, 3.0)
+    assert np.array_equal(gm[0], gm[4])                            # duplicates: equal bits
+    for k in (0, 1, 3, 6, 7, 10, 12):                              # alone = inside the bank, bit for bit
+        alone, _, _ = run_gpu(d, sigma, traj[k:k + 1], 1.0, t0, 6, 3.0)
+        assert np.array_equal(alone[0], gm[k]), k
+    # y-jitter breaks the mirror symmetry: no pairs, same answers as the oracle
+    jit = np.zeros((T, 2), np.float32)
+    jit[:, 1] = 0.3 * np.sin(np.arange(T) / 7.0)
+    assert np.all(P.tno_mf_plan_slots(traj, T, t0, jitter_xy=jit)[3] == 0)
+    om_j = oracle.snr_map(f, sigma, traj, 1.0, t0, jitter=jit)
+    from paper_2209_09848_b200 import MatchedFilter
+    with MatchedFilter(0) as mf:
+        mj, _ = mf.search(d, sigma, traj, 1.0, t0, jitter_xy=jit)
+        torch.cuda.synchronize()
+        assert mf.stats()[1] == 1
+        assert np.abs(mj.cpu().numpy().astype(np.float64) - om_j).max() <= TOL
+
+
 @pytest.mark.timeout(180)
 def test_many_work_items_per_cta_with_early_flushes():
     """More (tile, batch) work items than SMs, so every CTA walks several items, with trajectories whose
