@@ -87,10 +87,13 @@ typedef struct {
                                 3 = tabulated separable PRF, see tno_mf_set_prf_table; prf_sigma is ignored;
                                 4 = tabulated non-separable PRF, see tno_mf_set_prf_table2d; prf_sigma is ignored.
                                 In modes 2, 3 and 4 tno_mf_inject renders sources with the same taps. */
+    int32_t sep_shape;       /* 0 = the separable kernel picks its shape by modelled cost (normal use): 4 positions per
+                                thread x 5 slots per batch (tiles of 48 rows) or 5 x 4 (tiles of 60 rows);
+                                1 / 2 = always the first / second shape -- for tests.  Same results up to rounding. */
 } tno_mf_config;
 
 /* Create a context on cfg->device.  Errors: EINVAL (NULL pointers, topk < 0, NaN threshold,
- * workspace_limit_mb < 0, filter not 0 .. 4), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
+ * workspace_limit_mb < 0, filter not 0 .. 4, sep_shape not 0 .. 2), EUNSUPPORTED (no CUDA device / not compute capability 10.x), ECUDA, ENOMEM. */
 int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
 
 /* The search (formula above).
@@ -105,11 +108,14 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx);
  * arithmetic, n_traj > 65535, H * W > 2^31, H > 262140 rows -- the same row limit holds for every call
  * that takes frames or maps), ENOMEM, ECUDA.
  * Any H, W >= 1 is computed correctly; the TMA kernel needs W % 4 == 0 and 16-byte aligned
- * frames (and y-shift ranges below 63 tile heights of 60 px), other inputs take the generic kernel.
+ * frames (and y-shift ranges below 63 tile heights of 48 / 60 px), other inputs take the generic kernel.
  * The TMA kernel accumulates into a context-owned partial-sum workspace of (1 + ceil(y-shift range /
- * 60)) * n_traj * H * W floats, capped (cfg.workspace_limit_mb); a larger bank is searched in chunks
- * of whole batches with identical results.  Results are bitwise reproducible, and the map of a
- * trajectory does not depend on the other trajectories of the call.  All element offsets are 64-bit. */
+ * tile height)) * n_traj * H * W floats, capped (cfg.workspace_limit_mb); a larger bank is searched in chunks
+ * of whole batches with identical results.  Results are bitwise reproducible, and for a given kernel
+ * shape the map of a trajectory does not depend on the other trajectories of the call; with
+ * cfg.sep_shape = 0 the shape (tile height 48 or 60) is picked per call from the bank and the frame
+ * size, and the two shapes sum in different orders (differences of a few float32 ulps): pin
+ * cfg.sep_shape to compare maps bit for bit across banks.  All element offsets are 64-bit. */
 int tno_mf_search(tno_mf_ctx *ctx,
                   const float *frames, int32_t T, int32_t H, int32_t W,
                   const float *sigma_t,

@@ -30,7 +30,7 @@ class tno_mf_config(ctypes.Structure):
     _fields_ = [("device", ctypes.c_int32), ("stream", ctypes.c_void_p), ("topk", ctypes.c_int32),
                 ("snr_threshold", ctypes.c_float), ("force_generic", ctypes.c_int32),
                 ("record_events", ctypes.c_int32), ("workspace_limit_mb", ctypes.c_int32),
-                ("filter", ctypes.c_int32)]
+                ("filter", ctypes.c_int32), ("sep_shape", ctypes.c_int32)]
 
 
 class TnoMfError(RuntimeError):
@@ -126,12 +126,12 @@ def tno_mf_last_error(ctx=None) -> str:
 def tno_mf_create(device: int = 0, stream: Optional[int] = None, topk: int = 0,
                   snr_threshold: float = float("-inf"), force_generic: bool = False,
                   record_events: bool = False, workspace_limit_mb: int = 0, shift_stack: bool = False,
-                  filter: int = 0):
+                  filter: int = 0, sep_shape: int = 0):
     """Returns an opaque context handle.  `stream` is a raw cudaStream_t (int) or None."""
     cfg = tno_mf_config(device=int(device), stream=ctypes.c_void_p(stream or 0), topk=int(topk),
                         snr_threshold=float(snr_threshold), force_generic=int(bool(force_generic)),
                         record_events=int(bool(record_events)), workspace_limit_mb=int(workspace_limit_mb),
-                        filter=int(filter) if filter else int(bool(shift_stack)))
+                        filter=int(filter) if filter else int(bool(shift_stack)), sep_shape=int(sep_shape))
     ctx = ctypes.c_void_p()
     _check(_lib.tno_mf_create(ctypes.byref(cfg), ctypes.byref(ctx)), None)
     _CTX_TOPK[ctx.value] = int(topk)            # the binding checks the size of out_topk buffers against it

@@ -32,7 +32,6 @@ struct tno_mf_ctx {
     void *encode_fn = nullptr;
     std::string err;
     int32_t last_launches = 0, last_kernel = 0;
-    int32_t sep_variant = 0;          // kernel shape of the separable search (search_sep.cu)
     // host-fed search (tno_mf_search_host): rows [0, fed_rows) of every frame are on the device
     const float *feed_host = nullptr, *feed_host2 = nullptr;      // feed_host2: the validity weights of a masked search
     float *feed_dev = nullptr, *feed_dev2 = nullptr;
@@ -199,8 +198,10 @@ int tno_mf_create(const tno_mf_config *cfg, tno_mf_ctx **out_ctx) {
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: topk must be in [0, %d]", kMaxTopk);
     if (std::isnan(cfg->snr_threshold))
         return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: snr_threshold is NaN");
-    if (cfg->filter < 0 || cfg->filter > 4 || cfg->workspace_limit_mb < 0)
-        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 .. 4 and workspace_limit_mb >= 0");
+    if (cfg->filter < 0 || cfg->filter > 4 || cfg->workspace_limit_mb < 0 || cfg->sep_shape < 0 ||
+        cfg->sep_shape > sep_num_variants())
+        return fail(nullptr, TNO_MF_EINVAL, "tno_mf_create: filter must be 0 .. 4, workspace_limit_mb >= 0, sep_shape 0 .. %d",
+                    sep_num_variants());
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess || n_dev == 0) {
@@ -824,9 +825,26 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
     if (use_sep) {
         // slots (mirror pairs where the filter is symmetric under y -> -y: the Gaussian and the single tap)
         // packed into batches; both kernel variants take the same batches
-        variant = ctx->sep_variant;
+        // kernel shape: the one with the shorter modelled makespan.  A (tile, batch) work item costs, per frame and in
+        // issue cycles of a scheduler, tile_h / rows-per-warp ... folded into: tile_h x [ 14.5 (tile_h + 4) / tile_h for
+        // the x-pass + 2 (5 slots + 4) for the y-pass + 93 / rows of per-frame bookkeeping per consumer warp ]
+        // (DESIGN.md section 6); the persistent CTAs take ceil(items / SMs) items each.  Ties go to shape 0.
+        const bool sym = ctx->cfg.filter == 0 || ctx->cfg.filter == 1;
+        double best = 0.0;
+        for (int32_t v = 0; v < sep_num_variants(); ++v) {
+            const SepVariant cand = sep_variant(v);
+            build_slot_batches(&plan, cand.nb, sym);
+            double per_item = 0.0;
+            for (const SlotBatch &bt : plan.slot_batches)
+                per_item += 14.5 * (cand.tile_h + 4) / cand.tile_h + 2.0 * (5.0 * bt.slots.size() + 4.0) + 93.0 / cand.rows;
+            per_item *= (double)cand.tile_h / (double)plan.slot_batches.size();
+            const double items = (double)((W + 63) / 64) * sep_tile_rows(v, H) * (double)plan.slot_batches.size();
+            const double cost = std::ceil(items / ctx->n_sm) * per_item;
+            if (variant < 0 || cost < best * (1.0 - 1e-9)) { best = cost; variant = v; }
+        }
+        if (ctx->cfg.sep_shape > 0) variant = ctx->cfg.sep_shape - 1;
         sv = sep_variant(variant);
-        build_slot_batches(&plan, sv.nb, ctx->cfg.filter == 0 || ctx->cfg.filter == 1);
+        build_slot_batches(&plan, sv.nb, sym);
         int64_t range = 0;
         for (const AxisClass &c : plan.ycls) range = std::max<int64_t>(range, (int64_t)c.smax - c.smin);
         const int64_t np = 1 + (range + sv.tile_h - 1) / sv.tile_h;

@@ -97,6 +97,7 @@ void launch_inject(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t
 struct SepVariant {
     int32_t nb;           // slots per batch (a slot = a y-motion and its mirror image, plan.h)
     int32_t tile_h;       // positions (frame rows) per tile; the tile width is 64 columns
+    int32_t rows;         // positions per consumer thread
 };
 int32_t sep_num_variants();
 SepVariant sep_variant(int32_t v);

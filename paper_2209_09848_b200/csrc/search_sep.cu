@@ -118,7 +118,7 @@ constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per
 //   [16 + 8s + 5] d_{s,t}    [16 + 8s + 6], [.. + 7] planned-order index of the plus / minus member relative
 //                            to the first one of the batch, -1 = absent
 
-template <int R_, int NB_, int CW_, int SB_, int XR_>
+template <int R_, int NB_, int CW_, int SB_, int XR_, int PREGS_ = 80>
 struct SepCfg {
     static constexpr int R = R_, NB = NB_, CW = CW_, SB = SB_, XR = XR_;      // NB = slots per batch
     static constexpr int NT = 32 * (CW + kPW);     // consumer warps 0 .. CW-1, then the producer warpgroup
@@ -134,7 +134,7 @@ struct SepCfg {
     // register split: setmaxnreg moves registers between the warpgroups of the CTA, the total stays
     // what the launch allocated (NT x the per-thread count ptxas derives from __launch_bounds__)
     static constexpr int LREGS = 65536 / NT / 8 * 8;
-    static constexpr int PREGS = 80;
+    static constexpr int PREGS = PREGS_;
     static constexpr int CREGS_RAW = (NT * LREGS - kPW * 32 * PREGS) / (CW * 32) / 8 * 8;
     static constexpr int CREGS = CREGS_RAW > 232 ? 232 : CREGS_RAW;
     static_assert(CW % 4 == 0 && (CW * 32 * CREGS + kPW * 32 * PREGS) <= NT * LREGS, "register budget");
@@ -663,23 +663,30 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
 // (rows per thread, slots per batch, consumer warps, box stages, X buffers): tiles of CW x R positions x 64
 // columns.  A slot costs 4 R accumulator registers (E and O, two columns), the window and its sums and
 // differences 2 (R + 4) + 8 R.
-using V0 = SepCfg<4, 5, 12, 4, 8>;
+using V0 = SepCfg<4, 5, 12, 4, 8>;            // tiles of 48 positions, 5 slots: banks with 5 slots per x-motion (config 3)
+using V1 = SepCfg<5, 4, 12, 4, 8, 56>;        // tiles of 60 positions, 4 slots: the per-frame bookkeeping of a warp is
+                                              // spread over 5 positions instead of 4 (config 4: 8 x 8 grid = 4 slots)
 // (measured alternatives: 8 consumer warps x 6 rows is 4-10 % slower on every config)
 
-int32_t sep_num_variants() { return 1; }
-SepVariant sep_variant(int32_t) { return SepVariant{V0::NB, V0::HT}; }
-int32_t sep_table_words(int32_t) { return V0::TABW; }
+int32_t sep_num_variants() { return 2; }
+SepVariant sep_variant(int32_t v) {
+    return v == 0 ? SepVariant{V0::NB, V0::HT, V0::R} : SepVariant{V1::NB, V1::HT, V1::R};
+}
+int32_t sep_table_words(int32_t v) { return v == 0 ? V0::TABW : V1::TABW; }
 int32_t sep_tile_rows(int32_t v, int32_t H) {
     const int32_t ht = sep_variant(v).tile_h;
     return (H + 4 + ht - 1) / ht;
 }
 
-void launch_sep_tables(cudaStream_t st, int32_t, const ClassTables &tab, const int32_t *batch_xc,
+void launch_sep_tables(cudaStream_t st, int32_t v, const ClassTables &tab, const int32_t *batch_xc,
                        const int32_t *slot_yc, const int32_t *slot_flip, const int32_t *slot_q, int32_t n_batches,
                        int32_t squared, float *stage_tab) {
     const int64_t n = (int64_t)n_batches * tab.T;
     const unsigned grid = (unsigned)((n + 127) / 128);
-    k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
+    if (v == 0)
+        k_sep_tables<V0><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
+    else
+        k_sep_tables<V1><<<grid, 128, 0, st>>>(tab, batch_xc, slot_yc, slot_flip, slot_q, n_batches, squared, stage_tab);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
@@ -732,8 +739,7 @@ static int launch_t(cudaStream_t st, const SepArgs &a, void *encode_fn, int32_t 
 
 int launch_search_sep(cudaStream_t st, int32_t v, const SepArgs &a, void *encode_fn, int32_t *grid_out,
                       const char **err) {
-    (void)v;
-    return launch_t<V0>(st, a, encode_fn, grid_out, err);
+    return v == 0 ? launch_t<V0>(st, a, encode_fn, grid_out, err) : launch_t<V1>(st, a, encode_fn, grid_out, err);
 }
 
 void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, int32_t n_pieces, int64_t piece_stride,

@@ -13,7 +13,7 @@ class MatchedFilter:
 
     def __init__(self, device: int = 0, topk: int = 0, snr_threshold: float = float("-inf"),
                  force_generic: bool = False, record_events: bool = False, workspace_limit_mb: int = 0,
-                 shift_stack: bool = False, filter: int = 0, prf_table=None):
+                 shift_stack: bool = False, filter: int = 0, prf_table=None, sep_shape: int = 0):
         """filter: tno_mf_config::filter (0 Gaussian PRF, 1 shift-stack, 2 pixel-integrated Gaussian, 3 tabulated:
         prf_table [n_phase, 5], 4 tabulated non-separable: prf_table [n_phase_y, n_phase_x, 5, 5])."""
         import torch
@@ -22,7 +22,7 @@ class MatchedFilter:
         self.topk = int(topk)
         stream = torch.cuda.current_stream(self.device).cuda_stream
         self.ctx = B.tno_mf_create(device, stream, topk, snr_threshold, force_generic, record_events,
-                                   workspace_limit_mb, shift_stack, filter)
+                                   workspace_limit_mb, shift_stack, filter, sep_shape)
         if prf_table is not None:
             if int(filter) == 4:
                 B.tno_mf_set_prf_table2d(self.ctx, prf_table)

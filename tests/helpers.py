@@ -18,11 +18,11 @@ def cpu_inputs(cfg):
 
 
 def run_gpu(frames_dev, sigma_t, traj, prf_sigma, t0, topk, threshold, want_maps=True,
-            force_generic=False):
+            force_generic=False, sep_shape=0):
     """-> (maps float32 [K,H,W] numpy or None, candidates structured [K,topk] or None, stats)."""
     import torch
     from paper_2209_09848_b200 import MatchedFilter
-    with MatchedFilter(frames_dev.device.index or 0, topk, threshold, force_generic) as mf:
+    with MatchedFilter(frames_dev.device.index or 0, topk, threshold, force_generic, sep_shape=sep_shape) as mf:
         maps, cand = mf.search(frames_dev, sigma_t, traj, prf_sigma, t0, want_maps=want_maps)
         torch.cuda.synchronize()
         stats = mf.stats()

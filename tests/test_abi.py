@@ -35,7 +35,7 @@ def test_record_sizes_match_header():
     assert binding.TRAJ_DTYPE.itemsize == 16          # 4 x float
     assert binding.CAND_DTYPE.itemsize == 16          # float + 3 x int32
     assert binding.SOURCE_DTYPE.itemsize == 28        # traj + 2 x int32 + float
-    assert ctypes.sizeof(binding.tno_mf_config) == 40
+    assert ctypes.sizeof(binding.tno_mf_config) == 48          # 9 x int32/float + one pointer, 8-byte aligned
 
 
 def test_version_and_create_argument_errors():

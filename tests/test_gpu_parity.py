@@ -256,24 +256,46 @@ def test_fast_trajectories_need_many_pieces():
         check_topk_vs_own_map(gc[k], gm[k], k, 5, 3.0)
 
 
-def test_results_are_reproducible_and_independent_of_the_bank():
+@pytest.mark.parametrize("sep_shape", [0, 1, 2])
+def test_results_are_reproducible_and_independent_of_the_bank(sep_shape):
     """Bitwise identical maps from run to run, and the map of a trajectory does not depend on which
-    other trajectories are searched with it (summation order is a function of the trajectory)."""
+    other trajectories are searched with it (summation order is a function of the trajectory and of the kernel
+    shape; with sep_shape = 0 the library picks the shape per call, here the same one for both banks)."""
     torch = _torch()
     T, H, W = 130, 96, 128
     f, sigma = _bank_case(T, H, W, 13)
     vs = np.linspace(-0.2, 0.2, 5).astype(np.float32)
     traj = np.array([[vx, vy, 0, 0] for vx in vs[:2] for vy in vs], np.float32)
     d = torch.from_numpy(f).cuda()
-    a, _, _ = run_gpu(d, sigma, traj, 1.0, 65.0, 4, 3.0)
-    b, _, _ = run_gpu(d, sigma, traj, 1.0, 65.0, 4, 3.0)
+    a, _, _ = run_gpu(d, sigma, traj, 1.0, 65.0, 4, 3.0, sep_shape=sep_shape)
+    b, _, _ = run_gpu(d, sigma, traj, 1.0, 65.0, 4, 3.0, sep_shape=sep_shape)
     assert np.array_equal(a, b)
     sub = np.array([0, 3, 7])
-    c, _, _ = run_gpu(d, sigma, traj[sub], 1.0, 65.0, 4, 3.0)
+    c, _, _ = run_gpu(d, sigma, traj[sub], 1.0, 65.0, 4, 3.0, sep_shape=sep_shape)
     assert np.array_equal(a[sub], c)
 
 
-def test_mirror_pairs_edge_cases():
+@pytest.mark.parametrize("sep_shape", [1, 2])
+@pytest.mark.parametrize("cfg_idx", [1, 2])
+def test_both_kernel_shapes_on_configs_1_and_2(cfg_idx, sep_shape):
+    """The two shapes of the separable kernel (4 positions x 5 slots, tiles of 48 rows; 5 x 4, tiles of 60 rows),
+    each forced: full maps and lists against the oracle."""
+    torch = _torch()
+    cfg = tno_synth.CONFIGS[cfg_idx]
+    p, f = cpu_inputs(cfg)
+    om = oracle.snr_map(f, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0)
+    gm, gc, stats = run_gpu(torch.from_numpy(f).cuda(), p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0, cfg.topk,
+                            cfg.threshold, sep_shape=sep_shape)
+    assert stats[1] == 1
+    err = np.abs(gm.astype(np.float64) - om)
+    assert err.max() <= TOL, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    for k in range(cfg.n_traj):
+        check_topk(gc[k], om[k], k, cfg.topk, cfg.threshold)
+        check_topk_vs_own_map(gc[k], gm[k], k, cfg.topk, cfg.threshold)
+
+
+@pytest.mark.parametrize("sep_shape", [1, 2])
+def test_mirror_pairs_edge_cases(sep_shape):
     """Slots of the separable kernel: pairs (+-vy, +-ay), a pair with exact half-pixel ties
     (must NOT share a slot: floor(-d + 1/2) != -floor(d + 1/2) there), duplicates, a lone negative motion, vy = 0 with
     and without acceleration, six slots of one x-motion (two batches).  Every map against the oracle, and every
@@ -296,7 +318,7 @@ def test_mirror_pairs_edge_cases():
     assert member[7] == 1 and (batch[9], slot[9]) == (batch[10], slot[10])
     om = oracle.snr_map(f, sigma, traj, 1.0, t0)
     d = torch.from_numpy(f).cuda()
-    gm, gc, stats = run_gpu(d, sigma, traj, 1.0, t0, 6, 3.0)
+    gm, gc, stats = run_gpu(d, sigma, traj, 1.0, t0, 6, 3.0, sep_shape=sep_shape)
     assert stats[1] == 1
     err = np.abs(gm.astype(np.float64) - om)
     assert err.max() <= TOL, (err.max(), np.unravel_index(err.argmax(), err.shape))
@@ -305,7 +327,7 @@ def test_mirror_pairs_edge_cases():
         check_topk_vs_own_map(gc[k], gm[k], k, 6, 3.0)
     assert np.array_equal(gm[0], gm[4])                            # duplicates: equal bits
     for k in (0, 1, 3, 6, 7, 10, 12):                              # alone = inside the bank, bit for bit
-        alone, _, _ = run_gpu(d, sigma, traj[k:k + 1], 1.0, t0, 6, 3.0)
+        alone, _, _ = run_gpu(d, sigma, traj[k:k + 1], 1.0, t0, 6, 3.0, sep_shape=sep_shape)
         assert np.array_equal(alone[0], gm[k]), k
     # y-jitter breaks the mirror symmetry: no pairs, same answers as the oracle
     jit = np.zeros((T, 2), np.float32)
@@ -313,7 +335,7 @@ def test_mirror_pairs_edge_cases():
     assert np.all(P.tno_mf_plan_slots(traj, T, t0, jitter_xy=jit)[3] == 0)
     om_j = oracle.snr_map(f, sigma, traj, 1.0, t0, jitter=jit)
     from paper_2209_09848_b200 import MatchedFilter
-    with MatchedFilter(0) as mf:
+    with MatchedFilter(0, sep_shape=sep_shape) as mf:
         mj, _ = mf.search(d, sigma, traj, 1.0, t0, jitter_xy=jit)
         torch.cuda.synchronize()
         assert mf.stats()[1] == 1
