@@ -15,14 +15,14 @@ from helpers import TOL, check_topk_vs_own_map
 pytestmark = pytest.mark.gpu
 
 
-def _setup(cfg):
+def _setup(cfg, sep_shape=0):
     import torch
     from paper_2209_09848_b200 import MatchedFilter
     assert torch.cuda.is_available()
     dev = torch.device("cuda", 0)
     p = tno_synth.make_params(cfg)
     frames = tno_synth.stack_torch(p, dev)
-    mf = MatchedFilter(0, cfg.topk, cfg.threshold)
+    mf = MatchedFilter(0, cfg.topk, cfg.threshold, sep_shape=sep_shape)
     mf.inject(frames, p.traj[p.src_k], p.src_x, p.src_y, p.src_amp, cfg.prf_sigma, cfg.t0)
     torch.cuda.synchronize()
     return torch, mf, p, frames
@@ -138,7 +138,9 @@ def test_config4_long_sector_sampled_parity():
 
 def test_config5_curved_topk_only():
     cfg = tno_synth.CONFIGS[5]
-    torch, mf, p, frames = _setup(cfg)
+    # the kernel shape the full bank gets by cost (the first), pinned: the 16-trajectory run below is compared with
+    # the full run bit for bit, and the two shapes sum in different orders
+    torch, mf, p, frames = _setup(cfg, sep_shape=1)
     _, cand = mf.search(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0, want_maps=False)
     torch.cuda.synchronize()
     assert mf.stats()[1] == 1
