@@ -36,17 +36,20 @@
 // Structure:
 //   * persistent CTAs, one per SM, walk (tile, batch) work items batch-fastest, so the batches of
 //     one tile run on neighbouring CTAs at the same time and share the frame tiles in L2;
-//   * warp-specialised: one producer warpgroup (56 registers per thread after setmaxnreg) issues
-//     the TMA loads and runs the x-pass, 12 consumer warps (152 registers) run the y-pass; the
-//     roles are linked by mbarrier rings only, there is no CTA-wide barrier in the frame loop;
+//   * warp-specialised: one producer warpgroup (80 or 56 registers per thread after setmaxnreg), each of
+//     whose four warps owns every fourth frame -- it requests the frame's TMA box, runs its whole x-pass and
+//     hands one of its two X buffers to the consumers -- and 12 consumer warps (144 or 152 registers) that run
+//     the y-pass; the roles are linked by mbarrier rings only, there is no barrier among the producers and no
+//     CTA-wide barrier in the frame loop;
 //   * frame tiles of (HT + 4) rows x 76 columns are staged by TMA (cp.async.bulk.tensor.3d, zero
-//     fill outside the frame = "dropped from N") into a ring of box stages together with the
-//     per-(batch, frame) table (cp.async.bulk), completion on mbarriers;
-//   * x-pass: 4 outputs per thread from three 16-byte shared loads; the row pitches (76 and 68
-//     words) make a quarter-warp of 8 rows hit 32 distinct banks on both the loads and the stores;
-//   * y-pass: R rows x 2 columns x NB entries per thread in FP32 registers, packed FFMA2
-//     (fma.rn.f32x2: two columns per instruction), which halves the issue slots of the y-pass and
-//     leaves room for the producer warps on the same schedulers.
+//     fill outside the frame = "dropped from N") together with the per-(batch, frame) table row
+//     (cp.async.bulk), completion on mbarriers;
+//   * x-pass: 8 outputs per thread from four 16-byte shared loads, the next step's loads issued ahead; the row
+//     pitches (76 and 68 words) make a quarter-warp of 8 rows hit 32 distinct banks on both loads and stores;
+//   * y-pass: R positions x 2 columns x NB slots x (E, O) per thread in FP32 registers, packed FFMA2
+//     (fma.rn.f32x2: two columns per instruction, two issue cycles);
+//   * two shapes are compiled (R x NB = 4 x 5 and 5 x 4, tiles of 48 and 60 positions); the host picks one per
+//     search by modelled cost (api.cu).
 #include <algorithm>
 #include <cstdio>
 
