@@ -611,9 +611,20 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         if (in) {
             const int64_t off = (int64_t)y * W + x;
-            for (int32_t c = 0; c < n_pieces; ++c) {
-                const float4 p = __ldcs(reinterpret_cast<const float4 *>(pin + c * piece_stride + off));
-                v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
+            if (n_pieces <= 4) {
+                // the usual case: all loads in flight together, summed in piece order (a missing piece adds +0)
+                float4 p[4];
+#pragma unroll
+                for (int32_t c = 0; c < 4; ++c)
+                    p[c] = c < n_pieces ? __ldcs(reinterpret_cast<const float4 *>(pin + c * piece_stride + off))
+                                        : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int32_t c = 0; c < 4; ++c) { v.x += p[c].x; v.y += p[c].y; v.z += p[c].z; v.w += p[c].w; }
+            } else {
+                for (int32_t c = 0; c < n_pieces; ++c) {
+                    const float4 p = __ldcs(reinterpret_cast<const float4 *>(pin + c * piece_stride + off));
+                    v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
+                }
             }
             if (dpieces) {
                 // masked search: D was accumulated like N, from the validity weights
