@@ -551,9 +551,6 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                                         TNO_CHECK(pp + (int64_t)r * W >= lo && pp + (int64_t)r * W + 1 < lo + a.piece_stride);
                                     if (hm && (uint32_t)(ym + r) < (uint32_t)H)
                                         TNO_CHECK(pm + (int64_t)r * W >= lo && pm + (int64_t)r * W + 1 < lo + a.piece_stride);
-                                    // ... and belongs to a tile row that maps to the same piece: |P - y| = |d| must be
-                                    // smaller than (n_pieces - 1) tile heights
-                                    TNO_CHECK(abs(dq.y) <= (a.n_pieces - 1) * HT || a.n_pieces == 1 && dq.y == 0 || true);
                                 }
 #endif
 #pragma unroll
