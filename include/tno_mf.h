@@ -257,6 +257,25 @@ int tno_mf_inject_ex(tno_mf_ctx *ctx, float *frames, int32_t T, int32_t H, int32
 int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, int32_t W, int32_t box,
                 float *out_max, int32_t *out_argk, float *out_z, tno_mf_cand *out_topk);
 
+/* Z of one score map without any device allocation (the Z(x, y) of tno_mf_best): for callers that
+ * cannot call cudaMalloc -- code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ * tno_mf_best keeps its float64 summed-area tables in a context buffer that grows with cudaMalloc; this call keeps
+ * them in a static device array of the library and enqueues its three kernels on the context's stream, nothing
+ * else: no cudaMalloc, no cudaFree, no allocating library routine, no synchronisation.
+ *   score     DEVICE float32 [H][W] (e.g. out_max of tno_mf_best / tno_mf_search_max).  Read only.
+ *   box       odd, >= 1 (the paper uses 255).
+ *   out_z     DEVICE float32 [H][W], must not alias score.  Bit for bit the out_z of
+ *             tno_mf_best(score as a bank of one map).
+ * Limit: H * W <= 1 048 576 pixels (e.g. 1024 x 1024); the static array is 16 MiB, and every GPU that loads the
+ * library holds it until the process exits.  All calls on a device share the array, whatever their context or
+ * stream: calls that overlap on the GPU race on it -- keep them on one stream or order them with events.  The
+ * array keeps the last call's contents; every call overwrites the H * W entries it reads, so nothing has to be
+ * cleared.  The first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device):
+ * make that call before a graph capture starts.
+ * Errors: EINVAL (NULL or aliased pointers, sizes < 1, H * W beyond the limit -- the text names the limit and
+ * tno_mf_best as the path for larger maps --, even box, device ordinal > 63), ECUDA. */
+int tno_mf_local_z_static(tno_mf_ctx *ctx, const float *score, int32_t H, int32_t W, int32_t box, float *out_z);
+
 /* The search with the max over the filter bank fused into its epilogue ("We take
  * the maximum score across the filter bank, which then tells us the most likely trajectory, along with the score
  * of that trajectory"): everything tno_mf_search_masked does, plus

@@ -66,6 +66,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_flux.argtypes = [vp, vp, i32, i32, i32, vp]
     lib.tno_mf_best.restype = ctypes.c_int
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.tno_mf_local_z_static.restype = ctypes.c_int
+    lib.tno_mf_local_z_static.argtypes = [vp, vp, i32, i32, i32, vp]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
     lib.tno_mf_inject_ex.restype = ctypes.c_int
@@ -335,6 +337,15 @@ def tno_mf_best(ctx, snr, box: int, out_max, out_argk=None, out_z=None, out_topk
             "out_topk is smaller than [n][topk] records of 16 bytes"
         p_top = out_topk.data_ptr()
     _check(_lib.tno_mf_best(ctx, snr.data_ptr(), n, H, W, int(box), ptrs[0], ptrs[1], ptrs[2], p_top), ctx)
+
+
+def tno_mf_local_z_static(ctx, score, box: int, out_z) -> None:
+    """score, out_z: CUDA float32 tensors [H, W] with H * W <= 2**20 (the library's static scratch).  No device
+    allocation; enqueues on the context's stream.  Calls that overlap on the GPU share the scratch and race."""
+    assert score.is_cuda and score.is_contiguous() and score.dim() == 2 and score.element_size() == 4
+    H, W = score.shape
+    assert out_z.is_cuda and out_z.is_contiguous() and out_z.element_size() == 4 and out_z.numel() == H * W
+    _check(_lib.tno_mf_local_z_static(ctx, score.data_ptr(), H, W, int(box), out_z.data_ptr()), ctx)
 
 
 def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float) -> None:

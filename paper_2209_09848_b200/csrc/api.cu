@@ -1255,3 +1255,10 @@ int tno_mf_search_host_max(tno_mf_ctx *ctx, const float *frames_host, const floa
 }
 
 }  // extern "C"
+
+// What an entry point that lives in another file (local_z_static.cu) needs of the opaque context.
+namespace tno {
+CtxView ctx_view(const tno_mf_ctx *ctx) { return CtxView{ctx->stream, ctx->cfg.device}; }
+int ctx_fail(tno_mf_ctx *ctx, int code, const char *text) { return fail(ctx, code, "%s", text); }
+void ctx_set_launches(tno_mf_ctx *ctx, int32_t n) { ctx->last_launches = n; }
+}  // namespace tno

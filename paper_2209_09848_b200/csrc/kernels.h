@@ -137,4 +137,10 @@ void launch_finish(cudaStream_t st, const float *pieces, const float *dpieces, i
                    float *out_snr, uint64_t *maxkeys /* DEVICE [H][W] running (score, ~k) maximum, or NULL */,
                    const TopkSlots &slots);
 
+// ---- api.cu: the opaque context as seen by an entry point in another file (local_z_static.cu) ----
+struct CtxView { cudaStream_t stream; int32_t device; };
+CtxView ctx_view(const tno_mf_ctx *ctx);
+int ctx_fail(tno_mf_ctx *ctx, int code, const char *text);      // sets tno_mf_last_error(ctx), returns code
+void ctx_set_launches(tno_mf_ctx *ctx, int32_t n);              // what tno_mf_last_stats reports
+
 }  // namespace tno
