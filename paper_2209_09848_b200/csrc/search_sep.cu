@@ -239,6 +239,16 @@ __device__ __forceinline__ void red_add_v2_if(bool pred, float *addr, float2 v) 
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// One arrival for the whole (converged) warp: elect.sync picks the lane, no thread index needed.
+__device__ __forceinline__ void mbar_arrive_one(uint32_t bar) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n"
+        "}\n" ::"r"(bar)
+        : "memory");
+}
 
 // x-pass of one thread and step: 8 outputs X(c .. c+7) = sum_i g[i] R(c + O + i) from the 16 staged values
 // R(c .. c+15) of its row (four 16-byte loads), O = 0..3 the offset of the window in the 16-byte aligned box.
@@ -309,7 +319,10 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
     const uint32_t x_empty = x_full + 8 * XR;              //   [XR] X consumed by all consumer warps,
     const uint32_t f_done = x_empty + 8 * XR;              //   [NB] k-th flush of entry e finished by all of them
 
-    const int32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int32_t tid = threadIdx.x, lane = tid & 31;
+    // (through a shuffle the warp index is warp-uniform for the compiler: role tests, row ranges and barrier
+    // addresses derived from it live in uniform registers instead of being recomputed from the thread index)
+    const int32_t warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const int32_t T = a.T, H = a.H, W = a.W;
     const int32_t n_items = ntx * nty * a.n_batches;          // < 2^31 (checked by the host)
 
@@ -424,22 +437,26 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         const int32_t r0 = warp * R;
         int32_t n = 0;
         uint32_t fpar = 0;        // bit s = parity of the number of flushes of slot s so far
-        // this thread's window in X[0] as a shared-window address, kept in a register (not recomputed from the
-        // thread index every frame); the loads below are explicit ld.shared with immediate row offsets
-        uint32_t xw0 = smem_u32(Xbuf + r0 * kXP) + 8u * (uint32_t)lane;
-        asm volatile("" : "+r"(xw0));
+        // The only per-lane quantity a consumer keeps: the byte offset of its two columns, both in a row of X
+        // and in a row of a piece map.  Everything else below (window base, piece base, rows) is the same for
+        // the whole warp and stays in uniform registers; the loads are explicit ld.shared with immediate row
+        // offsets.
+        uint32_t lane8 = 8u * (uint32_t)lane;
+        asm volatile("" : "+r"(lane8));
+        const uint32_t xwu = smem_u32(Xbuf + r0 * kXP);
         for (int32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
             // flush coordinates of the item: the members of the batch have planned indices q_first + (the
-            // offsets in the table), a member's piece map starts at ebase + offset*H*W (this lane's two
-            // columns), and the accumulator row r of this warp holds output row yr0 + r - d (plus member) or
-            // yr0 + r + d (minus member)
+            // offsets in the table), a member's piece map starts at ebase + offset*H*W (column x0 of the tile;
+            // this lane's two columns are lane8 bytes further), and the accumulator row r of this warp holds
+            // output row yr0 + r - d (plus member) or yr0 + r + d (minus member)
             const int32_t b = item % a.n_batches, tile = a.ty0 * ntx + item / a.n_batches;
             const int32_t ty = tile / ntx;
-            const int32_t x = (tile % ntx) * kTileW + 2 * lane;
+            const int32_t x0 = (tile % ntx) * kTileW;
             float *ebase = a.pieces + (int64_t)(ty % a.n_pieces) * a.piece_stride +
-                           (int64_t)(__ldg(a.batch_q + b) - a.q0) * H * W + x;
-            // columns past the frame: make every row test fail
-            const int32_t yr0 = (x < W) ? ty * HT - 2 + r0 : INT32_MIN / 2;
+                           (int64_t)(__ldg(a.batch_q + b) - a.q0) * H * W + x0;
+            // bytes of a row of the tile that lie inside the frame (columns past it are never flushed)
+            const uint32_t wlim = 4u * (uint32_t)min(kTileW, W - x0);
+            const int32_t yr0 = ty * HT - 2 + r0;
             // else: positions without any tap in the frame
             const bool y_active = r0 < min(HT, H + 4 - ty * HT);
 
@@ -459,9 +476,11 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 if (y_active) {
                     // ---------------- y-pass: one register window of X for all slots of the batch, and the
                     // sums and differences of its rows about each of this thread's R positions
-                    const uint32_t xw = xw0 + (uint32_t)xr * (C::XBUF * 4);
+                    const uint32_t xw = xwu + (uint32_t)xr * (C::XBUF * 4) + lane8;
                     TNO_CHECK(xw + (R + 3) * (kXP * 4) + 8 <= smem_u32(Xbuf + (xr + 1) * C::XBUF));   // inside X[xr]
                     TNO_CHECK(hdr23.x >= 1 && hdr23.x <= NB && (hdr23.y >> NB) == 0);
+                    // (the weights of slot 0 are requested before the window, not after the sums that need it)
+                    const float4 wa0 = *reinterpret_cast<const float4 *>(tb);
                     float2 win[R + 4];
 #pragma unroll
                     for (int r = 0; r < R + 4; ++r)
@@ -494,7 +513,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                         // full batch: straight-line code, the weights of slot s + 1 are loaded
                         // before the FFMAs of slot s (the empty asm keeps ptxas from hoisting more
                         // loads than the register budget holds)
-                        float4 wa = *reinterpret_cast<const float4 *>(tb);
+                        float4 wa = wa0;
 #pragma unroll
                         for (int s = 0; s < NB; ++s) {
                             float4 wan = wa;
@@ -508,7 +527,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
 #pragma unroll
                         for (int s = 0; s < NB; ++s)
                             if (s < nfill) {
-                                const float4 wa = *reinterpret_cast<const float4 *>(tb + 8 * s);
+                                const float4 wa = s == 0 ? wa0 : *reinterpret_cast<const float4 *>(tb + 8 * s);
                                 const float w4 = d2v[s];
                                 TNO_FMAS(s)
                             }
@@ -517,7 +536,12 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 }
                 const int32_t fmask = hdr23.y;
                 __syncwarp();
-                if (lane == 0) mbar_arrive(x_empty + 8 * (xr));      // this warp no longer reads X[xr]
+                {
+                    // (the ring position again from the frame counter: nothing is kept across the FFMAs for it)
+                    int32_t n2 = n;
+                    asm volatile("" : "+r"(n2));
+                    mbar_arrive_one(x_empty + 8 * (n2 & (XR - 1)));  // this warp no longer reads X[xr]
+                }
                 if (fmask != 0) {
                     const int32_t fwait = reinterpret_cast<const int32_t *>(th)[10];
                     // ---------------- flush: piece[ty mod NP][member][P -+ d][x] += E +- O, E = O = 0
@@ -537,11 +561,17 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                             if (y_active) {
                                 const int4 dq = *reinterpret_cast<const int4 *>(tb + 8 * s + 4);   // (d_2, d, q+, q-)
                                 const int32_t yp = yr0 - dq.y, ym = yr0 + dq.y;
-                                float *pp = ebase + ((int64_t)dq.z * H + yp) * W;
-                                float *pm = ebase + ((int64_t)dq.w * H + ym) * W;
+                                // (through the empty asm the lane offset is a value of this frame: the addresses
+                                // are formed here from uniform registers, not carried through the frame loop)
+                                uint32_t l8 = lane8;
+                                asm volatile("" : "+r"(l8));
+                                float *pp = reinterpret_cast<float *>(
+                                    reinterpret_cast<char *>(ebase + ((int64_t)dq.z * H + yp) * W) + l8);
+                                float *pm = reinterpret_cast<float *>(
+                                    reinterpret_cast<char *>(ebase + ((int64_t)dq.w * H + ym) * W) + l8);
                                 asm volatile("" : "+l"(pp), "+l"(pm));      // one address each, then += W per row
-                                const bool hp = dq.z >= 0, hm = dq.w >= 0;
-                                TNO_CHECK(dq.z < 2 * NB && dq.w < 2 * NB && (hp || hm));
+                                const bool hp = dq.z >= 0 && l8 < wlim, hm = dq.w >= 0 && l8 < wlim;
+                                TNO_CHECK(dq.z < 2 * NB && dq.w < 2 * NB && (dq.z >= 0 || dq.w >= 0));
                                 TNO_CHECK(__ldg(a.batch_q + b) - a.q0 + max(dq.z, dq.w) < a.piece_stride / ((int64_t)H * W));
 #ifdef TNO_DEBUG_CHECKS
                                 for (int r = 0; r < R; ++r) {
@@ -566,7 +596,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                                 }
                             }
                             __syncwarp();
-                            if (lane == 0) mbar_arrive(f_done + 8 * (s));
+                            mbar_arrive_one(f_done + 8 * (s));
                         }
                     }
                 }
