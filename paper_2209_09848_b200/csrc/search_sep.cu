@@ -112,11 +112,11 @@ constexpr int kPW = 4;       // producer warps (one warpgroup: setmaxnreg is per
 // stage table entry (32-bit words), one per (batch, frame t):
 //   [0] xo = 4*floor((sx - 2)/4), the 16-byte aligned x offset of the staged box relative to the tile
 //   [1] o = sx - 2 - xo in 0..3, the column of the box at which the 5-tap window of output 0 starts
-//   [2] number of slots of the batch (they occupy slots 0 .. n-1)
-//   [3] flush mask: bit s set if slot s must be flushed after this frame
-//   [4..8] gx[0..4]
+//   [2..6] gx[0..4]
+//   [8] number of slots of the batch (they occupy slots 0 .. n-1)
+//   [9] flush mask: bit s set if slot s must be flushed after this frame
 //   [10] wait mask: bit s set if the previous flush of slot s is at most XR frames back
-//   [12..15], [11] d_2 / sigma_t^2 of slots 0..3 and of slot 4 (one 16-byte load + one word)
+//   [11], [12..15] d_2 / sigma_t^2 of slot 4 and of slots 0..3: the consumers read [8..15] with two 16-byte loads
 //   [16 + 8s + 0..4] (w[2], s_1, s_2, d_1, d_2) / sigma_t^2 of slot s (zeros if empty)
 //   [16 + 8s + 5] d_{s,t}    [16 + 8s + 6], [.. + 7] planned-order index of the plus / minus member relative
 //                            to the first one of the batch, -1 = absent
@@ -177,7 +177,7 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
     // squared = 1: the taps of the D pass over the validity weights, sum g^2 V / sigma^2
     for (int i = 0; i < 5; ++i) {
         const double gv = tab.gd[((int64_t)xc * T + t) * 5 + i];
-        out[4 + i] = squared ? (float)(gv * gv) : tab.g[((int64_t)xc * T + t) * 5 + i];
+        out[2 + i] = squared ? (float)(gv * gv) : tab.g[((int64_t)xc * T + t) * 5 + i];
     }
     int32_t n = 0, fmask = 0, fwait = 0;
     for (int e = 0; e < C::NB; ++e) {
@@ -219,8 +219,8 @@ __global__ void k_sep_tables(ClassTables tab, const int32_t *__restrict__ batch_
                 if (tab.shift[ci - t + u + 1] != tab.shift[ci - t + u] || (u + 1 + ph) % kSeg == 0) fwait |= 1 << e;
         }
     }
-    outi[2] = n;
-    outi[3] = fmask;
+    outi[8] = n;
+    outi[9] = fmask;
     outi[10] = fwait;
 }
 
@@ -347,7 +347,8 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         const int32_t pw = warp - CW;
         // position of this warp's next frame to REQUEST (iss_*) and to PROCESS (item, t) in the CTA's
         // sequence of (work item, frame)
-        int32_t iss_item = blockIdx.x, iss_t = pw, iss_k = 0;
+        int32_t iss_item = blockIdx.x, iss_t = pw;
+        uint32_t iss_k = 0;      // (ring counters are unsigned: their divisions and remainders are shifts and masks)
         auto advance = [&](int32_t &it, int32_t &tt) {
             tt += kPW;
             while (tt >= T) { tt -= T; it += gridDim.x; }
@@ -366,7 +367,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             }
             const int32_t b = iss_b;
             const int32_t *row = reinterpret_cast<const int32_t *>(a.stage_tab + ((int64_t)b * T + iss_t) * TABW);
-            const int32_t sb = pw + kPW * (iss_k % BST), n = pw + kPW * iss_k;
+            const uint32_t sb = pw + kPW * (iss_k % BST), n = pw + kPW * iss_k;
             TNO_CHECK(iss_item >= 0 && iss_item < n_items && iss_t >= 0 && iss_t < T && b < a.n_batches);
             TNO_CHECK(sb >= 0 && sb < SB && ((__ldg(row) & 3) == 0) && (uint32_t)__ldg(row + 1) < 4u);
             TNO_CHECK(iss_y0 + 4 < (a.ty0 + nty) * HT && iss_x0 < ntx * kTileW);
@@ -395,21 +396,21 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         // groups per frame.
         const int32_t row_in = lane & 7, oct_in = lane >> 3;
         int32_t cached = -1, xrows = 0;
-        for (int32_t k = 0; item < n_items; ++k) {
+        for (uint32_t k = 0; item < n_items; ++k) {
             if (item != cached) {
                 cached = item;
                 const int32_t Y0 = (a.ty0 + item / a.n_batches / ntx) * HT - 2;
                 // positions P >= H + 2 have no tap inside the frame: the X rows only they would read are skipped
                 xrows = min(HT, (H + 2 - Y0 + R - 1) / R * R) + 4;
             }
-            const int32_t sb = pw + kPW * (k % BST), xb = pw + kPW * (k % XST), n = pw + kPW * k;
+            const uint32_t sb = pw + kPW * (k % BST), xb = pw + kPW * (k % XST), n = pw + kPW * k;
             mbar_wait(full_box + 8 * (sb), (k / BST) & 1);
             if (k >= XST) mbar_wait(x_empty + 8 * (xb), (k / XST + 1) & 1);
             const float *tb = Tab + (n & (TS - 1)) * TABW;
             const int32_t o = reinterpret_cast<const int32_t *>(tb)[1];
             float g[5];
 #pragma unroll
-            for (int i = 0; i < 5; ++i) g[i] = tb[4 + i];
+            for (int i = 0; i < 5; ++i) g[i] = tb[2 + i];
             const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 8 * oct_in;
             float *dst = Xbuf + xb * C::XBUF + row_in * kXP + 8 * oct_in;
             TNO_CHECK(xrows >= 4 + R && xrows <= C::XROWS && (uint32_t)o < 4u && sb < SB);
@@ -435,7 +436,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
         // =============================================================== consumers: y-pass + flush
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::CREGS));
         const int32_t r0 = warp * R;
-        int32_t n = 0;
+        uint32_t n = 0;           // CTA-local frame counter (unsigned: ring positions are shifts and masks)
         uint32_t fpar = 0;        // bit s = parity of the number of flushes of slot s so far
         // The only per-lane quantity a consumer keeps: the byte offset of its two columns, both in a row of X
         // and in a row of a piece map.  Everything else below (window base, piece base, rows) is the same for
@@ -467,12 +468,13 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 for (int i = 0; i < R; ++i) accE[s][i] = accO[s][i] = make_float2(0.f, 0.f);
 
             for (int32_t t = 0; t < T; ++t) {
-                const int32_t xr = n & (XR - 1);
+                const uint32_t xr = n & (XR - 1);
                 mbar_wait(x_full + 8 * (xr), (n / XR) & 1);
                 const float *th = Tab + (n & (TS - 1)) * TABW;
                 const float *tb = th + kHdr;
-                // number of slots and flush mask of the frame, read together ahead of the FFMAs
-                const int2 hdr23 = *reinterpret_cast<const int2 *>(th + 2);
+                // number of slots and flush mask of the frame (and d_2 of slot 4), read together ahead of the FFMAs
+                const int4 hq = *reinterpret_cast<const int4 *>(th + 8);
+                const int2 hdr23 = make_int2(hq.x, hq.y);
                 if (y_active) {
                     // ---------------- y-pass: one register window of X for all slots of the batch, and the
                     // sums and differences of its rows about each of this thread's R positions
@@ -508,7 +510,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
     }
                     // d_2 of all slots: one 16-byte load and one word
                     const float4 d2q = *reinterpret_cast<const float4 *>(th + 12);
-                    const float d2v[5] = {d2q.x, d2q.y, d2q.z, d2q.w, th[11]};
+                    const float d2v[5] = {d2q.x, d2q.y, d2q.z, d2q.w, __int_as_float(hq.w)};
                     if (nfill == NB) {
                         // full batch: straight-line code, the weights of slot s + 1 are loaded
                         // before the FFMAs of slot s (the empty asm keeps ptxas from hoisting more
@@ -538,7 +540,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 __syncwarp();
                 {
                     // (the ring position again from the frame counter: nothing is kept across the FFMAs for it)
-                    int32_t n2 = n;
+                    uint32_t n2 = n;
                     asm volatile("" : "+r"(n2));
                     mbar_arrive_one(x_empty + 8 * (n2 & (XR - 1)));  // this warp no longer reads X[xr]
                 }
