@@ -472,15 +472,15 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                 mbar_wait(x_full + 8 * (xr), (n / XR) & 1);
                 const float *th = Tab + (n & (TS - 1)) * TABW;
                 const float *tb = th + kHdr;
-                // number of slots and flush mask of the frame (and d_2 of slot 4), read together ahead of the FFMAs
-                const int4 hq = *reinterpret_cast<const int4 *>(th + 8);
-                const int2 hdr23 = make_int2(hq.x, hq.y);
+                // number of slots and flush mask of the frame (and d_2 of slot 4), read together ahead of the FFMAs,
+                // but requested after the window: the header's move into uniform registers waits for its load, and
+                // the warp issues in order
+                int4 hq;
                 if (y_active) {
                     // ---------------- y-pass: one register window of X for all slots of the batch, and the
                     // sums and differences of its rows about each of this thread's R positions
                     const uint32_t xw = xwu + (uint32_t)xr * (C::XBUF * 4) + lane8;
                     TNO_CHECK(xw + (R + 3) * (kXP * 4) + 8 <= smem_u32(Xbuf + (xr + 1) * C::XBUF));   // inside X[xr]
-                    TNO_CHECK(hdr23.x >= 1 && hdr23.x <= NB && (hdr23.y >> NB) == 0);
                     // (the weights of slot 0 are requested before the window, not after the sums that need it)
                     const float4 wa0 = *reinterpret_cast<const float4 *>(tb);
                     float2 win[R + 4];
@@ -488,6 +488,9 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                     for (int r = 0; r < R + 4; ++r)
                         asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];"
                                      : "=f"(win[r].x), "=f"(win[r].y) : "r"(xw + (uint32_t)(r * kXP * 4)));
+                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(hq.x), "=r"(hq.y), "=r"(hq.z), "=r"(hq.w) : "r"(smem_u32(th + 8)));
+                    TNO_CHECK(hq.x >= 1 && hq.x <= NB && (hq.y >> NB) == 0);
                     float2 A1[R], B1[R], A2[R], B2[R];
                     const float2 neg1 = make_float2(-1.f, -1.f);
 #pragma unroll
@@ -497,7 +500,7 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                         A2[r] = __fadd2_rn(win[r + 4], win[r]);
                         B2[r] = __ffma2_rn(neg1, win[r], win[r + 4]);
                     }
-                    const int32_t nfill = hdr23.x;
+                    const int32_t nfill = hq.x;
 #define TNO_FMAS(s)                                                                                      \
     {                                                                                                    \
         const float2 w0 = make_float2(wa.x, wa.x), w1 = make_float2(wa.y, wa.y),                         \
@@ -535,8 +538,10 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
                             }
                     }
 #undef TNO_FMAS
+                } else {
+                    hq = *reinterpret_cast<const int4 *>(th + 8);
                 }
-                const int32_t fmask = hdr23.y;
+                const int32_t fmask = hq.y;
                 __syncwarp();
                 {
                     // (the ring position again from the frame counter: nothing is kept across the FFMAs for it)
