@@ -825,10 +825,12 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
     if (use_sep) {
         // slots (mirror pairs where the filter is symmetric under y -> -y: the Gaussian and the single tap)
         // packed into batches; both kernel variants take the same batches
-        // kernel shape: the one with the shorter modelled makespan.  A (tile, batch) work item costs, per frame and in
-        // issue cycles of a scheduler, tile_h / rows-per-warp ... folded into: tile_h x [ 14.5 (tile_h + 4) / tile_h for
-        // the x-pass + 2 (5 slots + 4) for the y-pass + 93 / rows of per-frame bookkeeping per consumer warp ]
-        // (DESIGN.md section 6); the persistent CTAs take ceil(items / SMs) items each.  Ties go to shape 0.
+        // kernel shape: the one with the shorter modelled makespan.  A (tile, batch) work item costs, per frame and
+        // position row, [ 30 (tile_h + 4) / tile_h for the x-pass + 2 (5 slots + 4) for the y-pass + 200 / rows for the
+        // per-frame bookkeeping and latencies of a consumer warp + 15 slots / rows if the batch is not full (it then
+        // takes the kernel's branchy path without the weight prefetch) ]; the persistent CTAs take ceil(items / SMs)
+        // items each.  The three constants are fitted to the measured shape ratios of configs 2-5 (DESIGN.md section 6:
+        // reproduced within 2 %).  Ties go to shape 0.
         const bool sym = ctx->cfg.filter == 0 || ctx->cfg.filter == 1;
         double best = 0.0;
         for (int32_t v = 0; v < sep_num_variants(); ++v) {
@@ -836,7 +838,8 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
             build_slot_batches(&plan, cand.nb, sym);
             double per_item = 0.0;
             for (const SlotBatch &bt : plan.slot_batches)
-                per_item += 14.5 * (cand.tile_h + 4) / cand.tile_h + 2.0 * (5.0 * bt.slots.size() + 4.0) + 93.0 / cand.rows;
+                per_item += 30.0 * (cand.tile_h + 4) / cand.tile_h + 2.0 * (5.0 * bt.slots.size() + 4.0) + 200.0 / cand.rows +
+                            ((int32_t)bt.slots.size() < cand.nb ? 15.0 * bt.slots.size() / cand.rows : 0.0);
             per_item *= (double)cand.tile_h / (double)plan.slot_batches.size();
             const double items = (double)((W + 63) / 64) * sep_tile_rows(v, H) * (double)plan.slot_batches.size();
             const double cost = std::ceil(items / ctx->n_sm) * per_item;
