@@ -138,9 +138,10 @@ def test_config4_long_sector_sampled_parity():
 
 def test_config5_curved_topk_only():
     cfg = tno_synth.CONFIGS[5]
-    # the kernel shape the full bank gets by cost (the first), pinned: the 16-trajectory run below is compared with
-    # the full run bit for bit, and the two shapes sum in different orders
-    torch, mf, p, frames = _setup(cfg, sep_shape=1)
+    # the kernel shape the full bank gets by cost (the second: its 8 or 24 slots per x-motion fill 4-slot batches),
+    # pinned: the 16-trajectory run below is compared with the full run bit for bit, and the two shapes sum in
+    # different orders
+    torch, mf, p, frames = _setup(cfg, sep_shape=2)
     _, cand = mf.search(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0, want_maps=False)
     torch.cuda.synchronize()
     assert mf.stats()[1] == 1
