@@ -47,7 +47,10 @@
 //   * x-pass: 8 outputs per thread from four 16-byte shared loads, the next step's loads issued ahead; the row
 //     pitches (76 and 68 words) make a quarter-warp of 8 rows hit 32 distinct banks on both loads and stores;
 //   * y-pass: R positions x 2 columns x NB slots x (E, O) per thread in FP32 registers, packed FFMA2
-//     (fma.rn.f32x2: two columns per instruction, two issue cycles);
+//     (fma.rn.f32x2: two columns per instruction, two issue cycles); the warp index goes through a shuffle so
+//     that ranges, bases, ring positions and barrier addresses are uniform-datapath values, the only per-lane
+//     register is the byte offset of the thread's two columns, and all shared loads of a frame (header, first
+//     weights, window) are requested together ahead of their first use;
 //   * two shapes are compiled (R x NB = 4 x 5 and 5 x 4, tiles of 48 and 60 positions); the host picks one per
 //     search by modelled cost (api.cu).
 #include <algorithm>
