@@ -49,7 +49,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)
             raise RuntimeError("nvcc failed on " + f)
-    cmd = [nvcc, "-shared", "-o", LIB + ".tmp"] + objs + ["-lcudart_static", "-lpthread", "-ldl", "-lrt"]
+    # (the arch again at the link step: without it nvcc adds an empty device-link stub for its default architecture)
+    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp"] + objs + \
+          ["-lcudart_static", "-lpthread", "-ldl", "-lrt"]
     if host_extra:
         cmd += ["-Xcompiler", ",".join(host_extra.split())]
     subprocess.run(cmd, check=True)
