@@ -408,9 +408,13 @@ k_scatter_fused(const float *__restrict__ D, int32_t T, int32_t N, int32_t n, co
         for (int32_t e = tid; e < FS * n; e += NT) {
             const int32_t f = e % FS, bb = e / FS;
             if (t0 + f < tb) {
-                const float *pr = prow + f * PP + blo[bb], *w = Wt + bb * max_sup;
+                const int32_t lo = blo[bb];
+                const float *pr = prow + f * PP + lo, *w = Wt + bb * max_sup;
+                // only the support [blo, bhi] of the column: past it the weights are zero, but the row is not -- its
+                // pad element is never written, and 0 x (whatever an earlier kernel left there, possibly NaN) is not 0
+                const int32_t ns = min(max_sup, bhi[bb] - lo + 1);
                 float sum = 0.f;
-                for (int32_t c = 0; c < max_sup; ++c) sum = fmaf(w[c], pr[c], sum);      // zero weights past the support
+                for (int32_t c = 0; c < ns; ++c) sum = fmaf(w[c], pr[c], sum);
                 cpart[((int64_t)i * T + (t0 + f)) * n + bb] = sum;
             }
         }

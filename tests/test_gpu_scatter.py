@@ -46,6 +46,35 @@ def test_loss_and_gradient_match_oracle(T, N, n):
     assert np.abs(ggs.cpu().numpy() - gs).max() <= 2e-5 * max(1.0, np.abs(gs).max())
 
 
+def test_gradient_does_not_depend_on_what_earlier_kernels_left_on_chip():
+    """The fused evaluation once multiplied a never-written pad element of its shared staging rows by a zero weight:
+    NaN whenever an earlier kernel had left a NaN bit pattern there.  Repeated calls from fresh contexts, between
+    kernels that fill shared memory with such patterns, must give the same finite gradient every time."""
+    torch = _torch()
+    import paper_2209_09848_b200 as P
+    from paper_2209_09848_b200 import MatchedFilter
+    T, N, n = 9, 512, 32
+    D, jit, beta, S = _problem(T + N + n, T, N, n)
+    rng = np.random.default_rng(1)
+    b0 = (beta + rng.standard_normal(beta.shape)).astype(np.float32)
+    S0 = (S + rng.standard_normal(S.shape)).astype(np.float32)
+    ref = None
+    for rep in range(12):
+        # a sort of all-ones int32 keys goes through shared memory: 0xffffffff is a NaN when read as a float
+        torch.sort(torch.full((1 << 16,), -1, dtype=torch.int32, device="cuda"))
+        with MatchedFilter(0) as mf:
+            d = [torch.from_numpy(a).cuda() for a in (D, b0, S0)]
+            ggb, ggs = torch.full_like(d[1], float("nan")), torch.full_like(d[2], float("nan"))
+            loss = P.tno_mf_scatter_lossgrad(mf.ctx, d[0], jit, 0.8, d[1], d[2], ggb, ggs)
+            torch.cuda.synchronize()
+        a, b = ggb.cpu().numpy(), ggs.cpu().numpy()
+        assert np.isfinite(loss) and np.all(np.isfinite(a)) and np.all(np.isfinite(b)), rep
+        if ref is None:
+            ref = (loss, a, b)
+        else:
+            assert loss == ref[0] and np.array_equal(a, ref[1]) and np.array_equal(b, ref[2]), rep
+
+
 def test_downsample_and_subtract():
     torch = _torch()
     import paper_2209_09848_b200 as P
