@@ -274,6 +274,45 @@ __device__ __forceinline__ void xpass_step(const XIn &u, float *dst, const float
     reinterpret_cast<float4 *>(dst)[0] = make_float4(v[0], v[1], v[2], v[3]);
     reinterpret_cast<float4 *>(dst)[1] = make_float4(v[4], v[5], v[6], v[7]);
 }
+// One frame of one producer warp.  Row groups of 8: a quarter-warp takes 8 rows at one offset of 8 columns (lane & 7 =
+// row, lane >> 3 = octet of columns: 32 distinct banks for the 16-byte loads at pitch 76 and the 16-byte stores at
+// pitch 68), the warp covers 8 rows x 32 columns per step and walks the two halves of each group; the loads of the
+// next step are issued before the arithmetic of the current one (in program order ahead of its stores, which the
+// compiler must assume may alias them).  A last group of m <= 4 rows (the 52 rows of the first kernel shape: m = 4)
+// is done in ONE step with lane & 3 = row and lane >> 2 = octet, all 64 columns: half the instructions of a
+// half-empty group of 8.
+template <int O>
+__device__ __forceinline__ void xpass_frame4(const float *srcb, float *dstb, int32_t lane, int32_t xrows,
+                                            const float (&g)[5]) {
+    const int32_t row_in = lane & 7, oct_in = lane >> 3;
+    const float *src = srcb + row_in * kBoxW + 8 * oct_in;
+    float *dst = dstb + row_in * kXP + 8 * oct_in;
+    const int32_t nfull = xrows >> 3, m = xrows & 7;          // row groups with all 8 rows, rows of the last group
+    const bool tail8 = m > 4 && row_in < m;                   // this lane's row of a last group of 5 .. 7 rows
+    XIn u = xpass_load(src);                    // left half of the current row group
+    for (int32_t i = 0; i < nfull; ++i) {
+        const XIn w = xpass_load(src + 32);     // right half
+        xpass_step<O>(u, dst, g);
+        src += 8 * kBoxW;
+        if (i + 1 < nfull || tail8) u = xpass_load(src);
+        xpass_step<O>(w, dst + 32, g);
+        dst += 8 * kXP;
+    }
+    if (m > 4) {
+        if (tail8) {
+            const XIn w = xpass_load(src + 32);
+            xpass_step<O>(u, dst, g);
+            xpass_step<O>(w, dst + 32, g);
+        }
+    } else if (m > 0) {
+        const int32_t r4 = lane & 3, o8 = lane >> 2;
+        if (r4 < m) {
+            const XIn t = xpass_load(srcb + (8 * nfull + r4) * kBoxW + 8 * o8);
+            xpass_step<O>(t, dstb + (8 * nfull + r4) * kXP + 8 * o8, g);
+        }
+    }
+}
+
 // One frame of one producer warp: this lane's rows row_in, row_in + 8, ... of the box, columns 8 oct_in .. + 7
 // and 32 + 8 oct_in .. + 7.  The loads of the next step are issued before the arithmetic of the current one
 // (in program order ahead of its stores, which the compiler must assume may alias them).
@@ -393,11 +432,6 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             for (int f = 0; f < BST; ++f) advance(ii, tt);
             iss_item = ii; iss_t = tt;
         }
-        // x-pass roles: a quarter-warp takes 8 rows at one offset of 8 columns: 32 distinct banks for the
-        // 16-byte loads (pitch 76) and for the 16-byte stores (pitch 68); the warp covers 8 rows x 32 columns
-        // per step (8 outputs per thread from 16 staged values) and walks 2 halves x ceil(rows / 8) row
-        // groups per frame.
-        const int32_t row_in = lane & 7, oct_in = lane >> 3;
         int32_t cached = -1, xrows = 0;
         for (uint32_t k = 0; item < n_items; ++k) {
             if (item != cached) {
@@ -414,17 +448,30 @@ k_search_sep(const __grid_constant__ CUtensorMap map, const SepArgs a, const int
             float g[5];
 #pragma unroll
             for (int i = 0; i < 5; ++i) g[i] = tb[2 + i];
-            const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 8 * oct_in;
-            float *dst = Xbuf + xb * C::XBUF + row_in * kXP + 8 * oct_in;
             TNO_CHECK(xrows >= 4 + R && xrows <= C::XROWS && (uint32_t)o < 4u && sb < SB);
             TNO_CHECK((xrows + 7) / 8 * 8 * kBoxW <= C::RBUF + 8 * kBoxW);      // loads stay inside the staging ring
-            const int32_t nfull = xrows >> 3;                       // row groups with all 8 rows
-            const bool tail = row_in < (xrows & 7);                 // this lane's row of the last, partial group
-            switch (o) {                                            // uniform across the CTA
-                case 0: xpass_frame<0>(src, dst, nfull, tail, g); break;
-                case 1: xpass_frame<1>(src, dst, nfull, tail, g); break;
-                case 2: xpass_frame<2>(src, dst, nfull, tail, g); break;
-                default: xpass_frame<3>(src, dst, nfull, tail, g); break;
+            if constexpr (C::XROWS % 8 != 0 && C::XROWS % 8 <= 4) {
+                // (the shape whose full tiles end in a group of <= 4 rows: that group in one step)
+                const float *src = Rbuf + sb * C::RBUF;
+                float *dst = Xbuf + xb * C::XBUF;
+                switch (o) {                                        // uniform across the CTA
+                    case 0: xpass_frame4<0>(src, dst, lane, xrows, g); break;
+                    case 1: xpass_frame4<1>(src, dst, lane, xrows, g); break;
+                    case 2: xpass_frame4<2>(src, dst, lane, xrows, g); break;
+                    default: xpass_frame4<3>(src, dst, lane, xrows, g); break;
+                }
+            } else {
+                const int32_t row_in = lane & 7, oct_in = lane >> 3;
+                const float *src = Rbuf + sb * C::RBUF + row_in * kBoxW + 8 * oct_in;
+                float *dst = Xbuf + xb * C::XBUF + row_in * kXP + 8 * oct_in;
+                const int32_t nfull = xrows >> 3;                   // row groups with all 8 rows
+                const bool tail = row_in < (xrows & 7);             // this lane's row of the last, partial group
+                switch (o) {
+                    case 0: xpass_frame<0>(src, dst, nfull, tail, g); break;
+                    case 1: xpass_frame<1>(src, dst, nfull, tail, g); break;
+                    case 2: xpass_frame<2>(src, dst, nfull, tail, g); break;
+                    default: xpass_frame<3>(src, dst, nfull, tail, g); break;
+                }
             }
             __syncwarp();
             if (lane == 0) {
