@@ -276,6 +276,13 @@ int tno_mf_best(tno_mf_ctx *ctx, const float *snr, int32_t n_traj, int32_t H, in
  * tno_mf_best as the path for larger maps --, even box, device ordinal > 63), ECUDA. */
 int tno_mf_local_z_static(tno_mf_ctx *ctx, const float *score, int32_t H, int32_t W, int32_t box, float *out_z);
 
+/* Debug aid: fill the shared memory of every SM of the context's device with `pattern` (one kernel on the context's
+ * stream that takes all the shared memory of an SM, a few waves of blocks).  Shared memory is not cleared between
+ * kernels; a kernel that reads a word it never wrote computes with what an earlier kernel left there.  The GPU tests
+ * call this with 0xffffffff (a NaN as a float) before every test, which turns such a read into a visible error --
+ * what compute-sanitizer's initcheck would report.  No effect on results.  Errors: EINVAL (NULL ctx), ECUDA. */
+int tno_mf_debug_poison_shared(tno_mf_ctx *ctx, uint32_t pattern);
+
 /* The search with the max over the filter bank fused into its epilogue ("We take
  * the maximum score across the filter bank, which then tells us the most likely trajectory, along with the score
  * of that trajectory"): everything tno_mf_search_masked does, plus

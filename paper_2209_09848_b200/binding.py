@@ -68,6 +68,8 @@ def _load() -> ctypes.CDLL:
     lib.tno_mf_best.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.tno_mf_local_z_static.restype = ctypes.c_int
     lib.tno_mf_local_z_static.argtypes = [vp, vp, i32, i32, i32, vp]
+    lib.tno_mf_debug_poison_shared.restype = ctypes.c_int
+    lib.tno_mf_debug_poison_shared.argtypes = [vp, ctypes.c_uint32]
     lib.tno_mf_inject.restype = ctypes.c_int
     lib.tno_mf_inject.argtypes = [vp, vp, i32, i32, i32, vp, i32, f32, f32]
     lib.tno_mf_inject_ex.restype = ctypes.c_int
@@ -346,6 +348,11 @@ def tno_mf_local_z_static(ctx, score, box: int, out_z) -> None:
     H, W = score.shape
     assert out_z.is_cuda and out_z.is_contiguous() and out_z.element_size() == 4 and out_z.numel() == H * W
     _check(_lib.tno_mf_local_z_static(ctx, score.data_ptr(), H, W, int(box), out_z.data_ptr()), ctx)
+
+
+def tno_mf_debug_poison_shared(ctx, pattern: int = 0xFFFFFFFF) -> None:
+    """Fill the shared memory of every SM with `pattern` (default: a NaN as a float); see include/tno_mf.h."""
+    _check(_lib.tno_mf_debug_poison_shared(ctx, int(pattern) & 0xFFFFFFFF), ctx)
 
 
 def tno_mf_inject(ctx, frames, sources: np.ndarray, prf_sigma: float, t0: float) -> None:

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtno_mf.so")
 CU = ["api.cu", "tables.cu", "search_generic.cu", "search_sep.cu", "topk.cu", "inject.cu", "best.cu", "background.cu", "scatter.cu",
-      "local_z_static.cu"]
+      "local_z_static.cu", "debug.cu"]
 CPP = ["plan.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "--fmad=true", "-Xcompiler", "-fPIC,-O2,-ffp-contract=off", "-Xptxas", "-v"]
