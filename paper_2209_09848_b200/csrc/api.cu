@@ -74,6 +74,14 @@ int fail(tno_mf_ctx *ctx, int code, const char *fmt, ...) {
                         "%s: %s", #expr, cudaGetErrorString(e_));                           \
     } while (0)
 
+// Debug aid (environment variable TNO_MF_POISON_WORKSPACE=1): every workspace buffer is filled with 0xff bytes -- NaN
+// as floats, -1 as integers -- when it is allocated, so that a kernel that reads workspace it never wrote shows in the
+// tests instead of computing with whatever the allocator handed out (profiles/r2_sanitizers.md).
+bool poison_workspace() {
+    static const bool on = [] { const char *v = getenv("TNO_MF_POISON_WORKSPACE"); return v && v[0] == '1'; }();
+    return on;
+}
+
 // Grow-only buffer.  cudaFree synchronises the device, so replacing a buffer that earlier work on
 // the stream may still read is safe.
 int reserve(tno_mf_ctx *ctx, DevBuf &b, size_t bytes) {
@@ -91,9 +99,13 @@ int reserve(tno_mf_ctx *ctx, DevBuf &b, size_t bytes) {
                         cudaGetErrorString(e));
         }
         b.cap = bytes;
-        return TNO_MF_OK;
+    } else {
+        b.cap = want;
     }
-    b.cap = want;
+    if (poison_workspace()) {
+        cudaMemset(b.p, 0xff, b.cap);
+        cudaDeviceSynchronize();
+    }
     return TNO_MF_OK;
 }
 
