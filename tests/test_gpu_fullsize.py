@@ -66,6 +66,17 @@ def _fullsize_with_maps(cfg, n_crop_traj, n_random, n_whole):
     torch.cuda.synchronize()
     assert mf.stats()[1] == 1, "the separable TMA kernel must be the one bench.py times"
     c = mf.candidates_to_numpy(cand)
+    # the same search from a second context (fresh workspace, shared memory poisoned in between): the same bits at every
+    # pixel of every map -- a lost or reordered partial sum anywhere in the launch bench.py times would show
+    if cfg.n_traj * cfg.H * cfg.W * 4 <= 4 << 30:
+        import paper_2209_09848_b200 as P
+        from paper_2209_09848_b200 import MatchedFilter
+        with MatchedFilter(0, cfg.topk, cfg.threshold) as mf2:
+            P.tno_mf_debug_poison_shared(mf2.ctx)
+            maps2, cand2 = mf2.search(frames, p.sigma_t, p.traj, cfg.prf_sigma, cfg.t0)
+            torch.cuda.synchronize()
+            assert torch.equal(maps2, maps) and torch.equal(cand2, cand)
+            del maps2, cand2
     host = frames.cpu().numpy()
     del frames
     rng = np.random.default_rng(cfg.seed)
