@@ -65,3 +65,50 @@ def test_calls_on_a_user_stream_match_the_default_stream():
     for name in ref:
         assert np.array_equal(ref[name], out[name], equal_nan=True), name
     assert np.all(np.isfinite(out["maps"])) and np.all(np.isfinite(out["gs"]))
+
+
+def test_two_contexts_on_two_streams_are_independent():
+    """include/tno_mf.h: "distinct contexts are independent".  Two contexts on two non-blocking streams, different banks
+    and stacks, their calls issued alternately without any synchronisation, against each run alone."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2209_09848_b200 import MatchedFilter
+    rng = np.random.default_rng(9)
+    T, H, W = 40, 192, 256
+    fa = torch.from_numpy(rng.standard_normal((T, H, W)).astype(np.float32)).cuda()
+    fb = torch.from_numpy(rng.standard_normal((T, H, W)).astype(np.float32)).cuda()
+    sigma = np.ones(T, np.float32)
+    ta = np.array([[0.1, -0.2, 0, 0], [0.1, 0.2, 0, 0], [-0.3, 0.05, 0, 0]], np.float32)
+    tb = np.array([[0.25, 0.3, 0, 0], [0.25, -0.3, 0, 0], [0.25, 0.1, 0, 0.002], [0.0, 0.0, 0, 0]], np.float32)
+
+    def alone(f, tr):
+        with MatchedFilter(0, 5, 2.0) as mf:
+            maps, top = mf.search(f, sigma, tr, 1.0, T / 2.0)
+            mx, ak, z, _ = mf.best(maps, 9)
+            torch.cuda.synchronize()
+            return [t.cpu().numpy() for t in (maps, top, mx, ak, z)]
+
+    ra, rb = alone(fa, ta), alone(fb, tb)
+    torch.cuda.synchronize()
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(sa):
+        ma = MatchedFilter(0, 5, 2.0)
+    with torch.cuda.stream(sb):
+        mb = MatchedFilter(0, 5, 2.0)
+    outs_a, outs_b = [], []
+    for rep in range(3):                                   # alternately, nothing waits for anything
+        with torch.cuda.stream(sa):
+            maps, top = ma.search(fa, sigma, ta, 1.0, T / 2.0)
+            outs_a.append((maps, top) + ma.best(maps, 9)[:3])
+        with torch.cuda.stream(sb):
+            maps, top = mb.search(fb, sigma, tb, 1.0, T / 2.0)
+            outs_b.append((maps, top) + mb.best(maps, 9)[:3])
+    sa.synchronize()
+    sb.synchronize()
+    for outs, ref in ((outs_a, ra), (outs_b, rb)):
+        for o in outs:
+            for t, r in zip(o, ref):
+                assert np.array_equal(t.cpu().numpy(), r)
+    ma.close()
+    mb.close()
