@@ -24,11 +24,15 @@ def _poisoned_shared_memory(request):
     if request.node.get_closest_marker("gpu") is not None:
         import torch
         if torch.cuda.is_available():
+            import warnings
             import paper_2209_09848_b200 as P
-            ctx = P.tno_mf_create(0, None, 0, 0.0)
             try:
-                P.tno_mf_debug_poison_shared(ctx)
-                torch.cuda.synchronize()
-            finally:
-                P.tno_mf_destroy(ctx)
+                ctx = P.tno_mf_create(0, None, 0, 0.0)
+                try:
+                    P.tno_mf_debug_poison_shared(ctx)
+                    torch.cuda.synchronize()
+                finally:
+                    P.tno_mf_destroy(ctx)
+            except P.TnoMfError as e:         # a debugging aid must not take the tests down with it
+                warnings.warn("shared memory not poisoned before this test: %s" % e)
     yield
