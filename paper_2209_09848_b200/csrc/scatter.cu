@@ -740,33 +740,52 @@ k_pair(const float *__restrict__ xn, const float *__restrict__ x, const float *_
     last_block_reduce(sy, yy, 1, partials, ticket, kStore0, 0, sc);
 }
 
-// VEC: four neighbouring pixels per thread (W % 4 == 0, 16-byte aligned frames)
+// VEC: four neighbouring pixels of four rows (y, y + 4, y + 8, y + 12) per thread (W % 4 == 0, 16-byte aligned frames):
+// the four 16-byte loads of the frame are requested before the stencil arithmetic, which keeps enough bytes in flight
+// per SM for an in-place stream; the column stencil is looked up once for the four rows
 template <bool VEC>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 k_scatter_subtract(float *__restrict__ frames, int32_t H, int32_t W, const float *__restrict__ S, int32_t n,
                    const int32_t *__restrict__ yi0, const float *__restrict__ yw, const int32_t *__restrict__ xi0,
                    const float *__restrict__ xw) {
-    constexpr int PX = VEC ? 4 : 1;
-    const int32_t x = (blockIdx.x * 64 + (threadIdx.x & 63)) * PX, y = blockIdx.y * 4 + (threadIdx.x >> 6), t = blockIdx.z;
+    constexpr int PX = VEC ? 4 : 1, RW = VEC ? 4 : 1;
+    const int32_t x = (blockIdx.x * 64 + (threadIdx.x & 63)) * PX, y = blockIdx.y * (4 * RW) + (threadIdx.x >> 6),
+                  t = blockIdx.z;
     if (x >= W || y >= H) return;
-    const int32_t i0 = yi0[y], i1 = min(i0 + 1, n - 1);
-    const float wy = yw[y];
-    const float *r0 = S + (int64_t)t * n * n + i0 * n, *r1 = S + (int64_t)t * n * n + i1 * n;
-    float u[PX];
+    float *p = frames + ((int64_t)t * H + y) * W + x;
+    float4 v[RW];
+    if (VEC) {
+#pragma unroll
+        for (int r = 0; r < RW; ++r)
+            if (y + 4 * r < H) v[r] = __ldcs(reinterpret_cast<const float4 *>(p + (int64_t)4 * r * W));
+    }
+    int32_t j0[PX], j1[PX];
+    float wx[PX];
 #pragma unroll
     for (int k = 0; k < PX; ++k) {
-        const int32_t j0 = xi0[x + k], j1 = min(j0 + 1, n - 1);
-        const float wx = xw[x + k];
-        u[k] = (1.f - wy) * ((1.f - wx) * __ldg(r0 + j0) + wx * __ldg(r0 + j1)) +
-               wy * ((1.f - wx) * __ldg(r1 + j0) + wx * __ldg(r1 + j1));
+        j0[k] = xi0[x + k];
+        j1[k] = min(j0[k] + 1, n - 1);
+        wx[k] = xw[x + k];
     }
-    float *p = frames + ((int64_t)t * H + y) * W + x;
-    if (VEC) {
-        float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
-        v.x -= u[0]; v.y -= u[1]; v.z -= u[2]; v.w -= u[3];
-        __stcs(reinterpret_cast<float4 *>(p), v);
-    } else {
-        p[0] -= u[0];
+#pragma unroll
+    for (int r = 0; r < RW; ++r) {
+        const int32_t yr = y + 4 * r;
+        if (yr >= H) break;
+        const int32_t i0 = yi0[yr], i1 = min(i0 + 1, n - 1);
+        const float wy = yw[yr];
+        const float *r0 = S + (int64_t)t * n * n + i0 * n, *r1 = S + (int64_t)t * n * n + i1 * n;
+        float u[PX];
+#pragma unroll
+        for (int k = 0; k < PX; ++k)
+            u[k] = (1.f - wy) * ((1.f - wx[k]) * __ldg(r0 + j0[k]) + wx[k] * __ldg(r0 + j1[k])) +
+                   wy * ((1.f - wx[k]) * __ldg(r1 + j0[k]) + wx[k] * __ldg(r1 + j1[k]));
+        if (VEC) {
+            float4 w = v[r];
+            w.x -= u[0]; w.y -= u[PX > 1 ? 1 : 0]; w.z -= u[PX > 2 ? 2 : 0]; w.w -= u[PX > 3 ? 3 : 0];
+            __stcs(reinterpret_cast<float4 *>(p + (int64_t)4 * r * W), w);
+        } else {
+            p[0] -= u[0];
+        }
     }
 }
 
@@ -778,7 +797,7 @@ void launch_downsample(cudaStream_t st, const float *frames, int32_t T, int32_t 
 void launch_scatter_subtract(cudaStream_t st, float *frames, int32_t T, int32_t H, int32_t W, const float *S, int32_t n,
                              const int32_t *yi0, const float *yw, const int32_t *xi0, const float *xw) {
     if (W % 4 == 0 && (reinterpret_cast<uintptr_t>(frames) & 15u) == 0) {
-        dim3 grid((unsigned)((W / 4 + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)T);
+        dim3 grid((unsigned)((W / 4 + 63) / 64), (unsigned)((H + 15) / 16), (unsigned)T);
         k_scatter_subtract<true><<<grid, 256, 0, st>>>(frames, H, W, S, n, yi0, yw, xi0, xw);
     } else {
         dim3 grid((unsigned)((W + 63) / 64), (unsigned)((H + 3) / 4), (unsigned)T);
