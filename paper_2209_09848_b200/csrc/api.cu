@@ -890,7 +890,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         qf[t] = (float)qd[t];
     }
     std::vector<TrajInfo> tinfo(n_traj);
-    int64_t rsd_total = 0, max_cells = 0;
+    int64_t rsd_total = 0, max_tiles = 0;               // (16 x 16 tiles of border cells: k_rsd_tables)
     for (int32_t k = 0; k < n_traj; ++k) {
         TrajInfo &ti = tinfo[k];
         ti.xc = plan.traj_xc[k];
@@ -900,7 +900,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
         ti.rsd_off = rsd_total;
         const int64_t cells = (int64_t)ti.bx.n * ti.by.n;
         rsd_total += cells;
-        max_cells = std::max(max_cells, cells);
+        max_tiles = std::max(max_tiles, (int64_t)((ti.bx.n + 15) / 16) * ((ti.by.n + 15) / 16));
     }
     // planned order q: batches in order, slots in order, plus member before minus member
     int32_t n_batches = 0;
@@ -1018,7 +1018,7 @@ static int search_core(tno_mf_ctx *ctx, const float *frames, const float *valid,
                         static_cast<float *>(ctx->g.p), static_cast<double *>(ctx->gd.p));
     launch_border_tables(st, tab.shift, tab.gd, tab.qd, reinterpret_cast<const AxisBorder *>(meta + o_bd), d_off,
                          n_cls, n_x, max_n, T, W, H, static_cast<double *>(ctx->ab.p));
-    launch_rsd_tables(st, d_ti, n_traj, max_cells, static_cast<const double *>(ctx->ab.p), d_off, n_x, T, d_rsd);
+    launch_rsd_tables(st, d_ti, n_traj, max_tiles, static_cast<const double *>(ctx->ab.p), d_off, n_x, T, d_rsd);
     ctx->last_launches += 3;
     CU_TRY(ctx, cudaGetLastError());
 

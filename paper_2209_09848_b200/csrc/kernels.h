@@ -16,7 +16,7 @@ void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a
 void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *gd, const double *qd,
                           const AxisBorder *border, const int64_t *off, int32_t n_cls, int32_t n_x,
                           int32_t max_n, int32_t T, int32_t W, int32_t H, double *out);
-void launch_rsd_tables(cudaStream_t st, const TrajInfo *traj, int32_t n_traj, int64_t max_cells,
+void launch_rsd_tables(cudaStream_t st, const TrajInfo *traj, int32_t n_traj, int64_t max_tiles,
                        const double *ab, const int64_t *off, int32_t n_x, int32_t T, float *rsd);
 
 // ---- search_generic.cu ----

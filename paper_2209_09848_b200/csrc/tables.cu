@@ -70,29 +70,37 @@ __global__ void k_border_tables(const int32_t *__restrict__ shift, const double 
 }
 
 // rsd[k][cy][cx] = 1 / sqrt(sum_t AX[xc][t][cx] * AY[yc][t][cy])   (0 where the sum is 0)
-// Eight neighbouring lanes share a cell: lane j sums the frames t = j (mod 8) in frame order, the eight partial sums
-// are added pairwise by a butterfly (the same order for every cell and run).  One thread per cell was a chain of T
-// dependent loads and multiply-adds on the few trajectories with the most border classes: 0.27 ms at T = 1000.
-__global__ void k_rsd_tables(const TrajInfo *__restrict__ traj, const double *__restrict__ ab,
-                             const int64_t *__restrict__ off, int32_t n_x, int32_t T,
-                             float *__restrict__ rsd) {
+// A small contraction over t per trajectory.  One block per 16 x 16 tile of border cells: the 16 columns of AX and
+// the 16 columns of AY the tile needs are staged in shared memory, kRsdFrames frames at a time, and every thread sums
+// its cell in frame order.  (One thread per cell reading global memory re-read every AX and AY value once per cell:
+// 0.27 ms at T = 1000, bound by L1/L2 traffic.)
+constexpr int kRsdTile = 16, kRsdFrames = 32;
+__global__ void __launch_bounds__(kRsdTile * kRsdTile)
+k_rsd_tables(const TrajInfo *__restrict__ traj, const double *__restrict__ ab, const int64_t *__restrict__ off,
+             int32_t n_x, int32_t T, float *__restrict__ rsd) {
+    __shared__ double sx[kRsdFrames][kRsdTile], sy[kRsdFrames][kRsdTile];
     const TrajInfo ti = traj[blockIdx.y];
     const int32_t ncx = ti.bx.n, ncy = ti.by.n;
-    const int64_t n_cells = (int64_t)ncx * ncy;
-    if ((int64_t)blockIdx.x * (blockDim.x >> 3) >= n_cells) return;           // whole block past the last cell
-    const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t id = min(gid >> 3, n_cells - 1);                             // (idle lanes repeat the last cell)
-    const int32_t sub = (int32_t)(gid & 7);
-    const int32_t cy = (int32_t)(id / ncx), cx = (int32_t)(id % ncx);
-    const double *ax = ab + off[ti.xc] + cx;
-    const double *ay = ab + off[n_x + ti.yc] + cy;
+    const int32_t tiles_x = (ncx + kRsdTile - 1) / kRsdTile;
+    const int32_t cx0 = (int32_t)(blockIdx.x % tiles_x) * kRsdTile, cy0 = (int32_t)(blockIdx.x / tiles_x) * kRsdTile;
+    if (cy0 >= ncy) return;                                   // (block-uniform) the grid is sized for the largest table
+    const int32_t tid = threadIdx.x, lx = tid % kRsdTile, ly = tid / kRsdTile;
+    const double *ax = ab + off[ti.xc];
+    const double *ay = ab + off[n_x + ti.yc];
     double D = 0.0;
-#pragma unroll 4
-    for (int32_t t = sub; t < T; t += 8) D += __ldg(ax + (int64_t)t * ncx) * __ldg(ay + (int64_t)t * ncy);
-    D += __shfl_xor_sync(0xffffffffu, D, 1);
-    D += __shfl_xor_sync(0xffffffffu, D, 2);
-    D += __shfl_xor_sync(0xffffffffu, D, 4);
-    if (sub == 0 && (gid >> 3) < n_cells) rsd[ti.rsd_off + id] = (D > 0.0) ? (float)(1.0 / sqrt(D)) : 0.0f;
+    for (int32_t t0 = 0; t0 < T; t0 += kRsdFrames) {
+        for (int32_t i = tid; i < kRsdFrames * kRsdTile; i += kRsdTile * kRsdTile) {
+            const int32_t t = t0 + i / kRsdTile, c = i % kRsdTile;
+            sx[i / kRsdTile][c] = (t < T && cx0 + c < ncx) ? __ldg(ax + (int64_t)t * ncx + cx0 + c) : 0.0;
+            sy[i / kRsdTile][c] = (t < T && cy0 + c < ncy) ? __ldg(ay + (int64_t)t * ncy + cy0 + c) : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int32_t tt = 0; tt < kRsdFrames; ++tt) D += sx[tt][lx] * sy[tt][ly];     // (frames past T add 0 * 0)
+        __syncthreads();
+    }
+    if (cx0 + lx < ncx && cy0 + ly < ncy)
+        rsd[ti.rsd_off + (int64_t)(cy0 + ly) * ncx + cx0 + lx] = (D > 0.0) ? (float)(1.0 / sqrt(D)) : 0.0f;
 }
 
 void launch_class_tables(cudaStream_t st, const float *cls_v, const float *cls_a, const float *times,
@@ -112,10 +120,10 @@ void launch_border_tables(cudaStream_t st, const int32_t *shift, const double *g
     k_border_tables<<<grid, 256, 0, st>>>(shift, gd, qd, border, off, n_x, T, W, H, out);
 }
 
-void launch_rsd_tables(cudaStream_t st, const TrajInfo *traj, int32_t n_traj, int64_t max_cells,
+void launch_rsd_tables(cudaStream_t st, const TrajInfo *traj, int32_t n_traj, int64_t max_tiles,
                        const double *ab, const int64_t *off, int32_t n_x, int32_t T, float *rsd) {
-    dim3 grid((unsigned)((max_cells + 15) / 16), (unsigned)n_traj);       // 16 cells x 8 lanes per block
-    k_rsd_tables<<<grid, 128, 0, st>>>(traj, ab, off, n_x, T, rsd);
+    dim3 grid((unsigned)max_tiles, (unsigned)n_traj);          // max_tiles: 16 x 16 tiles of the largest table
+    k_rsd_tables<<<grid, kRsdTile * kRsdTile, 0, st>>>(traj, ab, off, n_x, T, rsd);
 }
 
 }  // namespace tno
