@@ -741,7 +741,9 @@ k_finish(const float *__restrict__ pieces, const float *__restrict__ dpieces, in
                 atomicMax(maxkeys + off + 3, make_key(v.w, (uint32_t)k));
             }
         }
-        if (want_topk) {
+        // (one vote per warp and row group: most groups hold no candidate, and the four ballots below are skipped)
+        if (want_topk &&
+            __any_sync(0xffffffffu, in && fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w)) >= slots.threshold)) {
             const uint32_t pix = (uint32_t)(y * W + x);
             const float thr = slots.threshold;
             warp_push(in && v.x >= thr, make_key(v.x, pix), list, &count, lane);
